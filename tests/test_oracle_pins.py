@@ -1,0 +1,473 @@
+"""Pins for the float64 oracle (no GPU): closed forms, brute force, library
+routines, invariants and the values the paper prints.  P-numbers refer to
+SURVEY.md §8(c) / DESIGN.md "What pins each part of the oracle".
+A plausible mistake anywhere in oracle/ (dropped term, wrong sign or index,
+transposed operand) must fail at least one of these.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import scipy.signal
+
+import oracle
+import workloads
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _golden():
+    out = {}
+    for line in open(os.path.join(HERE, "golden", "paper_values.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = float(line[1])
+    return out
+
+
+def _rand_filters(rng, n, dmax=40, tau=(3.0, 60.0)):
+    t = rng.uniform(*tau, size=n)
+    w = rng.uniform(0.01, 1.5, size=n)
+    a = np.exp(-1.0 / t + 1j * w).astype(np.complex64)
+    b = ((rng.standard_normal(n) + 1j * rng.standard_normal(n)) / math.sqrt(2)).astype(np.complex64)
+    d = rng.integers(0, dmax + 1, size=n).astype(np.int32)
+    return a, b, d
+
+
+# ---- P1: single-filter impulse response is b a^(k-d) after the delay --------
+def test_p1_impulse_response_closed_form():
+    a = np.array([np.exp(-1 / 50.0 + 0.3j)], np.complex64)
+    b = np.array([0.7 - 0.2j], np.complex64)
+    d = np.array([17], np.int32)
+    x = np.zeros(400)
+    x[0] = 1.0
+    y = oracle.band_sum(x, a, b, d)
+    k = np.arange(400)
+    a64, b64 = complex(a[0]), complex(b[0])
+    want = np.where(k >= 17, b64 * a64 ** np.maximum(k - 17, 0), 0.0)
+    assert np.all(y[:17] == 0)
+    np.testing.assert_allclose(y, want, rtol=0, atol=1e-13)
+
+
+# ---- P2: tiny bank == direct convolution with truncated impulse responses ---
+def test_p2_bank_equals_direct_convolution():
+    rng = np.random.default_rng(2)
+    n = 300
+    x = rng.standard_normal(n)
+    for nf in (1, 3, 5):
+        a, b, d = _rand_filters(rng, nf)
+        s = oracle.band_sum(x, a, b, d)
+        h = np.zeros(n, complex)
+        for l in range(nf):
+            kk = np.arange(n - d[l])
+            h[d[l]:] += complex(b[l]) * complex(a[l]) ** kk
+        want = np.array([np.sum(h[:m + 1][::-1] * x[:m + 1]) for m in range(n)])
+        np.testing.assert_allclose(s, want, rtol=0, atol=1e-11)
+
+
+# ---- the recursion reduces to scipy.signal.lfilter (library routine) --------
+def test_recursion_equals_scipy_lfilter():
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal(500)
+    a, b, d = _rand_filters(rng, 4)
+    want = np.zeros(500, complex)
+    for l in range(4):
+        xd = np.concatenate([np.zeros(d[l]), x])[:500]
+        want += scipy.signal.lfilter([complex(b[l])], [1.0, -complex(a[l])], xd)
+    np.testing.assert_allclose(oracle.band_sum(x, a, b, d), want, rtol=0, atol=1e-11)
+
+
+# ---- P3: closed-form noise variance used by the generator -------------------
+def test_p3_noise_variance_closed_form_and_normalisation():
+    from workloads.gen import _noise_variance
+    rng = np.random.default_rng(4)
+    a, b, d = _rand_filters(rng, 6, dmax=30, tau=(3.0, 25.0))
+    n = 4000
+    h = np.zeros(n, complex)
+    for l in range(6):
+        h[d[l]:] += complex(b[l]) * complex(a[l]) ** np.arange(n - d[l])
+    V = _noise_variance(a.astype(complex)[None], b.astype(complex)[None], d[None])[0]
+    assert abs(V - np.sum(np.abs(h) ** 2)) < 1e-9 * V
+    # generated banks are scaled to E|z|^2 = 2 (A8): measure it through the oracle
+    bank = workloads.random_bank(np.random.default_rng(5), 6, 24, [2048], tau_range=(5.0, 60.0), max_delay=100)
+    x = np.random.default_rng(6).standard_normal((1, 60000)).astype(np.float32)
+    z = oracle.filter_bank(x, bank)[0]
+    m = np.mean(np.abs(z[:, 2000:]) ** 2)
+    assert abs(m - 2.0) < 0.12
+
+
+# ---- P4: linearity and shift invariance -------------------------------------
+def test_p4_linearity_and_shift():
+    rng = np.random.default_rng(7)
+    a, b, d = _rand_filters(rng, 5)
+    x1, x2 = rng.standard_normal(256), rng.standard_normal(256)
+    z1, z2 = oracle.band_sum(x1, a, b, d), oracle.band_sum(x2, a, b, d)
+    z12 = oracle.band_sum(2.5 * x1 - 0.75 * x2, a, b, d)
+    np.testing.assert_allclose(z12, 2.5 * z1 - 0.75 * z2, atol=1e-12)
+    xs = np.concatenate([np.zeros(13), x1])[:256]
+    zs = oracle.band_sum(xs, a, b, d)
+    np.testing.assert_allclose(zs[13:], z1[:-13], atol=1e-13)
+    assert np.all(zs[:13] == 0)
+
+
+# ---- P5: decimator / interpolator reduce to scipy routines ------------------
+def test_p5_decimator_is_lfilter_odd_phase():
+    dec, itp = workloads.halfband_taps()
+    rng = np.random.default_rng(8)
+    x = rng.standard_normal(1024)
+    y = oracle.decimate(x, dec.astype(np.float64))
+    want = scipy.signal.lfilter(dec.astype(np.float64), 1.0, x)[1::2]
+    np.testing.assert_allclose(y, want, atol=1e-13)
+    assert abs(np.sum(dec.astype(np.float64) ** 2) - 1.0) < 1e-6      # M2 noise gain
+    assert abs(np.sum(itp.astype(np.float64)) - 2.0) < 1e-6           # M4 DC gain after zero-stuffing
+
+
+def test_p5_interpolator_is_upfirdn():
+    dec, itp = workloads.halfband_taps()
+    rng = np.random.default_rng(9)
+    acc = rng.standard_normal(200) + 1j * rng.standard_normal(200)
+    s = rng.standard_normal(400) + 1j * rng.standard_normal(400)
+    got = oracle.interp_add(acc, itp.astype(np.float64), s)
+    want = scipy.signal.upfirdn(itp.astype(np.float64), acc, up=2)[:400] + s
+    np.testing.assert_allclose(got, want, atol=1e-12)
+    got0 = oracle.interp_add(acc, itp.astype(np.float64), None)
+    np.testing.assert_allclose(got0, want - s, atol=1e-12)
+
+
+def _small_multirate_bank(rng, T=3, L=8, rates=(4096, 2048, 1024, 512), out_band=1):
+    return workloads.random_bank(rng, T, L, list(rates), out_band, tau_range=(4.0, 40.0), max_delay=30)
+
+
+# ---- multirate composition written out with scipy (M1-M5 restated) ----------
+def test_multirate_bank_equals_scipy_composition():
+    rng = np.random.default_rng(10)
+    dec, itp = workloads.halfband_taps()
+    bank = _small_multirate_bank(rng)
+    x = rng.standard_normal((1, 2048)).astype(np.float32)
+    z = oracle.filter_bank(x, bank, dec, itp)[0]
+    g, h = dec.astype(np.float64), itp.astype(np.float64)
+    xb = [x[0].astype(np.float64)]
+    for _ in range(3):
+        xb.append(scipy.signal.lfilter(g, 1.0, xb[-1])[1::2])
+    for t in range(3):
+        sl = slice(bank["tmpl_offset"][t], bank["tmpl_offset"][t + 1])
+        a, b, d, bd = bank["a"][sl], bank["b"][sl], bank["delay"][sl], bank["band"][sl]
+        s = []
+        for bnd in range(4):
+            m = bd == bnd
+            sb = np.zeros(len(xb[bnd]), complex)
+            for l in np.nonzero(m)[0]:
+                xd = np.concatenate([np.zeros(d[l]), xb[bnd]])[:len(xb[bnd])]
+                sb += scipy.signal.lfilter([complex(b[l])], [1.0, -complex(a[l])], xd)
+            s.append(sb)
+        acc = s[3]
+        for bnd in (2, 1):
+            acc = s[bnd] + scipy.signal.upfirdn(h, acc, up=2)[:len(s[bnd])]
+        want = acc + s[0][1::2]
+        np.testing.assert_allclose(z[t], want, atol=1e-10)
+
+
+# ---- P6: periodic shift invariance of the multirate path --------------------
+def test_p6_multirate_periodic_shift_invariance():
+    rng = np.random.default_rng(11)
+    dec, itp = workloads.halfband_taps()
+    bank = _small_multirate_bank(rng)            # B = 4 -> period 2^(B-1) = 8 top-rate samples
+    x = rng.standard_normal(1024).astype(np.float32)
+    q = 3
+    xs = np.concatenate([np.zeros(8 * q, np.float32), x])[:1024]
+    z = oracle.filter_bank(x[None], bank, dec, itp)[0]
+    zs = oracle.filter_bank(xs[None], bank, dec, itp)[0]
+    sh = 4 * q                                   # output is at half the input rate
+    np.testing.assert_allclose(zs[:, sh:], z[:, :-sh], atol=1e-12)
+    assert np.all(zs[:, :sh] == 0)
+
+
+# ---- P8: B = 1 multirate plumbing == plain single-rate sum ------------------
+def test_p8_single_band_path_is_plain_sum():
+    rng = np.random.default_rng(12)
+    bank = workloads.random_bank(rng, 3, 7, [2048], 0, tau_range=(4.0, 40.0), max_delay=30)
+    x = rng.standard_normal((2, 512)).astype(np.float32)
+    z = oracle.filter_bank(x, bank)
+    for D in range(2):
+        for t in range(3):
+            sl = slice(bank["tmpl_offset"][t], bank["tmpl_offset"][t + 1])
+            s = oracle.band_sum(x[D].astype(np.float64), bank["a"][sl], bank["b"][sl], bank["delay"][sl])
+            assert np.array_equal(z[D, t], s)
+    # a template subset is the same numbers as the full run (templates are independent)
+    zs = oracle.filter_bank(x, bank, templates=[2, 0])
+    assert np.array_equal(zs[:, 0], z[:, 2]) and np.array_equal(zs[:, 1], z[:, 0])
+
+
+# ---- P9: peak finder against brute force, with planted exact ties -----------
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_p9_peaks_mode0_bruteforce_with_ties(dtype):
+    rng = np.random.default_rng(13)
+    z = (rng.standard_normal((9, 300)) + 1j * rng.standard_normal((9, 300))).astype(dtype)
+    z[2, 250] = z[2, 40] = 9.0 + 0j              # exact tie -> lowest index wins
+    z[5] *= 0.01                                 # below threshold
+    k, v = oracle.peaks_mode0(z, 1.0)
+    m2 = (z.real.astype(dtype(0).real.dtype) ** 2 + z.imag.astype(dtype(0).real.dtype) ** 2)
+    for r in range(9):
+        assert k[r] == int(np.argmax(m2[r]))     # numpy argmax returns the first maximum
+        assert v[r] == int(m2[r].max() > 1.0)
+    assert k[2] == 40 and v[5] == 0
+
+
+def test_p9_peaks_mode1_bruteforce_and_guarantees():
+    rng = np.random.default_rng(14)
+    T, n, bs = 10, 200, 4
+    z = (rng.standard_normal((T, n)) + 1j * rng.standard_normal((T, n))) * 1.2
+    z[1, 50] = z[3, 50] = 5.0                    # tie across templates at one sample -> lowest t
+    z[6, 10] = z[6, 120] = 6.0                   # tie in time within a template -> lowest k
+    thr = 2.0
+    k, v = oracle.peaks_mode1(z, thr, bs)
+    m2 = np.abs(z) ** 2
+    for t0 in range(0, T, bs):
+        blk = m2[t0:t0 + bs]
+        tstar = np.argmax(blk, axis=0)           # first maximum = lowest t
+        kept = blk.max(axis=0) > thr * thr
+        for t in range(t0, min(T, t0 + bs)):
+            cand = [kk for kk in range(n) if kept[kk] and tstar[kk] == t - t0]
+            if not cand:
+                assert v[t] == 0
+                continue
+            best = max(cand, key=lambda kk: (m2[t, kk], -kk))
+            assert v[t] == 1 and k[t] == best
+        # at most one candidate per sample per bank
+        ks = [k[t] for t in range(t0, min(T, t0 + bs)) if v[t]]
+        assert len(ks) == len(set(ks))
+    assert v[1] == 1 and (v[3] == 0 or k[3] != 50)
+    assert k[6] == 10
+
+
+# ---- sky table: P15 -----------------------------------------------------------
+def _table(nside, dets, sigma, gmst=1.234):
+    pos, resp = workloads.detector_geometry(dets)
+    U2, dl = oracle.sky_table(nside, pos, resp, sigma, gmst, 2048.0)
+    return pos, resp, U2, dl
+
+
+def test_p15_healpix_and_table_invariants():
+    g = _golden()
+    assert 12 * 16 * 16 == g["sky_pixels_foreground"] and 12 * 8 * 8 == g["sky_pixels_background"]
+    for ns in (1, 2, 4, 8):
+        th, ph = oracle.healpix_ring_centres(ns)
+        assert len(th) == 12 * ns * ns
+        v = np.stack([np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph), np.cos(th)], 1)
+        assert np.abs(v.sum(0)).max() < 1e-12                      # centres sum to zero
+        assert len(np.unique(np.round(np.cos(th), 12))) == 4 * ns - 1   # 4 nside - 1 rings
+        assert np.all(np.diff(np.cos(th)) <= 1e-15)                # RING order: north to south
+        d = v @ v.T
+        np.fill_diagonal(d, -1)
+        assert d.max() < 1 - 1e-6                                  # all distinct
+    # equal-area pixels: nearest-neighbour spacing ~ sqrt(4 pi / npix); PAPER.md:171 max 1.9 deg at nside 16
+    th, ph = oracle.healpix_ring_centres(16)
+    v = np.stack([np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph), np.cos(th)], 1)
+    nn = np.degrees(np.arccos(np.clip(np.sort(v @ v.T, axis=1)[:, -2], -1, 1)))
+    assert 2.5 < nn.min() and nn.max() < 2 * 2.0 * 1.9
+    assert abs((1 - math.cos(math.radians(g["pixel_max_angle_deg"]))) * 100 - g["pixel_max_snr_loss_percent"]) < 0.01
+    pos, resp, U2, dl = _table(8, ["H1", "L1", "V1"], [1, 1, 0.5])
+    P = U2 @ U2.transpose(0, 2, 1)
+    np.testing.assert_allclose(U2.transpose(0, 2, 1) @ U2, np.broadcast_to(np.eye(2), (768, 2, 2)), atol=1e-12)
+    np.testing.assert_allclose(P @ P, P, atol=1e-12)
+    np.testing.assert_allclose(np.trace(P, axis1=1, axis2=2), 2.0, atol=1e-12)
+    for i in range(3):
+        for j in range(i + 1, 3):
+            lt = np.linalg.norm(pos[i] - pos[j]) / workloads.C_LIGHT
+            assert np.abs(dl[:, i] - dl[:, j]).max() <= lt * 2048.0 + 1.0
+            assert np.abs(dl[:, i] - dl[:, j]).max() >= lt * 2048.0 * 0.95 - 1.0
+    lts = sorted(np.linalg.norm(pos[i] - pos[j]) / workloads.C_LIGHT * 1e3 for i in range(3) for j in range(i + 1, 3))
+    np.testing.assert_allclose(lts, [10.01, 26.45, 27.29], atol=0.05)   # known light-travel times (ms)
+
+
+def test_table_signs_against_plane_wave():
+    """A delta-like pulse arriving from direction p0 hits detector I at geocentre
+    time + tau_I: the detector CLOSER to the source (larger r.n) is hit earlier,
+    so its delay is more negative.  Pins the sign of the delay table."""
+    pos, resp, U2, dl = _table(4, ["H1", "L1", "V1"], [1, 1, 1])
+    th, ph = oracle.healpix_ring_centres(4)
+    lam = ph - 1.234
+    n = np.stack([np.sin(th) * np.cos(lam), np.sin(th) * np.sin(lam), np.cos(th)], 1)
+    proj = n @ pos.T
+    for p in range(0, 192, 7):
+        order_geo = np.argsort(-proj[p])
+        assert np.all(np.diff(dl[p][order_geo]) >= 0)
+    # projector equals the projector onto the column space of G_sigma (pinv form, Eq. 25)
+    G, _ = oracle.g_sigma(th, ph, resp, [1, 1, 1], 1.234)
+    for p in (0, 50, 191):
+        Pg = G[p] @ np.linalg.pinv(G[p])
+        np.testing.assert_allclose(U2[p] @ U2[p].T, Pg, atol=1e-10)
+
+
+def test_antenna_pattern_textbook_special_cases():
+    """A detector with arms along x, y at the origin: overhead source (theta=0)
+    gives |F+|^2+|Fx|^2 = 1; a source in the detector plane along an arm gives
+    1/4; along the bisector gives 0 (textbook interferometer pattern)."""
+    resp = np.zeros((1, 3, 3))
+    resp[0, 0, 0], resp[0, 1, 1] = 0.5, -0.5
+    def power(theta, phi):
+        G, _ = oracle.g_sigma(np.array([theta]), np.array([phi]), resp, [1.0], 0.0)
+        return float(np.sum(G[0, 0] ** 2))
+    assert abs(power(0.0, 0.3) - 1.0) < 1e-12
+    assert abs(power(math.pi / 2, 0.0) - 0.25) < 1e-12
+    assert abs(power(math.pi / 2, math.pi / 4) - 0.0) < 1e-12
+    # 1/4 (1+cos^2)^2 cos^2(2phi) + cos^2 sin^2(2phi)
+    th, ph = 0.7, 0.4
+    want = 0.25 * (1 + math.cos(th) ** 2) ** 2 * math.cos(2 * ph) ** 2 + math.cos(th) ** 2 * math.sin(2 * ph) ** 2
+    assert abs(power(th, ph) - want) < 1e-12
+
+
+def _dense_view(z):
+    """z complex [D][R][n] -> view args for a linear (non-wrapping) buffer."""
+    D, R, n = z.shape
+    return dict(det_stride=R * n, row_stride=n, ring_len=n, k_newest=n - 1)
+
+
+# ---- P10 / P11 / P12 / P13: coherent statistic --------------------------------
+def test_p10_p11_identity_and_two_detector_case():
+    rng = np.random.default_rng(20)
+    pos, resp, U2, dl = _table(4, ["H1", "L1"], [1, 1])
+    z = rng.standard_normal((2, 3, 400)) + 1j * rng.standard_normal((2, 3, 400))
+    k = np.array([200, 150, 300])
+    res, pix, mp = oracle.sky_search(U2.astype(np.float32), dl, z, trig_valid=[1, 1, 1], trig_row=[0, 1, 2],
+                                     trig_det=[0, 1, 0], trig_k=k, want_map=True, **_dense_view(z))
+    for i, (T, r) in enumerate(zip([0, 1, 0], [0, 1, 2])):
+        O = 1 - T
+        for p in range(192):
+            tot = abs(z[T, r, k[i]]) ** 2 + abs(z[O, r, k[i] + dl[p, O] - dl[p, T]]) ** 2
+            assert abs(mp[i, p] - tot) < 1e-6 * tot          # N_d = 2: coh2 = sum |z|^2 (fp32 U2 rounding)
+    # fp32-rounded U2 is orthonormal to ~1e-7 only, so coh2 may exceed tot2 by that much (null clamps at 0)
+    np.testing.assert_allclose(res[:, 0, 0] + res[:, 0, 1], res[:, 0, 2], rtol=1e-6)
+    assert np.all(res[:, 0, 1] < 1e-5 * res[:, 0, 2])
+
+
+def test_p10_identity_three_detectors_and_manual_formula():
+    rng = np.random.default_rng(21)
+    pos, resp, U2, dl = _table(4, ["H1", "L1", "V1"], [1, 1, 0.5])
+    u2 = U2.astype(np.float32)
+    z = rng.standard_normal((3, 2, 600)) + 1j * rng.standard_normal((3, 2, 600))
+    v = _dense_view(z)
+    for (row, T, k) in [(0, 1, 300), (1, 2, 222)]:
+        for p in (0, 17, 100, 191):
+            ok, coh2, null2, tot2 = oracle.sky_eval(u2, dl, z, row=row, det=T, k=k, p=p, **v)
+            vec = np.array([z[I, row, k + dl[p, I] - dl[p, T]] for I in range(3)])
+            c = u2[p].astype(np.float64).T @ vec
+            assert ok and abs(coh2 - np.sum(np.abs(c) ** 2)) < 1e-12
+            assert abs(tot2 - np.sum(np.abs(vec) ** 2)) < 1e-12 and abs(coh2 + null2 - tot2) < 1e-12
+            assert coh2 <= tot2 * (1 + 1e-6)
+
+
+def test_p12_noise_expectations_four_and_two_dof():
+    g = _golden()
+    rng = np.random.default_rng(22)
+    pos, resp, U2, dl = _table(2, ["H1", "L1", "V1"], [1, 1, 0.5])
+    n = 120000
+    z = rng.standard_normal((3, 1, n)) + 1j * rng.standard_normal((3, 1, n))     # unit variance per quadrature
+    ks = np.arange(100, n - 100, 3)
+    acc_c, acc_n = 0.0, 0.0
+    u2 = U2.astype(np.float32)
+    v = _dense_view(z)
+    for k in ks[:20000]:
+        ok, coh2, null2, tot2 = oracle.sky_eval(u2, dl, z, row=0, det=0, k=int(k), p=11, **v)
+        acc_c += coh2
+        acc_n += null2
+    assert abs(acc_c / 20000 - g["coh_dof"]) < 0.08                          # E coh2 = 4
+    assert abs(acc_n / 20000 - (2 * 3 - 4)) < 0.06                           # E null2 = 2 N_d - 4
+
+
+def test_p13_injected_signal_recovers_its_pixel_and_zero_null():
+    rng = np.random.default_rng(23)
+    pos, resp, U2, dl = _table(8, ["H1", "L1", "V1"], [1, 1, 0.5])
+    u2 = U2.astype(np.float32)
+    n = 800
+    for p0, T in [(5, 0), (300, 1), (700, 2)]:
+        z = np.zeros((3, 1, n), complex)
+        c = rng.standard_normal(2) + 1j * rng.standard_normal(2)
+        amp = u2[p0].astype(np.float64) @ c
+        o = np.arange(-20, 21)
+        env = np.exp(-o ** 2 / (2 * 6.0 ** 2)) * np.exp(0.6j * o)
+        k0 = 400
+        for I in range(3):
+            z[I, 0, k0 + dl[p0, I] - dl[p0, T] + o] = amp[I] * env
+        res, pix, mp = oracle.sky_search(u2, dl, z, trig_valid=[1], trig_row=[0], trig_det=[T], trig_k=[k0],
+                                         want_map=True, **_dense_view(z))
+        tot = np.sum(np.abs(amp) ** 2)
+        assert abs(mp[0, p0] - tot) < 1e-6 * tot                 # all power in the signal plane
+        same = [p for p in range(768) if np.array_equal(dl[p] - dl[p, T], dl[p0] - dl[p0, T])]
+        assert pix[0, 0] in same                                 # unique up to pixels sharing the delay tuple
+        assert res[0, 0, 1] < 1e-5 * tot                         # null = 0 at the true pixel
+
+
+def test_out_of_range_and_invalid_triggers():
+    rng = np.random.default_rng(24)
+    pos, resp, U2, dl = _table(2, ["H1", "L1", "V1"], [1, 1, 1])
+    z = rng.standard_normal((3, 1, 300)) + 1j * rng.standard_normal((3, 1, 300))
+    res, pix, _ = oracle.sky_search(U2.astype(np.float32), dl, z, trig_valid=[1, 1, 0, 1], trig_row=[0] * 4,
+                                    trig_det=[0] * 4, trig_k=[10, 295, 150, 150], **_dense_view(z))
+    assert list(pix[:, 0][:3]) == [-1, -1, -1] and pix[3, 0] >= 0
+    assert np.all(res[:3] == 0)
+
+
+# ---- P16: time slides ----------------------------------------------------------
+def test_p16_time_slides_special_cases():
+    rng = np.random.default_rng(25)
+    pos, resp, U2, dl = _table(4, ["H1", "L1", "V1"], [1, 1, 0.5])
+    u2 = U2.astype(np.float32)
+    step, S = 128, 5
+    base = rng.standard_normal((3, 2, step)) + 1j * rng.standard_normal((3, 2, step))
+    z = np.tile(base, (1, 1, 8))                                 # periodic with period = step
+    n = z.shape[2]
+    tr = dict(trig_valid=[1, 1], trig_row=[0, 1], trig_det=[0, 2], trig_k=[n - 100, n - 90])
+    fg, fpix, _ = oracle.sky_search(u2, dl, z, **tr, **_dense_view(z))
+    bg, bpix, _ = oracle.sky_search(u2, dl, z, n_slides=S, step=step, slide_mult=[1, 1, 1], **tr, **_dense_view(z))
+    for s in range(S):                                           # periodic ring: every slide == foreground
+        np.testing.assert_allclose(bg[:, s], fg[:, 0], rtol=1e-12)
+        assert np.array_equal(bpix[:, s], fpix[:, 0])
+    z2 = rng.standard_normal((3, 2, n)) + 1j * rng.standard_normal((3, 2, n))
+    fg2, fpix2, _ = oracle.sky_search(u2, dl, z2, **tr, **_dense_view(z2))
+    bg0, bpix0, _ = oracle.sky_search(u2, dl, z2, n_slides=3, step=step, slide_mult=[0, 0, 0], **tr, **_dense_view(z2))
+    for s in range(3):                                           # multipliers 0: slide == foreground
+        assert np.array_equal(bg0[:, s], fg2[:, 0]) and np.array_equal(bpix0[:, s], fpix2[:, 0])
+    # a genuine slide equals the foreground of a manually shifted copy (companions moved later by s*step)
+    bg1, bpix1, _ = oracle.sky_search(u2, dl, z2, n_slides=2, step=step, slide_mult=[1, 1, 1], **tr, **_dense_view(z2))
+    for s in (1, 2):
+        for i, T in enumerate([0, 2]):
+            zz = np.roll(z2, s * step, axis=2)
+            zz[T] = z2[T]
+            f, fp, _ = oracle.sky_search(u2, dl, zz, trig_valid=[1], trig_row=[i], trig_det=[T],
+                                         trig_k=[tr["trig_k"][i]], **_dense_view(zz))
+            np.testing.assert_allclose(bg1[i, s - 1], f[0, 0], rtol=1e-12)
+            assert bpix1[i, s - 1] == fp[0, 0]
+
+
+# ---- P17: the paper's printed arithmetic ---------------------------------------
+def test_p17_paper_cost_arithmetic():
+    g = _golden()
+    flops = g["flop_per_filter_sample"] * g["o3_filters_per_template"] * g["o3_templates"] * g["o3_sample_rate"] * g["o3_detectors"]
+    assert abs(flops / 1e12 - g["o3_filter_tflops"]) < 0.05
+    assert abs(flops / (g["cpu_core_gflops"] * 1e9) - g["o3_cpu_cores"]) < 20
+    nd = g["o3_detectors"]
+    coh = 4 * nd ** 3 * g["o3_templates"] * (g["sky_pixels_foreground"] + g["n_time_shifts"] * g["sky_pixels_background"])
+    assert abs(coh / 1e12 - g["coherent_worst_case_tflops"]) < 0.06
+    # Table I: network SNR = quadrature sum of the detector SNRs
+    for rl, rh, rv, net in [(13.8, 8.9, 3.8, 16.9), (24.4, 19.4, 3.7, 31.5), (9.9, 4.4, 4.1, 11.6)]:
+        assert abs(math.sqrt(rl ** 2 + rh ** 2 + rv ** 2) - net) < 0.15
+    # the update counted by the paper: 2 mul + 4 fma + 2 add = 12 flop in 8 instructions
+    assert 2 * 1 + 4 * 2 + 2 * 1 == g["flop_per_filter_sample"]
+
+
+# ---- generator sanity (inputs only) ---------------------------------------------
+def test_generator_is_seeded_and_shaped():
+    b0 = workloads.bank_for_config(0)
+    b0b = workloads.bank_for_config(0)
+    assert np.array_equal(b0["a"], b0b["a"]) and np.array_equal(b0["delay"], b0b["delay"])
+    assert b0["n_templates"] == 4 and len(b0["a"]) == 128 and b0["delay"].max() <= 2047
+    assert np.all(np.abs(b0["a"]) < 1)
+    s0 = workloads.strain_for_config(0)
+    assert s0["strain"].shape == (2, 2048) and s0["strain"].dtype == np.float32
+    b2 = workloads.bank_for_config(2, n_templates=2)
+    cnt = np.bincount(b2["band"][:600], minlength=8)
+    assert list(cnt) == [75] * 8 and np.all(np.diff(b2["band"][:600].astype(int)) >= 0)
+    from workloads.gen import _split_over_bands
+    assert _split_over_bands(700, 8) == [87, 87, 87, 87, 88, 88, 88, 88]
