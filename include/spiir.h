@@ -1,0 +1,222 @@
+/*
+ * spiir.h — C ABI of the B200-native SPIIR hot path (arXiv 2011.06787).
+ *
+ * Two stages, both hand-written CUDA for sm_100a behind this boundary:
+ *   1. the SPIIR filter bank  — PAPER.md:122-131 (Sec. II B 1, "Eq. 8"):
+ *        z_t[k] = sum_{l in t} y_l[k],  y_l[k] = a_l y_l[k-1] + b_l x[k - d_l]
+ *      over (multirate) whitened strain, with all state carried across streaming
+ *      chunks, plus the per-second candidate selection of PAPER.md:162-167;
+ *   2. the coherent sky search — PAPER.md:147-157 (Eq. 9, 10)
+ *      (HEALPix directions, look-up tables of U and time offsets) and its
+ *      time-slide background.
+ *
+ * Conventions
+ *   - Every function returns an int status: SPIIR_OK or a negative SPIIR_E* code;
+ *     spiir_last_error() gives the text of the last failure on this thread.
+ *   - Pointers named host_* are host memory, dev_* are device memory owned by the
+ *     caller.  The library owns only the opaque handle and the workspace carve-up;
+ *     it never frees caller memory and allocates nothing after spiir_bank_init.
+ *   - All device work is enqueued on the caller's stream (passed as void*, a
+ *     cudaStream_t); no call synchronises the device.  Outputs are valid once the
+ *     stream has been synchronised by the caller.
+ *   - Complex numbers are interleaved (re, im) float32.
+ *   - Sample indices k are ABSOLUTE output-rate sample counts since the last
+ *     spiir_bank_reset (int64).
+ */
+#ifndef SPIIR_H
+#define SPIIR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPIIR_OK          0
+#define SPIIR_EINVAL     -1   /* null pointer, bad size, bands not halving, delay > max_delay, ... */
+#define SPIIR_ENOMEM     -2   /* workspace too small */
+#define SPIIR_ECUDA      -3   /* CUDA runtime error (text in spiir_last_error) */
+#define SPIIR_EOVERFLOW  -4   /* a fixed-size internal table would overflow */
+
+#define SPIIR_MAX_BANDS   8
+#define SPIIR_MAX_DET     4
+#define SPIIR_FIR_TAPS   32
+
+typedef struct spiir_bank spiir_bank;              /* opaque */
+typedef struct { float re, im; } spiir_c32;
+
+/* Description of a filter bank (all arrays host memory, copied at init).
+ * Filters are stored template by template (CSR); within a template in any order.
+ * A filter l is the triple (a, b, delay) of PAPER.md:122 — feedback coefficient
+ * (paper a_0, north_star a1), feed-forward coefficient (paper b_1, north_star b0),
+ * integer delay in samples of ITS OWN band — plus the index of its rate band. */
+typedef struct {
+  int32_t n_det;                         /* 1..SPIIR_MAX_DET; coefficients are shared by detectors      */
+  int32_t n_templates;
+  int32_t n_bands;                       /* 1..SPIIR_MAX_BANDS                                          */
+  int32_t out_band;                      /* band whose rate is the output rate; must be 0 or 1          */
+  int32_t band_rate_hz[SPIIR_MAX_BANDS]; /* strictly halving: rate[b+1] * 2 == rate[b]                  */
+  int32_t max_delay[SPIIR_MAX_BANDS];    /* history depth per band, samples of that band                */
+  int64_t n_filters;                     /* total                                                        */
+  const int64_t*   host_tmpl_offset;     /* [n_templates+1] CSR into the filter arrays                  */
+  const spiir_c32* host_a;               /* [n_filters] feedback                                        */
+  const spiir_c32* host_b;               /* [n_filters] feed-forward                                    */
+  const int32_t*   host_delay;           /* [n_filters] 0 <= delay <= max_delay[band]                   */
+  const uint8_t*   host_band;            /* [n_filters]                                                 */
+  const float*     host_fir_dec;         /* [32] decimation taps: x_{b+1}[m] = sum_j g[j] x_b[2m+1-j]   */
+  const float*     host_fir_int;         /* [32] interpolation taps h (factor 2 included):
+                                            acc_b[m] = s_b[m] + sum_j h[j] v[m-j], v = zero-stuffed acc_{b+1} */
+  int32_t max_chunk_samples;             /* largest n_samples of one spiir_filter_chunk call (band 0)   */
+  int32_t bank_size;                     /* templates per "template bank" for peak mode 1 */
+  int64_t ring_len;                      /* SNR history kept per (detector, template), output samples;
+                                            >= max_chunk_samples >> out_band                            */
+} spiir_bank_desc;
+
+/* Device bytes spiir_bank_init needs for this bank (coefficients, IIR state, delay
+ * lines, FIR / interpolator histories, band-sum scratch, SNR ring, peak slots). */
+int spiir_bank_workspace_bytes(const spiir_bank_desc* desc, size_t* bytes);
+
+/* Plans the device layout, copies the coefficients, zeroes all carried state.
+ * dev_workspace: 256-byte aligned device memory of at least the queried size; it
+ * must stay alive until spiir_bank_free.  Errors: EINVAL, ENOMEM, ECUDA. */
+int spiir_bank_init(spiir_bank** out, const spiir_bank_desc* desc,
+                    void* dev_workspace, size_t bytes, void* stream);
+
+/* Zeroes every carried state (IIR states, histories, ring, sample counter). */
+int spiir_bank_reset(spiir_bank* bank, void* stream);
+
+/* Releases the host-side handle (never the workspace). */
+int spiir_bank_free(spiir_bank* bank);
+
+/* One streaming chunk (H0-H3 of DESIGN.md): decimate the strain into the rate
+ * bands, run every filter's recursion over the chunk with its state carried
+ * from the previous call, sum per template, combine the bands up to the output
+ * rate, append the SNR to the ring and track each template's maximum.
+ *   dev_strain : [n_det][n_samples] float32 at band_rate_hz[0]
+ *   n_samples  : multiple of 4 * 2^(n_bands-1), <= max_chunk_samples
+ *   dev_snr_out: [n_det][n_templates][n_samples >> out_band] complex, or NULL (ring only)
+ */
+int spiir_filter_chunk(spiir_bank* bank, const float* dev_strain, int32_t n_samples,
+                       spiir_c32* dev_snr_out, void* stream);
+
+/* A single-detector candidate.  40 bytes. */
+typedef struct {
+  int32_t valid;      /* 1 if this slot holds a candidate                          */
+  int32_t tmpl;       /* template index (row of the SNR view)                      */
+  int32_t det;        /* detector the candidate was found in                       */
+  int32_t _pad;
+  int64_t k;          /* absolute output-rate sample index of the maximum          */
+  float   z_re, z_im; /* complex SNR there                                         */
+  float   snr;        /* |z|                                                       */
+  float   _pad2;
+} spiir_trigger;
+
+/* Candidate selection over the LAST chunk (H4).
+ *   mode 0: per (detector, template) the sample of largest |z|^2 (lowest k on exact
+ *           ties); valid iff |z|^2 > thr^2 (strict; thr = 0 keeps every slot).
+ *   mode 1: the paper's two-step rule per bank of desc.bank_size templates:
+ *           at each sample keep the loudest template if above threshold, then per
+ *           template keep its loudest kept sample.
+ * |z|^2 is decided in float32 as fl(fl(re*re) + fl(im*im)).
+ *   dev_trig : [n_det][n_templates] dense slots (deterministic order)
+ *   dev_count: one int32, number of valid slots */
+int spiir_peaks(spiir_bank* bank, float snr_threshold, int32_t mode,
+                spiir_trigger* dev_trig, int32_t* dev_count, void* stream);
+
+/* A window onto complex SNR series: z(det,row,k) = dev_z[det*det_stride +
+ * row*row_stride + (k mod ring_len)] (strides in complex elements), defined for
+ * max(0, k_newest - ring_len + 1) <= k <= k_newest. */
+typedef struct {
+  const spiir_c32* dev_z;
+  int64_t det_stride, row_stride;
+  int64_t ring_len, k_newest;
+} spiir_snr_view;
+
+/* The bank's own SNR ring as a view (rows = templates). */
+int spiir_bank_snr_view(const spiir_bank* bank, spiir_snr_view* view);
+
+/* Host helper (float64 inside, not on the hot path) — the per-direction look-up
+ * table of: HEALPix RING pixel centres of `nside`,
+ * G+ / Gx of each detector at psi = 0, U2 = first two left
+ * singular vectors of the sensitivity-weighted response G_sigma (Eq. 27,
+ * PAPER.md:473), delay = rint(-(r_I . n)/c * fs_hz) per detector against the
+ * geocentre (differences delay[p][I] - delay[p][T] are taken at use).
+ *   host_det_pos_m [n_det][3] Earth-fixed metres; host_det_resp [n_det][3][3]
+ *   response tensors (x x^T - y y^T)/2; host_sigma [n_det] sensitivity weights.
+ *   Outputs: host_u2 [12 nside^2][n_det][2], host_delay [12 nside^2][n_det]. */
+int spiir_sky_table_build(int32_t nside, int32_t n_det, const double* host_det_pos_m,
+                          const double* host_det_resp, const double* host_sigma,
+                          double gmst_rad, double fs_hz, float* host_u2, int32_t* host_delay);
+
+/* A look-up table prepared for the device (opaque).  The plan re-orders the
+ * directions so that those sharing one tuple of inter-detector delays are
+ * adjacent, and stores for each direction the projector U2 U2^T (Eq. 28,
+ * rho_c^2 = z^H U I U^T z) next to its pixel index.  Results are
+ * always reported with the caller's pixel numbering. */
+typedef struct spiir_sky_plan spiir_sky_plan;
+
+/* Device bytes a plan for (n_det, n_pix) with outputs for up to max_slots
+ * trigger slots needs (table stream + compaction lists). */
+int spiir_sky_plan_workspace_bytes(int32_t n_det, int32_t n_pix, int32_t max_slots, size_t* bytes);
+
+/* host_u2 [n_pix][n_det][2] float32, host_delay [n_pix][n_det] int32 (any table,
+ * e.g. from spiir_sky_table_build; copied).  dev_workspace: 256-byte aligned,
+ * alive until spiir_sky_plan_free.  n_det 2..SPIIR_MAX_DET.  Synchronises the
+ * stream once (setup, not hot path).  Errors: EINVAL, ENOMEM, ECUDA. */
+int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int32_t max_slots,
+                        const float* host_u2, const int32_t* host_delay,
+                        void* dev_workspace, size_t bytes, void* stream);
+int spiir_sky_plan_free(spiir_sky_plan* plan);
+/* Number of distinct delay tuples of the plan (introspection / DESIGN.md §5). */
+int32_t spiir_sky_plan_tuples(const spiir_sky_plan* plan);
+
+/* Result of one (trigger[, slide]) search: the maximum over directions of the
+ * coherent SNR^2 (Eq. 9), the pixel where it occurs (lowest index on exact
+ * ties), and tot2 = sum_I |z_I|^2, null2 = max(tot2 - coh2, 0) (Eq. 10) there.
+ * pix = -1 (and zeros) if the slot is invalid or any gather of the search would
+ * leave the valid range of the view. */
+typedef struct { float coh2, null2, tot2; int32_t pix; } spiir_sky_result;
+
+/* H5: for every valid trigger (T, t, k) and every direction p:
+ *   v_I = z_I[t][k + delay[p][I] - delay[p][T]],
+ *   coh2 = sum_j |sum_I U2[p][I][j] v_I|^2 = sum_IJ (U2 U2^T)_IJ Re(v_I conj v_J).
+ *   dev_trig [n_slots] (n_slots <= the plan's max_slots); dev_out [n_slots];
+ *   dev_skymap (optional, may be NULL) [n_slots][n_pix] coh2 (zeros for slots
+ *   with pix = -1). */
+int coherent_sky_search(spiir_sky_plan* plan, const spiir_snr_view* view,
+                        const spiir_trigger* dev_trig, int32_t n_slots,
+                        spiir_sky_result* dev_out, float* dev_skymap, void* stream);
+
+/* H6: the same search for slides s = 1..n_slides with detector I != T read at
+ * k - s*step_samples*host_slide_mult[I] + delay difference.
+ *   bg_plan may be a coarser table than the foreground's.
+ *   dev_out [n_slots][n_slides] (slide s at index s-1). */
+int timeslide_background(spiir_sky_plan* bg_plan, const spiir_snr_view* view,
+                         const spiir_trigger* dev_trig, int32_t n_slots,
+                         int32_t n_slides, int64_t step_samples, const int32_t* host_slide_mult,
+                         spiir_sky_result* dev_out, void* stream);
+/* Introspection: the layout chosen for a band (lanes per unit G, filters per lane
+ * F, units, padded slots, shared-memory history depth) and counters for bench. */
+typedef struct {
+  int32_t lanes_per_unit, filters_per_lane, n_units, n_units_long;
+  int32_t smem_history, smem_bytes;
+  int64_t n_filters, n_slots;
+} spiir_band_plan;
+int spiir_bank_band_plan(const spiir_bank* bank, int32_t band, spiir_band_plan* plan);
+/* Filter-sample updates (real filters only, all detectors) one chunk of n_samples performs. */
+int64_t spiir_bank_updates_per_chunk(const spiir_bank* bank, int32_t n_samples);
+/* Kernels launched by this library on this thread so far (bench bookkeeping). */
+int64_t spiir_launch_count(void);
+
+/* Measurement helper: runs a dependency-free FP32 FMA loop on every SM and
+ * returns the duration of `reps` launches in *ms_out and the FMA-lane-operations
+ * performed per launch in *fma_per_launch (peak = 2*fma/time flop/s). */
+int spiir_fp32_peak_probe(int32_t reps, double* ms_out, double* fma_per_launch, void* stream);
+
+const char* spiir_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPIIR_H */

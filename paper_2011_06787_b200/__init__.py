@@ -1,0 +1,17 @@
+"""B200-native SPIIR hot path (arXiv 2011.06787): filter bank + coherent sky search.
+
+The product is the C-ABI library ``libspiir_b200.so`` (include/spiir.h), hand-written
+CUDA for sm_100a; this package is its thin ctypes binding.  PyTorch is used by the
+callers for device memory and streams only.  Nothing here imports ``oracle``.
+"""
+from .binding import (  # noqa: F401
+    lib, last_error, SpiirError, EXPORTS, LIB_PATH,
+    spiir_bank_desc, spiir_snr_view, spiir_band_plan, TRIGGER_DTYPE, RESULT_DTYPE,
+    make_desc, Bank, SkyPlan, SnrView, sky_table_build,
+    triggers_to_numpy, triggers_from_numpy, results_to_numpy, fp32_peak_probe,
+    SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EOVERFLOW,
+)
+from . import binding as _b
+
+for _n in EXPORTS:                      # the C names themselves: spiir_bank_init, spiir_filter_chunk, ...
+    globals()[_n] = getattr(_b, _n)

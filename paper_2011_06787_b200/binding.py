@@ -1,0 +1,315 @@
+"""ctypes binding of libspiir_b200.so — argument marshalling only.
+
+Every function of include/spiir.h is exposed under its C name (``spiir_bank_init``,
+``spiir_filter_chunk``, ``spiir_peaks``, ``coherent_sky_search``,
+``timeslide_background`` ...), taking raw device pointers (ints) exactly as the C
+ABI does.  The small classes below (Bank, SkyPlan, SnrView) only own the torch
+tensors that back the workspaces and outputs and pass ``tensor.data_ptr()`` and
+``torch.cuda.current_stream().cuda_stream`` through; every step of the path runs in
+the library's CUDA kernels.  There is no CPU fallback: a missing library raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libspiir_b200.so")
+
+SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EOVERFLOW = 0, -1, -2, -3, -4
+SPIIR_MAX_BANDS, SPIIR_MAX_DET, SPIIR_FIR_TAPS = 8, 4, 32
+
+
+class SpiirError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("spiir error %d: %s" % (code, text))
+        self.code = code
+
+
+class spiir_bank_desc(C.Structure):
+    _fields_ = [
+        ("n_det", C.c_int32), ("n_templates", C.c_int32), ("n_bands", C.c_int32), ("out_band", C.c_int32),
+        ("band_rate_hz", C.c_int32 * SPIIR_MAX_BANDS), ("max_delay", C.c_int32 * SPIIR_MAX_BANDS),
+        ("n_filters", C.c_int64),
+        ("host_tmpl_offset", C.c_void_p), ("host_a", C.c_void_p), ("host_b", C.c_void_p),
+        ("host_delay", C.c_void_p), ("host_band", C.c_void_p),
+        ("host_fir_dec", C.c_void_p), ("host_fir_int", C.c_void_p),
+        ("max_chunk_samples", C.c_int32), ("bank_size", C.c_int32), ("ring_len", C.c_int64),
+    ]
+
+
+class spiir_snr_view(C.Structure):
+    _fields_ = [("dev_z", C.c_void_p), ("det_stride", C.c_int64), ("row_stride", C.c_int64),
+                ("ring_len", C.c_int64), ("k_newest", C.c_int64)]
+
+
+class spiir_band_plan(C.Structure):
+    _fields_ = [("lanes_per_unit", C.c_int32), ("filters_per_lane", C.c_int32), ("n_units", C.c_int32),
+                ("n_units_long", C.c_int32), ("smem_history", C.c_int32), ("smem_bytes", C.c_int32),
+                ("n_filters", C.c_int64), ("n_slots", C.c_int64)]
+
+
+# numpy views of the two plain structs that live in device arrays
+TRIGGER_DTYPE = np.dtype([("valid", "<i4"), ("tmpl", "<i4"), ("det", "<i4"), ("_pad", "<i4"), ("k", "<i8"),
+                          ("z_re", "<f4"), ("z_im", "<f4"), ("snr", "<f4"), ("_pad2", "<f4")])
+RESULT_DTYPE = np.dtype([("coh2", "<f4"), ("null2", "<f4"), ("tot2", "<f4"), ("pix", "<i4")])
+assert TRIGGER_DTYPE.itemsize == 40 and RESULT_DTYPE.itemsize == 16
+
+_SIGNATURES = {
+    "spiir_bank_workspace_bytes": (C.c_int, [C.POINTER(spiir_bank_desc), C.POINTER(C.c_size_t)]),
+    "spiir_bank_init": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(spiir_bank_desc), C.c_void_p, C.c_size_t, C.c_void_p]),
+    "spiir_bank_reset": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "spiir_bank_free": (C.c_int, [C.c_void_p]),
+    "spiir_filter_chunk": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
+    "spiir_peaks": (C.c_int, [C.c_void_p, C.c_float, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "spiir_bank_snr_view": (C.c_int, [C.c_void_p, C.POINTER(spiir_snr_view)]),
+    "spiir_sky_table_build": (C.c_int, [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                        C.c_double, C.c_void_p, C.c_void_p]),
+    "spiir_sky_plan_workspace_bytes": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]),
+    "spiir_sky_plan_init": (C.c_int, [C.POINTER(C.c_void_p), C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
+                                      C.c_void_p, C.c_size_t, C.c_void_p]),
+    "spiir_sky_plan_free": (C.c_int, [C.c_void_p]),
+    "spiir_sky_plan_tuples": (C.c_int32, [C.c_void_p]),
+    "coherent_sky_search": (C.c_int, [C.c_void_p, C.POINTER(spiir_snr_view), C.c_void_p, C.c_int32, C.c_void_p,
+                                      C.c_void_p, C.c_void_p]),
+    "timeslide_background": (C.c_int, [C.c_void_p, C.POINTER(spiir_snr_view), C.c_void_p, C.c_int32, C.c_int32,
+                                       C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "spiir_bank_band_plan": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(spiir_band_plan)]),
+    "spiir_bank_updates_per_chunk": (C.c_int64, [C.c_void_p, C.c_int32]),
+    "spiir_launch_count": (C.c_int64, []),
+    "spiir_fp32_peak_probe": (C.c_int, [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
+    "spiir_last_error": (C.c_char_p, []),
+}
+EXPORTS = sorted(_SIGNATURES)
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library.  Raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("%s is missing: run `python -m paper_2011_06787_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def last_error():
+    return lib().spiir_last_error().decode()
+
+
+def _check(rc):
+    if rc != SPIIR_OK:
+        raise SpiirError(rc, last_error())
+    return rc
+
+
+def _mk(name):
+    def call(*args):
+        return getattr(lib(), name)(*args)
+    call.__name__ = name
+    call.__doc__ = "C ABI %s — see include/spiir.h" % name
+    return call
+
+
+for _n in EXPORTS:
+    globals()[_n] = _mk(_n)
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _hp(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def make_desc(bank, n_det, max_chunk_samples, ring_len, bank_size=1000, dec_taps=None, int_taps=None):
+    """spiir_bank_desc from a workloads bank dict; returns (desc, keepalive list)."""
+    d = spiir_bank_desc()
+    rates = list(bank["band_rates"])
+    keep = [np.ascontiguousarray(bank["tmpl_offset"], dtype=np.int64),
+            np.ascontiguousarray(np.asarray(bank["a"], dtype=np.complex64)).view(np.float32),
+            np.ascontiguousarray(np.asarray(bank["b"], dtype=np.complex64)).view(np.float32),
+            np.ascontiguousarray(bank["delay"], dtype=np.int32),
+            np.ascontiguousarray(bank["band"], dtype=np.uint8),
+            None if dec_taps is None else np.ascontiguousarray(dec_taps, dtype=np.float32),
+            None if int_taps is None else np.ascontiguousarray(int_taps, dtype=np.float32)]
+    d.n_det, d.n_templates, d.n_bands, d.out_band = n_det, int(bank["n_templates"]), len(rates), int(bank["out_band"])
+    for i in range(SPIIR_MAX_BANDS):
+        d.band_rate_hz[i] = rates[i] if i < len(rates) else 0
+        d.max_delay[i] = int(bank["max_delay"][i]) if i < len(rates) else 0
+    d.n_filters = len(keep[3])
+    d.host_tmpl_offset, d.host_a, d.host_b, d.host_delay, d.host_band, d.host_fir_dec, d.host_fir_int = \
+        [None if k is None else k.ctypes.data for k in keep]
+    d.max_chunk_samples, d.bank_size, d.ring_len = int(max_chunk_samples), int(bank_size), int(ring_len)
+    return d, keep
+
+
+class SnrView:
+    """A spiir_snr_view over a caller tensor z float32 [n_det][rows][ring_len][2] on the device."""
+
+    def __init__(self, z=None, k_newest=None, raw=None):
+        if raw is not None:
+            self.c, self._keep = raw, None
+            return
+        assert z.is_cuda and z.dim() == 4 and z.shape[-1] == 2 and z.is_contiguous()
+        n_det, rows, ring_len, _ = z.shape
+        self._keep = z
+        self.c = spiir_snr_view(z.data_ptr(), rows * ring_len, ring_len, ring_len,
+                                ring_len - 1 if k_newest is None else int(k_newest))
+
+
+class Bank:
+    """Owns the workspace tensor of one spiir_bank and forwards to the C ABI."""
+
+    def __init__(self, bank, n_det, max_chunk_samples, ring_len=None, bank_size=1000, dec_taps=None, int_taps=None):
+        import torch
+        n_out_max = max_chunk_samples >> int(bank["out_band"])
+        ring_len = n_out_max if ring_len is None else ring_len
+        self.desc, self._keep = make_desc(bank, n_det, max_chunk_samples, ring_len, bank_size, dec_taps, int_taps)
+        nbytes = C.c_size_t(0)
+        _check(lib().spiir_bank_workspace_bytes(C.byref(self.desc), C.byref(nbytes)))
+        self.workspace_bytes = nbytes.value
+        self.ws = torch.empty(nbytes.value + 256, dtype=torch.uint8, device="cuda")
+        base = (self.ws.data_ptr() + 255) // 256 * 256
+        self.h = C.c_void_p()
+        _check(lib().spiir_bank_init(C.byref(self.h), C.byref(self.desc), C.c_void_p(base), nbytes, _stream()))
+        self.n_det, self.n_templates = n_det, int(bank["n_templates"])
+        self.out_band, self.n_bands = int(bank["out_band"]), len(bank["band_rates"])
+        self.n_slots = self.n_det * self.n_templates
+        self.trig = torch.zeros(self.n_slots, 40, dtype=torch.uint8, device="cuda")
+        self.count = torch.zeros(1, dtype=torch.int32, device="cuda")
+
+    def reset(self):
+        _check(lib().spiir_bank_reset(self.h, _stream()))
+
+    def filter_chunk(self, strain, snr_out=None):
+        """strain: float32 cuda [n_det][n]; snr_out: float32 cuda [n_det][T][n>>out_band][2] or None."""
+        assert strain.is_cuda and strain.is_contiguous() and strain.dtype.is_floating_point and strain.element_size() == 4
+        n = strain.shape[-1]
+        if snr_out is not None:
+            assert snr_out.is_cuda and snr_out.is_contiguous()
+            assert snr_out.numel() == self.n_det * self.n_templates * (n >> self.out_band) * 2
+        _check(lib().spiir_filter_chunk(self.h, C.c_void_p(strain.data_ptr()), n,
+                                        C.c_void_p(snr_out.data_ptr()) if snr_out is not None else None, _stream()))
+
+    def peaks(self, threshold, mode=0):
+        _check(lib().spiir_peaks(self.h, C.c_float(threshold), mode, C.c_void_p(self.trig.data_ptr()),
+                                 C.c_void_p(self.count.data_ptr()), _stream()))
+        return self.trig, self.count
+
+    def snr_view(self):
+        v = spiir_snr_view()
+        _check(lib().spiir_bank_snr_view(self.h, C.byref(v)))
+        return SnrView(raw=v)
+
+    def band_plan(self, band):
+        p = spiir_band_plan()
+        _check(lib().spiir_bank_band_plan(self.h, band, C.byref(p)))
+        return {f[0]: getattr(p, f[0]) for f in spiir_band_plan._fields_}
+
+    def updates_per_chunk(self, n_samples):
+        return int(lib().spiir_bank_updates_per_chunk(self.h, n_samples))
+
+    def close(self):
+        if self.h:
+            lib().spiir_bank_free(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def sky_table_build(nside, pos, resp, sigma, gmst, fs):
+    """Host look-up table (spiir_sky_table_build): returns (u2 float32 [P][D][2], delay int32 [P][D])."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    resp = np.ascontiguousarray(resp, dtype=np.float64)
+    sigma = np.ascontiguousarray(sigma, dtype=np.float64)
+    n_det = pos.shape[0]
+    npix = 12 * nside * nside
+    u2 = np.zeros((npix, n_det, 2), np.float32)
+    delay = np.zeros((npix, n_det), np.int32)
+    _check(lib().spiir_sky_table_build(nside, n_det, _hp(pos), _hp(resp), _hp(sigma), float(gmst), float(fs),
+                                       _hp(u2), _hp(delay)))
+    return u2, delay
+
+
+class SkyPlan:
+    """Owns the workspace of one spiir_sky_plan and the output tensors of its searches."""
+
+    def __init__(self, u2, delay, max_slots):
+        import torch
+        u2 = np.ascontiguousarray(u2, dtype=np.float32)
+        delay = np.ascontiguousarray(delay, dtype=np.int32)
+        self.n_pix, self.n_det = int(u2.shape[0]), int(u2.shape[1])
+        self.max_slots = int(max_slots)
+        nbytes = C.c_size_t(0)
+        _check(lib().spiir_sky_plan_workspace_bytes(self.n_det, self.n_pix, self.max_slots, C.byref(nbytes)))
+        self.ws = torch.empty(nbytes.value + 256, dtype=torch.uint8, device="cuda")
+        base = (self.ws.data_ptr() + 255) // 256 * 256
+        self.h = C.c_void_p()
+        _check(lib().spiir_sky_plan_init(C.byref(self.h), self.n_det, self.n_pix, self.max_slots, _hp(u2), _hp(delay),
+                                         C.c_void_p(base), nbytes, _stream()))
+        self.n_tuples = int(lib().spiir_sky_plan_tuples(self.h))
+
+    def search(self, view, trig, n_slots, out=None, skymap=None):
+        """coherent_sky_search; trig: uint8 cuda [n_slots][40]; returns out float32-bytes cuda [n_slots][16]."""
+        import torch
+        if out is None:
+            out = torch.empty(n_slots, 16, dtype=torch.uint8, device="cuda")
+        _check(lib().coherent_sky_search(self.h, C.byref(view.c), C.c_void_p(trig.data_ptr()), n_slots,
+                                         C.c_void_p(out.data_ptr()),
+                                         C.c_void_p(skymap.data_ptr()) if skymap is not None else None, _stream()))
+        return out
+
+    def background(self, view, trig, n_slots, n_slides, step, mult, out=None):
+        import torch
+        if out is None:
+            out = torch.empty(n_slots * n_slides, 16, dtype=torch.uint8, device="cuda")
+        m = np.ascontiguousarray(mult, dtype=np.int32)
+        _check(lib().timeslide_background(self.h, C.byref(view.c), C.c_void_p(trig.data_ptr()), n_slots, n_slides,
+                                          int(step), _hp(m), C.c_void_p(out.data_ptr()), _stream()))
+        return out
+
+    def close(self):
+        if self.h:
+            lib().spiir_sky_plan_free(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def triggers_to_numpy(trig):
+    return trig.cpu().numpy().view(TRIGGER_DTYPE).reshape(-1)
+
+
+def triggers_from_numpy(arr):
+    import torch
+    arr = np.ascontiguousarray(arr, dtype=TRIGGER_DTYPE)
+    return torch.from_numpy(arr.view(np.uint8).reshape(-1, 40)).cuda()
+
+
+def results_to_numpy(out):
+    return out.cpu().numpy().view(RESULT_DTYPE).reshape(-1)
+
+
+def fp32_peak_probe(reps=20):
+    """(FP32 FMA lane-ops/s, ms) from the library's dependency-free FFMA kernel."""
+    ms, fma = C.c_double(0), C.c_double(0)
+    _check(lib().spiir_fp32_peak_probe(reps, C.byref(ms), C.byref(fma), _stream()))
+    return fma.value * reps / (ms.value * 1e-3), ms.value

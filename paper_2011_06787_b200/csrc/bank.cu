@@ -1,0 +1,453 @@
+// Host side of the filter bank: layout planning, workspace carve-up, streaming
+// state bookkeeping and the C-ABI entry points spiir_bank_* / spiir_filter_chunk.
+// (include/spiir.h documents the contract; DESIGN.md §3-§4 the layout.)
+#include <algorithm>
+#include <cstdarg>
+#include <cstring>
+#include <map>
+#include <numeric>
+
+#include "spiir_internal.cuh"
+
+namespace spiir {
+
+static thread_local std::string g_error;
+static thread_local int64_t g_launches = 0;
+
+void set_error(const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  g_error = buf;
+}
+void count_launch(int n) { g_launches += n; }
+
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
+
+// Host images of the arrays the plan produces (filled only when `fill` is set).
+struct PlanImages {
+  std::vector<float4> coef[SPIIR_MAX_BANDS];
+  std::vector<int32_t> off[SPIIR_MAX_BANDS];
+  std::vector<int32_t> tb_first, tb_count;
+};
+
+static int validate(const spiir_bank_desc* d) {
+  SPIIR_REQUIRE(d != nullptr, "desc is NULL");
+  SPIIR_REQUIRE(d->n_det >= 1 && d->n_det <= SPIIR_MAX_DET, "n_det %d out of range", d->n_det);
+  SPIIR_REQUIRE(d->n_templates >= 1, "n_templates %d", d->n_templates);
+  SPIIR_REQUIRE(d->n_bands >= 1 && d->n_bands <= SPIIR_MAX_BANDS, "n_bands %d out of range", d->n_bands);
+  SPIIR_REQUIRE(d->out_band >= 0 && d->out_band <= 1 && d->out_band < d->n_bands, "out_band %d must be 0 or 1",
+                d->out_band);
+  for (int b = 0; b + 1 < d->n_bands; ++b)
+    SPIIR_REQUIRE(d->band_rate_hz[b] == 2 * d->band_rate_hz[b + 1], "band rates must halve (band %d)", b);
+  SPIIR_REQUIRE(d->host_tmpl_offset && d->host_a && d->host_b && d->host_delay && d->host_band,
+                "a filter array is NULL");
+  SPIIR_REQUIRE(d->n_bands == 1 || (d->host_fir_dec && d->host_fir_int), "FIR taps are NULL");
+  const int gran = 4 << (d->n_bands - 1);
+  SPIIR_REQUIRE(d->max_chunk_samples >= gran && d->max_chunk_samples % gran == 0,
+                "max_chunk_samples %d must be a positive multiple of %d", d->max_chunk_samples, gran);
+  SPIIR_REQUIRE(d->n_bands == 1 || d->max_chunk_samples <= 4096, "max_chunk_samples > 4096 with several bands");
+  SPIIR_REQUIRE(d->max_chunk_samples <= 8192, "max_chunk_samples > 8192");
+  SPIIR_REQUIRE(d->ring_len >= (d->max_chunk_samples >> d->out_band), "ring_len shorter than one chunk");
+  SPIIR_REQUIRE(d->host_tmpl_offset[0] == 0 && d->host_tmpl_offset[d->n_templates] == d->n_filters,
+                "tmpl_offset does not span n_filters");
+  for (int t = 0; t < d->n_templates; ++t)
+    SPIIR_REQUIRE(d->host_tmpl_offset[t + 1] >= d->host_tmpl_offset[t], "tmpl_offset not monotone at %d", t);
+  for (int b = 0; b < d->n_bands; ++b) SPIIR_REQUIRE(d->max_delay[b] >= 0, "max_delay[%d] < 0", b);
+  SPIIR_REQUIRE(d->bank_size >= 1, "bank_size %d must be >= 1", d->bank_size);
+  SPIIR_REQUIRE((d->n_templates + d->bank_size - 1) / d->bank_size <= 65535, "too many template banks");
+  for (int64_t l = 0; l < d->n_filters; ++l) {
+    const int b = d->host_band[l];
+    SPIIR_REQUIRE(b < d->n_bands, "filter %lld: band %d out of range", (long long)l, b);
+    SPIIR_REQUIRE(d->host_delay[l] >= 0 && d->host_delay[l] <= d->max_delay[b],
+                  "filter %lld: delay %d outside [0, max_delay[%d]=%d]", (long long)l, d->host_delay[l], b,
+                  d->max_delay[b]);
+  }
+  return SPIIR_OK;
+}
+
+// Chooses lanes-per-unit G and filters-per-lane F of a band: fewest issue slots
+// for the band's templates (8F FP32 per lane-sample + load + reduction share).
+static void choose_shape(const std::vector<int>& cnt, int* G_out, int* F_out) {
+  double best = 1e300;
+  for (int G : {8, 16, 32})
+    for (int F = 4; F <= 12; ++F) {
+      const double red = (G == 8 ? 28.0 : G == 16 ? 30.0 : 32.0) / 4.0;
+      double cost = 0;
+      for (int c : cnt)
+        if (c > 0) cost += (double)((c + G * F - 1) / (G * F)) * G * (8.0 * F + 0.25 * F + red + 1.0);
+      if (cost < best) { best = cost; *G_out = G; *F_out = F; }
+    }
+}
+
+// Builds the whole device layout.  With img == nullptr only sizes are computed.
+static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
+  const int B = d->n_bands, T = d->n_templates, D = d->n_det;
+  bk->desc = *d;
+  bk->groups.clear();
+  size_t cur = 0;
+  auto take = [&](size_t bytes) { size_t o = cur; cur = align_up(cur + bytes, 256); return o; };
+  if (img) { img->tb_first.assign((size_t)T * B, 0); img->tb_count.assign((size_t)T * B, 0); }
+
+  // per band: filters of each template
+  std::vector<std::vector<int64_t>> ids((size_t)T);
+  std::map<std::tuple<int, int, int>, size_t> group_of;
+  for (int b = 0; b < B; ++b) {
+    spiir_bank_host_band& hb = bk->band[b];
+    hb = spiir_bank_host_band();
+    hb.rate = d->band_rate_hz[b];
+    hb.nmax = d->max_chunk_samples >> b;
+    std::vector<int> cnt(T, 0), maxd(T, 0);
+    for (int t = 0; t < T; ++t) {
+      ids[t].clear();
+      for (int64_t l = d->host_tmpl_offset[t]; l < d->host_tmpl_offset[t + 1]; ++l)
+        if (d->host_band[l] == b) { ids[t].push_back(l); maxd[t] = std::max(maxd[t], d->host_delay[l]); }
+      cnt[t] = (int)ids[t].size();
+      hb.n_filters += cnt[t];
+    }
+    choose_shape(cnt, &hb.G, &hb.F);
+    const int G = hb.G, F = hb.F, cap_unit = G * F, upw = 32 / G;
+    hb.Hcap = std::max(32, round_up(d->max_delay[b], 4));
+    const int nsubmax = std::min(hb.nmax, kSubChunkMax);
+    // shared history depth: covers >= 98 % of the filters, bounded by the smem budget
+    {
+      std::vector<std::pair<int, int>> v;
+      for (int t = 0; t < T; ++t) if (cnt[t]) v.push_back({maxd[t], cnt[t]});
+      std::sort(v.begin(), v.end());
+      int64_t acc = 0; int h98 = 0;
+      for (auto& e : v) { acc += e.second; h98 = e.first; if (acc * 100 >= hb.n_filters * 98) break; }
+      const int budget = kSmemFloatsMax - nsubmax;
+      int Hs = round_up(std::max(h98, 1), 64);
+      if (hb.Hcap <= budget && hb.Hcap <= Hs + Hs / 4) Hs = hb.Hcap;
+      hb.Hs = std::min(std::min(Hs, budget / 4 * 4), hb.Hcap);
+    }
+    hb.cap = round_up(hb.Hcap + hb.nmax + 4, 32);
+    hb.reps = hb.Hs + nsubmax;
+    // units: short classes first
+    std::vector<int> first(T, 0), nun(T, 0);
+    int nus = 0, nul = 0;
+    for (int t = 0; t < T; ++t) {
+      nun[t] = (cnt[t] + cap_unit - 1) / cap_unit;
+      if (cnt[t] && maxd[t] <= hb.Hs) { first[t] = nus; nus += nun[t]; }
+    }
+    const int nus_pad = round_up(nus, upw);
+    for (int t = 0; t < T; ++t)
+      if (cnt[t] && maxd[t] > hb.Hs) { first[t] = nus_pad + nul; nul += nun[t]; }
+    const int nul_pad = round_up(nul, upw);
+    hb.n_units = nus_pad + nul_pad;
+    hb.n_units_long = nul_pad;
+    hb.n_wu_short = nus_pad / upw;
+    hb.n_wu_long = nul_pad / upw;
+    const size_t slots = (size_t)hb.n_units * cap_unit;
+    hb.off_coef = take(slots * sizeof(float4));
+    hb.off_off = take(slots * sizeof(int32_t));
+    // launch groups, one per (G, F, class); CTAs listed band by band (heaviest band first)
+    for (int cls = 0; cls < 2; ++cls) {
+      const int nwu = cls ? hb.n_wu_long : hb.n_wu_short;
+      if (!nwu) continue;
+      auto key = std::make_tuple(G, F, cls);
+      if (!group_of.count(key)) {
+        group_of[key] = bk->groups.size();
+        spiir_launch_group g; g.G = G; g.F = F; g.xg = cls;
+        bk->groups.push_back(g);
+      }
+      spiir_launch_group& g = bk->groups[group_of[key]];
+      const int wu0 = cls ? hb.n_wu_short : 0;
+      for (int w = 0; w < nwu; w += kBankWarps)
+        g.work.push_back(CtaWork{b, wu0 + w, wu0 + std::min(nwu, w + kBankWarps), 0});
+      if (!cls) g.smem_bytes = std::max(g.smem_bytes, kReplicas * hb.reps * 4 + 16);
+    }
+    if (img) {
+      img->coef[b].assign(slots, make_float4(0.f, 0.f, 0.f, 0.f));
+      img->off[b].assign(slots, 0);
+      const int prpu = F * (G / 8);                          // phase-rows per unit
+      std::vector<std::pair<int, int64_t>> order;
+      for (int t = 0; t < T; ++t) {
+        img->tb_first[(size_t)t * B + b] = first[t];
+        img->tb_count[(size_t)t * B + b] = nun[t];
+        if (!cnt[t]) continue;
+        const bool lng = maxd[t] > hb.Hs;
+        order.clear();
+        for (int64_t l : ids[t]) {
+          const int dl = d->host_delay[l];
+          const int e = (lng ? hb.Hcap : hb.Hs) - dl;
+          const int al = e & 3;
+          const int off = al * (lng ? hb.cap : hb.reps) + (e - al);
+          order.push_back({((off >> 2) & 7), l});
+          (void)off;
+        }
+        // deal the filters, sorted by their 16-byte bank group, round-robin over the
+        // phase-rows (8 lanes x one LDS.128) so that equal groups land in different rows
+        std::stable_sort(order.begin(), order.end(),
+                         [](const std::pair<int, int64_t>& x, const std::pair<int, int64_t>& y) { return x.first < y.first; });
+        const int PR = nun[t] * prpu;
+        for (size_t j = 0; j < order.size(); ++j) {
+          const int64_t l = order[j].second;
+          const int pr = (int)(j % PR), pos = (int)(j / PR);
+          const int ul = pr / prpu, rem = pr % prpu, f = rem / (G / 8), half = rem % (G / 8);
+          const int unit = first[t] + ul, g8 = half * 8 + pos;
+          const int wu = unit / upw, lane = (unit % upw) * G + g8;
+          const size_t slot = ((size_t)wu * F + f) * 32 + lane;
+          const int dl = d->host_delay[l];
+          const int e = (lng ? hb.Hcap : hb.Hs) - dl;
+          const int al = e & 3;
+          img->coef[b][slot] = make_float4(d->host_a[l].re, d->host_a[l].im, d->host_b[l].re, d->host_b[l].im);
+          img->off[b][slot] = al * (lng ? hb.cap : hb.reps) + (e - al);
+        }
+      }
+    }
+  }
+  // carried state (zeroed by reset) is laid out contiguously
+  bk->off_state_begin = cur;
+  for (int b = 0; b < B; ++b) {
+    spiir_bank_host_band& hb = bk->band[b];
+    const size_t slots = (size_t)hb.n_units * hb.G * hb.F;
+    hb.off_state = take((size_t)D * slots * sizeof(float2));
+    hb.off_x[0] = take((size_t)D * kReplicas * hb.cap * sizeof(float));
+    hb.off_x[1] = take((size_t)D * kReplicas * hb.cap * sizeof(float));
+    hb.off_uphist = take((size_t)D * T * kUpHist * sizeof(float2));
+  }
+  bk->off_peak = take((size_t)D * T * sizeof(PeakRec));
+  bk->off_ring = take((size_t)D * T * (size_t)d->ring_len * sizeof(float2));
+  bk->bytes_state_total = cur - bk->off_state_begin;
+  for (int b = 0; b < B; ++b) {
+    spiir_bank_host_band& hb = bk->band[b];
+    hb.off_S = take((size_t)D * hb.n_units * hb.nmax * sizeof(float2));
+  }
+  bk->off_tb_first = take((size_t)T * B * sizeof(int32_t));
+  bk->off_tb_count = take((size_t)T * B * sizeof(int32_t));
+  bk->off_taps = take(2 * SPIIR_FIR_TAPS * sizeof(float));
+  const int n_out_max = d->max_chunk_samples >> d->out_band;
+  const int n_banks = (T + std::max(1, d->bank_size) - 1) / std::max(1, d->bank_size);
+  (void)n_out_max; (void)n_banks;
+  bk->off_m1 = take((size_t)D * T * sizeof(unsigned long long));
+  for (auto& g : bk->groups) g.off_work = take(g.work.size() * sizeof(CtaWork));
+  bk->ws_bytes = cur;
+  return SPIIR_OK;
+}
+
+}  // namespace spiir
+
+using namespace spiir;
+
+extern "C" {
+
+const char* spiir_last_error(void) { return g_error.c_str(); }
+int64_t spiir_launch_count(void) { return g_launches; }
+
+int spiir_bank_workspace_bytes(const spiir_bank_desc* desc, size_t* bytes) {
+  int rc = validate(desc);
+  if (rc) return rc;
+  SPIIR_REQUIRE(bytes != nullptr, "bytes is NULL");
+  spiir_bank tmp;
+  rc = plan(desc, &tmp, nullptr);
+  if (rc) return rc;
+  *bytes = tmp.ws_bytes;
+  return SPIIR_OK;
+}
+
+int spiir_bank_init(spiir_bank** out, const spiir_bank_desc* desc, void* dev_workspace, size_t bytes, void* stream) {
+  int rc = validate(desc);
+  if (rc) return rc;
+  SPIIR_REQUIRE(out && dev_workspace, "out or workspace is NULL");
+  SPIIR_REQUIRE(((uintptr_t)dev_workspace & 255) == 0, "workspace must be 256-byte aligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  spiir_bank* bk = new spiir_bank();
+  PlanImages img;
+  rc = plan(desc, bk, &img);
+  if (rc) { delete bk; return rc; }
+  if (bytes < bk->ws_bytes) {
+    set_error("workspace too small: %zu < %zu", bytes, bk->ws_bytes);
+    delete bk;
+    return SPIIR_ENOMEM;
+  }
+  bk->ws = (char*)dev_workspace;
+  auto fail = [&](cudaError_t e, const char* what) {
+    set_error("%s failed: %s", what, cudaGetErrorString(e));
+    delete bk;
+    return SPIIR_ECUDA;
+  };
+  cudaError_t e;
+  for (int b = 0; b < desc->n_bands; ++b) {
+    auto& hb = bk->band[b];
+    if (!img.coef[b].empty()) {
+      e = cudaMemcpyAsync(bk->ws + hb.off_coef, img.coef[b].data(), img.coef[b].size() * sizeof(float4),
+                          cudaMemcpyHostToDevice, st);
+      if (e != cudaSuccess) return fail(e, "copy coef");
+      e = cudaMemcpyAsync(bk->ws + hb.off_off, img.off[b].data(), img.off[b].size() * sizeof(int32_t),
+                          cudaMemcpyHostToDevice, st);
+      if (e != cudaSuccess) return fail(e, "copy off");
+    }
+  }
+  e = cudaMemcpyAsync(bk->ws + bk->off_tb_first, img.tb_first.data(), img.tb_first.size() * 4, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return fail(e, "copy tb_first");
+  e = cudaMemcpyAsync(bk->ws + bk->off_tb_count, img.tb_count.data(), img.tb_count.size() * 4, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return fail(e, "copy tb_count");
+  float taps[2 * SPIIR_FIR_TAPS] = {0};
+  if (desc->host_fir_dec) memcpy(taps, desc->host_fir_dec, SPIIR_FIR_TAPS * sizeof(float));
+  if (desc->host_fir_int) memcpy(taps + SPIIR_FIR_TAPS, desc->host_fir_int, SPIIR_FIR_TAPS * sizeof(float));
+  e = cudaMemcpyAsync(bk->ws + bk->off_taps, taps, sizeof(taps), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return fail(e, "copy taps");
+  for (auto& g : bk->groups) {
+    e = cudaMemcpyAsync(bk->ws + g.off_work, g.work.data(), g.work.size() * sizeof(CtaWork), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail(e, "copy work");
+  }
+  // the host images die with this scope: wait for the copies
+  e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(e, "cudaStreamSynchronize");
+  // host pointers of the caller are not kept
+  bk->desc.host_tmpl_offset = nullptr; bk->desc.host_a = nullptr; bk->desc.host_b = nullptr;
+  bk->desc.host_delay = nullptr; bk->desc.host_band = nullptr; bk->desc.host_fir_dec = nullptr;
+  bk->desc.host_fir_int = nullptr;
+  rc = spiir_bank_reset(bk, stream);
+  if (rc) { delete bk; return rc; }
+  *out = bk;
+  return SPIIR_OK;
+}
+
+int spiir_bank_reset(spiir_bank* bk, void* stream) {
+  SPIIR_REQUIRE(bk != nullptr, "bank is NULL");
+  SPIIR_CUDA_OK(cudaMemsetAsync(bk->ws + bk->off_state_begin, 0, bk->bytes_state_total, (cudaStream_t)stream));
+  bk->parity = 0;
+  bk->k_next = 0;
+  bk->last_n_out = 0;
+  bk->last_k0 = 0;
+  for (int b = 0; b < bk->desc.n_bands; ++b) bk->band[b].prev_n = 0;
+  return SPIIR_OK;
+}
+
+int spiir_bank_free(spiir_bank* bk) {
+  SPIIR_REQUIRE(bk != nullptr, "bank is NULL");
+  delete bk;
+  return SPIIR_OK;
+}
+
+int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_samples, spiir_c32* dev_snr_out,
+                       void* stream) {
+  SPIIR_REQUIRE(bk != nullptr && dev_strain != nullptr, "bank or strain is NULL");
+  const spiir_bank_desc& d = bk->desc;
+  const int B = d.n_bands, D = d.n_det, T = d.n_templates;
+  const int gran = 4 << (B - 1);
+  SPIIR_REQUIRE(n_samples > 0 && n_samples % gran == 0 && n_samples <= d.max_chunk_samples,
+                "n_samples %d must be a positive multiple of %d and <= %d", n_samples, gran, d.max_chunk_samples);
+  SPIIR_REQUIRE(((uintptr_t)dev_strain & 15) == 0, "dev_strain must be 16-byte aligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int newp = bk->parity ^ 1;
+
+  PrepParams pp;
+  memset(&pp, 0, sizeof(pp));
+  pp.strain = dev_strain; pp.n0 = n_samples; pp.n_bands = B;
+  pp.taps_dec = (const float*)(bk->ws + bk->off_taps);
+  BankParams P;
+  memset(&P, 0, sizeof(P));
+  for (int b = 0; b < B; ++b) {
+    auto& hb = bk->band[b];
+    const int n = n_samples >> b;
+    pp.xnew[b] = (float*)(bk->ws + hb.off_x[newp]);
+    pp.xold[b] = (const float*)(bk->ws + hb.off_x[bk->parity]);
+    pp.x_det_stride[b] = (int64_t)kReplicas * hb.cap;
+    pp.cap[b] = hb.cap; pp.Hcap[b] = hb.Hcap; pp.n[b] = n; pp.prev_n[b] = hb.prev_n;
+    BandDev& bd = P.band[b];
+    const size_t slots = (size_t)hb.n_units * hb.G * hb.F;
+    bd.coef = (const float4*)(bk->ws + hb.off_coef);
+    bd.off = (const int32_t*)(bk->ws + hb.off_off);
+    bd.state = (float2*)(bk->ws + hb.off_state);
+    bd.S = (float2*)(bk->ws + hb.off_S);
+    bd.xrep = pp.xnew[b];
+    bd.x_det_stride = pp.x_det_stride[b];
+    bd.state_det_stride = (int64_t)slots;
+    bd.S_det_stride = (int64_t)hb.n_units * hb.nmax;
+    bd.n = n; bd.nmax = hb.nmax; bd.Hcap = hb.Hcap; bd.Hs = hb.Hs; bd.cap = hb.cap; bd.reps = hb.reps;
+    bd.nsub = std::min(n, std::min(hb.nmax, kSubChunkMax));
+  }
+  launch_prep(pp, D, st);
+  SPIIR_CUDA_OK(cudaGetLastError());
+  for (auto& g : bk->groups) {
+    int rc = launch_bank_group(g.G, g.F, g.xg, P, (const CtaWork*)(bk->ws + g.off_work), (int)g.work.size(), D,
+                               g.xg ? 0 : g.smem_bytes, st);
+    if (rc) return rc;
+  }
+  CombineParams cp;
+  memset(&cp, 0, sizeof(cp));
+  for (int b = 0; b < B; ++b) {
+    auto& hb = bk->band[b];
+    cp.S[b] = (const float2*)(bk->ws + hb.off_S);
+    cp.S_det_stride[b] = (int64_t)hb.n_units * hb.nmax;
+    cp.nmax[b] = hb.nmax; cp.n[b] = n_samples >> b;
+    cp.uphist[b] = (float2*)(bk->ws + hb.off_uphist);
+  }
+  cp.tb_first = (const int32_t*)(bk->ws + bk->off_tb_first);
+  cp.tb_count = (const int32_t*)(bk->ws + bk->off_tb_count);
+  cp.taps_int = (const float*)(bk->ws + bk->off_taps) + SPIIR_FIR_TAPS;
+  cp.ring = (float2*)(bk->ws + bk->off_ring);
+  cp.ring_len = d.ring_len; cp.ring_det_stride = (int64_t)T * d.ring_len;
+  cp.snr_out = (float2*)dev_snr_out;
+  cp.n_out = n_samples >> d.out_band;
+  cp.k0 = bk->k_next;
+  cp.peak = (PeakRec*)(bk->ws + bk->off_peak);
+  cp.B = B; cp.out_band = d.out_band; cp.T = T;
+  cp.bufA = kUpHist + (d.max_chunk_samples >> d.out_band);
+  cp.bufB = (B - 1 > d.out_band) ? kUpHist + (d.max_chunk_samples >> (d.out_band + 1)) : 0;
+  launch_combine(cp, D, st);
+  SPIIR_CUDA_OK(cudaGetLastError());
+
+  bk->parity = newp;
+  for (int b = 0; b < B; ++b) bk->band[b].prev_n = n_samples >> b;
+  bk->last_k0 = bk->k_next;
+  bk->last_n_out = cp.n_out;
+  bk->k_next += cp.n_out;
+  return SPIIR_OK;
+}
+
+int spiir_peaks(spiir_bank* bk, float snr_threshold, int32_t mode, spiir_trigger* dev_trig, int32_t* dev_count,
+                void* stream) {
+  SPIIR_REQUIRE(bk && dev_trig && dev_count, "bank, dev_trig or dev_count is NULL");
+  SPIIR_REQUIRE(mode == 0 || mode == 1, "mode %d must be 0 or 1", mode);
+  SPIIR_REQUIRE(snr_threshold >= 0.f, "snr_threshold must be >= 0");
+  SPIIR_REQUIRE(bk->last_n_out > 0, "spiir_peaks before the first spiir_filter_chunk");
+  const spiir_bank_desc& d = bk->desc;
+  PeakParams p;
+  memset(&p, 0, sizeof(p));
+  p.peak = (const PeakRec*)(bk->ws + bk->off_peak);
+  p.ring = (const float2*)(bk->ws + bk->off_ring);
+  p.ring_len = d.ring_len; p.ring_det_stride = (int64_t)d.n_templates * d.ring_len;
+  p.key = (unsigned long long*)(bk->ws + bk->off_m1);
+  p.k0 = bk->last_k0; p.n = bk->last_n_out;
+  p.T = d.n_templates; p.D = d.n_det; p.bank_size = d.bank_size;
+  p.thr2 = snr_threshold * snr_threshold;       // float32 product, as the oracle's decision path
+  p.trig = dev_trig; p.count = dev_count;
+  return launch_peaks(p, mode, (cudaStream_t)stream);
+}
+
+int spiir_bank_snr_view(const spiir_bank* bk, spiir_snr_view* view) {
+  SPIIR_REQUIRE(bk && view, "bank or view is NULL");
+  view->dev_z = (const spiir_c32*)(bk->ws + bk->off_ring);
+  view->row_stride = bk->desc.ring_len;
+  view->det_stride = (int64_t)bk->desc.n_templates * bk->desc.ring_len;
+  view->ring_len = bk->desc.ring_len;
+  view->k_newest = bk->k_next - 1;
+  return SPIIR_OK;
+}
+
+int spiir_bank_band_plan(const spiir_bank* bk, int32_t band, spiir_band_plan* p) {
+  SPIIR_REQUIRE(bk && p && band >= 0 && band < bk->desc.n_bands, "bad arguments");
+  const auto& hb = bk->band[band];
+  p->lanes_per_unit = hb.G; p->filters_per_lane = hb.F;
+  p->n_units = hb.n_units; p->n_units_long = hb.n_units_long;
+  p->smem_history = hb.Hs; p->smem_bytes = kReplicas * hb.reps * 4 + 16;
+  p->n_filters = hb.n_filters; p->n_slots = (int64_t)hb.n_units * hb.G * hb.F;
+  return SPIIR_OK;
+}
+
+int64_t spiir_bank_updates_per_chunk(const spiir_bank* bk, int32_t n_samples) {
+  if (!bk) return 0;
+  int64_t u = 0;
+  for (int b = 0; b < bk->desc.n_bands; ++b) u += bk->band[b].n_filters * (int64_t)(n_samples >> b);
+  return u * bk->desc.n_det;
+}
+
+}  // extern "C"

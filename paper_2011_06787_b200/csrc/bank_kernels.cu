@@ -1,0 +1,382 @@
+// Device kernels of the SPIIR filter bank (H0-H3 of DESIGN.md) for sm_100a.
+//
+//   k_prep    H0  history shift + x2 decimator chain + 4 pre-shifted replicas per band
+//   k_bank    H1+H2 delay fetch + IIR recursion + per-unit band sums (THE hot loop)
+//   k_combine H3  unit sums -> band sums -> interpolating cascade -> SNR ring, fused
+//                 per-template peak tracking (H4 mode 0)
+//
+// PAPER.md:129 (Eq. 8): y_l[k] = a_l y_l[k-1] + b_l x[k-d_l]; z[k] = sum_l y_l[k];
+// templates and filters are independent -> GPU threads.  The mapping,
+// the replica trick and the reduction are this implementation's own.
+#include "spiir_internal.cuh"
+
+namespace spiir {
+
+// ---------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// 1-D TMA bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// ------------------------------------------------------------------- k_prep
+
+constexpr int kPrepThreads = 512;
+constexpr int kPrepStage = 4096 + 32;
+
+__global__ void __launch_bounds__(kPrepThreads) k_prep(PrepParams p) {
+  __shared__ __align__(16) float stage[kPrepStage];
+  __shared__ float g[SPIIR_FIR_TAPS];
+  const int det = blockIdx.x, tid = threadIdx.x;
+  if (tid < SPIIR_FIR_TAPS) g[tid] = p.taps_dec[tid];
+  for (int b = 0; b < p.n_bands; ++b) {
+    float* xn = p.xnew[b] + det * p.x_det_stride[b];
+    const float* xo = p.xold[b] + det * p.x_det_stride[b];
+    const int H = p.Hcap[b], n = p.n[b], pn = p.prev_n[b], cap = p.cap[b];
+    // (a) carry the last H samples of the previous layout to the front of the new one
+    for (int j = tid; j < H; j += kPrepThreads) xn[j] = xo[pn + j];
+    // (b) the new samples of this band
+    if (b == 0) {
+      const float4* src = reinterpret_cast<const float4*>(p.strain + (size_t)det * p.n0);
+      float4* dst = reinterpret_cast<float4*>(xn + H);
+      for (int j = tid; j < n / 4; j += kPrepThreads) dst[j] = __ldg(src + j);   // coalesced float4 loads
+    } else {
+      // x_b[m] = sum_j g[j] x_{b-1}[2m+1-j]: stage band b-1 (31 samples of history + its new
+      // samples) in shared memory with float4 loads, then every thread forms outputs.
+      const float* xp = p.xnew[b - 1] + det * p.x_det_stride[b - 1] + p.Hcap[b - 1] - 32;
+      const int np = p.n[b - 1] + 32;
+      __syncthreads();                       // band b-1 complete, previous use of stage[] finished
+      for (int j = tid; j < np / 4; j += kPrepThreads)
+        reinterpret_cast<float4*>(stage)[j] = reinterpret_cast<const float4*>(xp)[j];
+      __syncthreads();
+      for (int m = tid; m < n; m += kPrepThreads) {
+        float acc = 0.f;
+#pragma unroll
+        for (int j = 0; j < SPIIR_FIR_TAPS; ++j) acc = fmaf(g[j], stage[32 + 2 * m + 1 - j], acc);
+        xn[H + m] = acc;
+      }
+    }
+    __syncthreads();
+    // (c) replicas r = 1..3: rep_r[j] = rep_0[j + r]  (aligned float4 reads for any delay)
+    const int tot = H + n;
+    for (int j = tid; j < tot; j += kPrepThreads) {
+#pragma unroll
+      for (int r = 1; r < kReplicas; ++r) xn[(size_t)r * cap + j] = (j + r < tot) ? xn[j + r] : 0.f;
+    }
+  }
+}
+
+void launch_prep(const PrepParams& p, int n_det, cudaStream_t st) {
+  k_prep<<<n_det, kPrepThreads, 0, st>>>(p);
+  count_launch();
+}
+
+// ------------------------------------------------------------------- k_bank
+// Sum 8 per-lane values (4 complex samples) over the G lanes of a unit.  After the
+// three halving steps lane (g & 7) holds element (g & 7) summed over its 8-lane
+// group; wider units finish with plain butterflies.
+template <int G>
+__device__ __forceinline__ float reduce8(float (&s)[8], int lane) {
+  float w[4], u[2], t;
+  const bool b4 = lane & 4, b2 = lane & 2, b1 = lane & 1;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float send = b4 ? s[j] : s[j + 4];
+    const float keep = b4 ? s[j + 4] : s[j];
+    w[j] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+  }
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const float send = b2 ? w[j] : w[j + 2];
+    const float keep = b2 ? w[j + 2] : w[j];
+    u[j] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+  }
+  {
+    const float send = b1 ? u[0] : u[1];
+    const float keep = b1 ? u[1] : u[0];
+    t = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+  }
+  if (G >= 16) t += __shfl_xor_sync(0xffffffffu, t, 8);
+  if (G >= 32) t += __shfl_xor_sync(0xffffffffu, t, 16);
+  return t;
+}
+
+template <int F>
+struct FilterRegs {
+  float ar[F], ai[F], br[F], bi[F], yr[F], yi[F];
+  int off[F];
+};
+
+// Four consecutive samples of all F filters of this lane; s[] receives the lane's
+// partial sums (re0, im0, re1, im1, ...).  Per update: FMUL + 2 FFMA per component
+// and one FADD per component into the sum = 8 FP32 instructions (12 flop).
+template <int F, bool XG>
+__device__ __forceinline__ void step4(FilterRegs<F>& r, const float* __restrict__ x, int i, float (&s)[8]) {
+#pragma unroll
+  for (int f = 0; f < F; ++f) {
+    float4 xv;
+    if (XG) xv = __ldg(reinterpret_cast<const float4*>(x + r.off[f] + i));
+    else    xv = *reinterpret_cast<const float4*>(x + r.off[f] + i);
+    const float xs[4] = {xv.x, xv.y, xv.z, xv.w};
+    float yr = r.yr[f], yi = r.yi[f];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const float tr = fmaf(-r.ai[f], yi, r.br[f] * xs[q]);
+      const float ti = fmaf(r.ai[f], yr, r.bi[f] * xs[q]);
+      const float nr = fmaf(r.ar[f], yr, tr);
+      const float ni = fmaf(r.ar[f], yi, ti);
+      yr = nr; yi = ni;
+      if (f == 0) { s[2 * q] = yr; s[2 * q + 1] = yi; }
+      else        { s[2 * q] += yr; s[2 * q + 1] += yi; }
+    }
+    r.yr[f] = yr; r.yi[f] = yi;
+  }
+}
+
+template <int G, int F, bool XG>
+__global__ void __launch_bounds__(kBankThreads, 2)
+k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
+  extern __shared__ __align__(128) float xs[];
+  const CtaWork w = work[blockIdx.x];
+  const BandDev& B = P.band[w.band];
+  const int det = blockIdx.y;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int wu = w.wu_begin + warp;
+  const bool active = wu < w.wu_end;
+
+  FilterRegs<F> r;
+  const size_t slot0 = ((size_t)wu * F) * 32 + lane;
+  float2* st = B.state + (size_t)det * B.state_det_stride;
+  if (active) {
+#pragma unroll
+    for (int f = 0; f < F; ++f) {
+      const float4 c = __ldg(B.coef + slot0 + f * 32);
+      r.ar[f] = c.x; r.ai[f] = c.y; r.br[f] = c.z; r.bi[f] = c.w;
+      r.off[f] = __ldg(B.off + slot0 + f * 32);
+      const float2 y = st[slot0 + f * 32];
+      r.yr[f] = y.x; r.yi[f] = y.y;
+    }
+  }
+  constexpr int UPW = 32 / G;                        // units per warp
+  const int unit = wu * UPW + lane / G;
+  const int g = lane % G;
+  float* Sout = reinterpret_cast<float*>(B.S + (size_t)det * B.S_det_stride + (size_t)unit * B.nmax);
+  const int n = B.n;
+
+  if (XG) {
+    // long-delay units: read the replicas straight from global memory (L1/L2 resident)
+    if (active) {
+      const float* x = B.xrep + (size_t)det * B.x_det_stride;
+      for (int i = 0; i < n; i += 4) {
+        float s[8];
+        step4<F, true>(r, x, i, s);
+        const float t = reduce8<G>(s, lane);
+        if (g < 8) Sout[2 * i + g] = t;
+      }
+    }
+  } else {
+    uint64_t* bar = reinterpret_cast<uint64_t*>(xs + kReplicas * B.reps);
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    __syncthreads();
+    uint32_t phase = 0;
+    const float* src0 = B.xrep + (size_t)det * B.x_det_stride + (B.Hcap - B.Hs);
+    for (int m0 = 0; m0 < n; m0 += B.nsub) {
+      const int len = min(B.nsub, n - m0);
+      if (m0 > 0) __syncthreads();                   // every warp finished reading the previous window
+      if (threadIdx.x == 0) {
+        const uint32_t bytes = (uint32_t)(B.Hs + len) * 4u;
+        mbar_expect_tx(bar, bytes * kReplicas);
+#pragma unroll
+        for (int rep = 0; rep < kReplicas; ++rep)
+          tma_load_1d(xs + rep * B.reps, src0 + (size_t)rep * B.cap + m0, bytes, bar);
+      }
+      mbar_wait(bar, phase);
+      phase ^= 1u;
+      if (active) {
+        float* So = Sout + 2 * m0;
+        for (int i = 0; i < len; i += 4) {
+          float s[8];
+          step4<F, false>(r, xs, i, s);
+          const float t = reduce8<G>(s, lane);
+          if (g < 8) So[2 * i + g] = t;
+        }
+      }
+    }
+  }
+  if (active) {
+#pragma unroll
+    for (int f = 0; f < F; ++f) st[slot0 + f * 32] = make_float2(r.yr[f], r.yi[f]);
+  }
+}
+
+template <int G, int F, bool XG>
+static int launch_one(const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det, int smem, cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_bank<G, F, XG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    configured = true;
+  }
+  k_bank<G, F, XG><<<dim3(n_cta, n_det), kBankThreads, smem, st>>>(P, dev_work);
+  count_launch();
+  SPIIR_CUDA_OK(cudaGetLastError());
+  return SPIIR_OK;
+}
+
+#define SPIIR_F_CASES(G, XG)                                                          \
+  switch (F) {                                                                        \
+    case 4:  return launch_one<G, 4, XG>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 5:  return launch_one<G, 5, XG>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 6:  return launch_one<G, 6, XG>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 7:  return launch_one<G, 7, XG>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 8:  return launch_one<G, 8, XG>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 9:  return launch_one<G, 9, XG>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 10: return launch_one<G, 10, XG>(P, dev_work, n_cta, n_det, smem, st);       \
+    case 11: return launch_one<G, 11, XG>(P, dev_work, n_cta, n_det, smem, st);       \
+    case 12: return launch_one<G, 12, XG>(P, dev_work, n_cta, n_det, smem, st);       \
+    default: break;                                                                   \
+  }
+
+int launch_bank_group(int G, int F, int xg, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
+                      int smem, cudaStream_t st) {
+  if (!xg) {
+    if (G == 8) { SPIIR_F_CASES(8, false) }
+    else if (G == 16) { SPIIR_F_CASES(16, false) }
+    else if (G == 32) { SPIIR_F_CASES(32, false) }
+  } else {
+    if (G == 8) { SPIIR_F_CASES(8, true) }
+    else if (G == 16) { SPIIR_F_CASES(16, true) }
+    else if (G == 32) { SPIIR_F_CASES(32, true) }
+  }
+  set_error("no kernel instance for G=%d F=%d", G, F);
+  return SPIIR_EINVAL;
+}
+
+// ---------------------------------------------------------------- k_combine
+
+constexpr int kCombineThreads = 256;
+
+__device__ __forceinline__ float2 unit_sum(const float2* __restrict__ S, int nmax, int first, int count, int m) {
+  float2 a = make_float2(0.f, 0.f);
+  for (int u = 0; u < count; ++u) {
+    const float2 v = S[(size_t)(first + u) * nmax + m];
+    a.x += v.x; a.y += v.y;
+  }
+  return a;
+}
+
+__global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_constant__ CombineParams p) {
+  extern __shared__ __align__(16) float2 cbuf[];
+  __shared__ float h[SPIIR_FIR_TAPS];
+  __shared__ float red_m2[kCombineThreads / 32];
+  __shared__ int red_k[kCombineThreads / 32];
+  const int t = blockIdx.x, det = blockIdx.y, tid = threadIdx.x;
+  if (tid < SPIIR_FIR_TAPS) h[tid] = p.taps_int[tid];
+  float2* buf[2] = {cbuf, cbuf + p.bufA};
+  const int B = p.B, ob = p.out_band;
+
+  // acc_{B-1} = s_{B-1}, then acc_b = s_b + up2(acc_{b+1}) down to the output band
+  for (int b = B - 1; b >= ob; --b) {
+    float2* cur = buf[(b - ob) & 1];
+    const int n = p.n[b];
+    const float2* S = p.S[b] + (size_t)det * p.S_det_stride[b];
+    const int first = p.tb_first[t * B + b], count = p.tb_count[t * B + b];
+    float2* hist = (b > ob) ? p.uphist[b] + ((size_t)det * p.T + t) * kUpHist : nullptr;
+    if (hist && tid < kUpHist) cur[tid] = hist[tid];
+    if (b == B - 1) {
+      for (int m = tid; m < n; m += kCombineThreads) cur[kUpHist + m] = unit_sum(S, p.nmax[b], first, count, m);
+    } else {
+      const float2* src = buf[(b + 1 - ob) & 1];
+      for (int m = tid; m < n; m += kCombineThreads) {
+        float2 a = unit_sum(S, p.nmax[b], first, count, m);
+        const int par = m & 1, c = kUpHist + (m >> 1);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+          const float hv = h[2 * q + par];
+          const float2 v = src[c - q];
+          a.x = fmaf(hv, v.x, a.x);
+          a.y = fmaf(hv, v.y, a.y);
+        }
+        cur[kUpHist + m] = a;
+      }
+    }
+    __syncthreads();
+    if (hist && tid < kUpHist) hist[tid] = cur[n + tid];       // last 15 of [old history | new samples]
+  }
+
+  // output samples, ring append, fused per-template maximum (H4 mode 0)
+  const float2* acc = buf[0] + kUpHist;
+  const int n_out = p.n_out;
+  const float2* S0 = (ob == 1) ? p.S[0] + (size_t)det * p.S_det_stride[0] : nullptr;
+  const int first0 = (ob == 1) ? p.tb_first[t * B] : 0, count0 = (ob == 1) ? p.tb_count[t * B] : 0;
+  float2* ring = p.ring + (size_t)det * p.ring_det_stride + (size_t)t * p.ring_len;
+  float2* out = p.snr_out ? p.snr_out + ((size_t)det * p.T + t) * n_out : nullptr;
+  float best = -1.f; int bk = 0; float2 bz = make_float2(0.f, 0.f);
+  for (int m = tid; m < n_out; m += kCombineThreads) {
+    float2 z = acc[m];
+    if (ob == 1) {                                             // band 0 runs at twice the output rate (M5)
+      const float2 v = unit_sum(S0, p.nmax[0], first0, count0, 2 * m + 1);
+      z.x += v.x; z.y += v.y;
+    }
+    ring[(p.k0 + m) % p.ring_len] = z;
+    if (out) out[m] = z;
+    const float m2 = __fadd_rn(__fmul_rn(z.x, z.x), __fmul_rn(z.y, z.y));
+    if (m2 > best) { best = m2; bk = m; bz = z; }
+  }
+  const int mybk = bk;
+  // block arg-max, lowest k on ties
+  for (int o = 16; o; o >>= 1) {
+    const float om = __shfl_xor_sync(0xffffffffu, best, o);
+    const int ok = __shfl_xor_sync(0xffffffffu, bk, o);
+    if (om > best || (om == best && ok < bk)) { best = om; bk = ok; }
+  }
+  if ((tid & 31) == 0) { red_m2[tid >> 5] = best; red_k[tid >> 5] = bk; }
+  __syncthreads();
+  float fb = red_m2[0]; int fk = red_k[0];
+  for (int wv = 1; wv < kCombineThreads / 32; ++wv)
+    if (red_m2[wv] > fb || (red_m2[wv] == fb && red_k[wv] < fk)) { fb = red_m2[wv]; fk = red_k[wv]; }
+  if (fk % kCombineThreads == tid && fb >= 0.f) {              // the thread that owns sample fk holds its z
+    // bz belongs to this thread's own best; recompute from the ring if they differ
+    float2 z = (mybk == fk) ? bz : ring[(p.k0 + fk) % p.ring_len];
+    PeakRec rec; rec.k = p.k0 + fk; rec.zr = z.x; rec.zi = z.y; rec.m2 = fb; rec._pad = 0;
+    p.peak[(size_t)det * p.T + t] = rec;
+  }
+}
+
+void launch_combine(const CombineParams& p, int n_det, cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    cudaFuncSetAttribute(k_combine, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    configured = true;
+  }
+  const size_t smem = (size_t)(p.bufA + p.bufB) * sizeof(float2);
+  k_combine<<<dim3(p.T, n_det), kCombineThreads, smem, st>>>(p);
+  count_launch();
+}
+
+}  // namespace spiir
