@@ -209,6 +209,15 @@ int64_t spiir_bank_updates_per_chunk(const spiir_bank* bank, int32_t n_samples);
 /* Kernels launched by this library on this thread so far (bench bookkeeping). */
 int64_t spiir_launch_count(void);
 
+/* Profiling aid for bench.py (off by default; the hot path records no events when
+ * off): when enabled, every spiir_filter_chunk records CUDA events on the caller's
+ * stream at its begin and end and around its recursion-kernel launches (k_bank).
+ * spiir_bank_timing_read synchronises those events, returns the summed durations
+ * (ms) of the recursion brackets and of the whole calls and the number of calls
+ * recorded since the last read, and clears the record. */
+int spiir_bank_timing_enable(spiir_bank* bank, int32_t enable);
+int spiir_bank_timing_read(spiir_bank* bank, double* ms_recursion, double* ms_chunk, int32_t* n_chunks);
+
 /* Measurement helper: runs a dependency-free FP32 FMA loop on every SM and
  * returns the duration of `reps` launches in *ms_out and the FMA-lane-operations
  * performed per launch in *fma_per_launch (peak = 2*fma/time flop/s). */

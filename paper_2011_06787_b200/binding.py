@@ -77,6 +77,9 @@ _SIGNATURES = {
     "spiir_bank_band_plan": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(spiir_band_plan)]),
     "spiir_bank_updates_per_chunk": (C.c_int64, [C.c_void_p, C.c_int32]),
     "spiir_launch_count": (C.c_int64, []),
+    "spiir_bank_timing_enable": (C.c_int, [C.c_void_p, C.c_int32]),
+    "spiir_bank_timing_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                         C.POINTER(C.c_int32)]),
     "spiir_fp32_peak_probe": (C.c_int, [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
     "spiir_last_error": (C.c_char_p, []),
 }
@@ -215,6 +218,15 @@ class Bank:
         p = spiir_band_plan()
         _check(lib().spiir_bank_band_plan(self.h, band, C.byref(p)))
         return {f[0]: getattr(p, f[0]) for f in spiir_band_plan._fields_}
+
+    def timing_enable(self, on=True):
+        _check(lib().spiir_bank_timing_enable(self.h, 1 if on else 0))
+
+    def timing_read(self):
+        """(ms in the recursion kernels, ms in whole filter_chunk calls, number of calls) since the last read."""
+        a, c, n = C.c_double(0), C.c_double(0), C.c_int32(0)
+        _check(lib().spiir_bank_timing_read(self.h, C.byref(a), C.byref(c), C.byref(n)))
+        return a.value, c.value, n.value
 
     def updates_per_chunk(self, n_samples):
         return int(lib().spiir_bank_updates_per_chunk(self.h, n_samples))

@@ -113,17 +113,13 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
     const int G = hb.G, F = hb.F, cap_unit = G * F, upw = 32 / G;
     hb.Hcap = std::max(32, round_up(d->max_delay[b], 4));
     const int nsubmax = std::min(hb.nmax, kSubChunkMax);
-    // shared history depth: covers >= 98 % of the filters, bounded by the smem budget
+    // shared history depth: the deepest template that still fits the shared-memory budget;
+    // templates beyond it (chirp-matched ones) read their input from L1/L2
     {
-      std::vector<std::pair<int, int>> v;
-      for (int t = 0; t < T; ++t) if (cnt[t]) v.push_back({maxd[t], cnt[t]});
-      std::sort(v.begin(), v.end());
-      int64_t acc = 0; int h98 = 0;
-      for (auto& e : v) { acc += e.second; h98 = e.first; if (acc * 100 >= hb.n_filters * 98) break; }
-      const int budget = kSmemFloatsMax - nsubmax;
-      int Hs = round_up(std::max(h98, 1), 64);
-      if (hb.Hcap <= budget && hb.Hcap <= Hs + Hs / 4) Hs = hb.Hcap;
-      hb.Hs = std::min(std::min(Hs, budget / 4 * 4), hb.Hcap);
+      const int budget = (kSmemFloatsMax - nsubmax) / 4 * 4;
+      int h = 0;
+      for (int t = 0; t < T; ++t) if (cnt[t] && maxd[t] <= budget) h = std::max(h, maxd[t]);
+      hb.Hs = std::min(std::max(round_up(h, 4), 4), hb.Hcap);
     }
     hb.cap = round_up(hb.Hcap + hb.nmax + 4, 32);
     hb.reps = hb.Hs + nsubmax;
@@ -320,8 +316,31 @@ int spiir_bank_reset(spiir_bank* bk, void* stream) {
   return SPIIR_OK;
 }
 
+int spiir_bank_timing_enable(spiir_bank* bk, int32_t enable) {
+  SPIIR_REQUIRE(bk != nullptr, "bank is NULL");
+  bk->timing = enable != 0;
+  bk->ev_used = 0;
+  return SPIIR_OK;
+}
+
+int spiir_bank_timing_read(spiir_bank* bk, double* ms_recursion, double* ms_chunk, int32_t* n_chunks) {
+  SPIIR_REQUIRE(bk && ms_recursion && ms_chunk && n_chunks, "a pointer is NULL");
+  double a = 0, c = 0;
+  for (size_t i = 0; i + 3 < bk->ev_used; i += 4) {
+    float m1 = 0.f, m2 = 0.f;
+    SPIIR_CUDA_OK(cudaEventSynchronize(bk->ev_pool[i + 3]));
+    SPIIR_CUDA_OK(cudaEventElapsedTime(&m1, bk->ev_pool[i + 1], bk->ev_pool[i + 2]));
+    SPIIR_CUDA_OK(cudaEventElapsedTime(&m2, bk->ev_pool[i], bk->ev_pool[i + 3]));
+    a += m1; c += m2;
+  }
+  *ms_recursion = a; *ms_chunk = c; *n_chunks = (int32_t)(bk->ev_used / 4);
+  bk->ev_used = 0;
+  return SPIIR_OK;
+}
+
 int spiir_bank_free(spiir_bank* bk) {
   SPIIR_REQUIRE(bk != nullptr, "bank is NULL");
+  for (cudaEvent_t e : bk->ev_pool) cudaEventDestroy(e);
   delete bk;
   return SPIIR_OK;
 }
@@ -364,13 +383,26 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     bd.n = n; bd.nmax = hb.nmax; bd.Hcap = hb.Hcap; bd.Hs = hb.Hs; bd.cap = hb.cap; bd.reps = hb.reps;
     bd.nsub = std::min(n, std::min(hb.nmax, kSubChunkMax));
   }
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  if (bk->timing) {
+    while (bk->ev_pool.size() < bk->ev_used + 4) {
+      cudaEvent_t e;
+      SPIIR_CUDA_OK(cudaEventCreate(&e));
+      bk->ev_pool.push_back(e);
+    }
+    for (int i = 0; i < 4; ++i) ev[i] = bk->ev_pool[bk->ev_used + i];
+    bk->ev_used += 4;
+    SPIIR_CUDA_OK(cudaEventRecord(ev[0], st));
+  }
   launch_prep(pp, D, st);
   SPIIR_CUDA_OK(cudaGetLastError());
+  if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[1], st));
   for (auto& g : bk->groups) {
     int rc = launch_bank_group(g.G, g.F, g.xg, P, (const CtaWork*)(bk->ws + g.off_work), (int)g.work.size(), D,
                                g.xg ? 0 : g.smem_bytes, st);
     if (rc) return rc;
   }
+  if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[2], st));
   CombineParams cp;
   memset(&cp, 0, sizeof(cp));
   for (int b = 0; b < B; ++b) {
@@ -394,6 +426,7 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
   cp.bufB = (B - 1 > d.out_band) ? kUpHist + (d.max_chunk_samples >> (d.out_band + 1)) : 0;
   launch_combine(cp, D, st);
   SPIIR_CUDA_OK(cudaGetLastError());
+  if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[3], st));
 
   bk->parity = newp;
   for (int b = 0; b < B; ++b) bk->band[b].prev_n = n_samples >> b;

@@ -141,4 +141,8 @@ struct spiir_bank {
   int64_t k_next = 0;            // absolute output index of the next chunk's first sample
   int last_n_out = 0;            // output samples of the last chunk
   int64_t last_k0 = 0;
+  // optional profiling (spiir_bank_timing_*): 4 events per chunk: call begin, k_bank begin/end, call end
+  bool timing = false;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
 };

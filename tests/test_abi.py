@@ -1,0 +1,112 @@
+"""CPU-only checks of the C-ABI library: it builds, loads, exports every symbol that
+include/spiir.h declares, and rejects bad arguments before touching a device.
+(No compute calls here; parity lives in the -m gpu tests.)"""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import workloads
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def sp():
+    from paper_2011_06787_b200 import build
+    build.build()
+    import paper_2011_06787_b200 as sp
+    sp.lib()
+    return sp
+
+
+def _declared():
+    txt = open(os.path.join(ROOT, "include", "spiir.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    names = re.findall(r"\b([a-z][a-z0-9_]*)\s*\(", txt)
+    return sorted({n for n in names if n.startswith("spiir_") or n in ("coherent_sky_search", "timeslide_background")})
+
+
+def test_every_declared_symbol_is_exported(sp):
+    L = C.CDLL(sp.LIB_PATH)
+    decl = _declared()
+    assert {"spiir_bank_init", "spiir_filter_chunk", "spiir_peaks", "coherent_sky_search",
+            "timeslide_background"} <= set(decl)
+    for n in decl:
+        assert hasattr(L, n), n
+    assert sorted(sp.EXPORTS) == decl                      # the binding names the same set
+
+
+def test_struct_sizes_match_the_header(sp):
+    assert C.sizeof(sp.spiir_snr_view) == 40
+    assert C.sizeof(sp.spiir_bank_desc) == 16 + 32 + 32 + 8 + 7 * 8 + 8 + 8
+    assert sp.TRIGGER_DTYPE.itemsize == 40 and sp.RESULT_DTYPE.itemsize == 16
+
+
+def test_workspace_query_and_bad_arguments(sp):
+    bank = workloads.bank_for_config(0)
+    d, keep = sp.make_desc(bank, 2, 2048, 2048)
+    n = C.c_size_t(0)
+    assert sp.spiir_bank_workspace_bytes(C.byref(d), C.byref(n)) == sp.SPIIR_OK and n.value > 0
+    # each of these must be refused with EINVAL and a message
+    def bad(mut):
+        d2, k2 = sp.make_desc(bank, 2, 2048, 2048)
+        mut(d2)
+        rc = sp.spiir_bank_workspace_bytes(C.byref(d2), C.byref(n))
+        assert rc == sp.SPIIR_EINVAL and sp.last_error()
+    bad(lambda d: setattr(d, "n_det", 0))
+    bad(lambda d: setattr(d, "n_det", 5))
+    bad(lambda d: setattr(d, "n_bands", 9))
+    bad(lambda d: setattr(d, "out_band", 1))               # single band: out_band must be 0
+    bad(lambda d: setattr(d, "max_chunk_samples", 2050))   # not a multiple of 4
+    bad(lambda d: setattr(d, "ring_len", 100))             # shorter than one chunk
+    bad(lambda d: setattr(d, "host_a", None))
+    bad(lambda d: setattr(d, "bank_size", 0))
+    def small_delay(d):
+        d.max_delay[0] = 5                                  # filters with larger delays exist
+    bad(small_delay)
+    assert sp.spiir_bank_workspace_bytes(None, C.byref(n)) == sp.SPIIR_EINVAL
+    # band rates must halve
+    bank8 = workloads.random_bank(np.random.default_rng(0), 2, 16, [4096, 2048, 1000], out_band=1)
+    dec, itp = workloads.halfband_taps()
+    d3, k3 = sp.make_desc(bank8, 2, 4096, 2048, dec_taps=dec, int_taps=itp)
+    assert sp.spiir_bank_workspace_bytes(C.byref(d3), C.byref(n)) == sp.SPIIR_EINVAL
+
+
+def test_null_handles_are_refused(sp):
+    assert sp.spiir_bank_reset(None, None) == sp.SPIIR_EINVAL
+    assert sp.spiir_bank_free(None) == sp.SPIIR_EINVAL
+    assert sp.spiir_filter_chunk(None, None, 2048, None, None) == sp.SPIIR_EINVAL
+    assert sp.spiir_peaks(None, C.c_float(4.0), 0, None, None, None) == sp.SPIIR_EINVAL
+    assert sp.coherent_sky_search(None, None, None, 1, None, None, None) == sp.SPIIR_EINVAL
+    assert sp.timeslide_background(None, None, None, 1, 1, 2048, None, None, None) == sp.SPIIR_EINVAL
+    n = C.c_size_t(0)
+    assert sp.spiir_sky_plan_workspace_bytes(1, 192, 8, C.byref(n)) == sp.SPIIR_EINVAL
+    assert sp.spiir_sky_plan_workspace_bytes(3, 3072, 1536, C.byref(n)) == sp.SPIIR_OK and n.value > 3072 * 32
+
+
+def test_host_table_builder_matches_the_oracle_table(sp):
+    """spiir_sky_table_build (own closed-form SVD) vs oracle/sky.py (numpy SVD): delays
+    exactly, projectors U2 U2^T to float32 rounding (A20: only the projector is unique)."""
+    import oracle
+    for dets, sigma, nside in ((["H1", "L1", "V1"], [1.0, 1.0, 0.5], 16), (["H1", "L1"], [1.0, 1.0], 4),
+                               (["H1", "L1", "V1"], [1.0, 1.0, 0.5], 1)):
+        pos, resp = workloads.detector_geometry(dets)
+        u2, dl = sp.sky_table_build(nside, pos, resp, sigma, 1.2345, 2048.0)
+        U2o, dlo = oracle.sky_table(nside, pos, resp, sigma, 1.2345, 2048.0)
+        assert np.array_equal(dl, dlo)
+        P = np.einsum("pik,pjk->pij", u2.astype(float), u2.astype(float))
+        Po = np.einsum("pik,pjk->pij", U2o, U2o)
+        assert np.abs(P - Po).max() < 1e-6
+
+
+def test_product_package_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2011_06787_b200")
+    for dp, _, fs in os.walk(pkg):
+        for f in fs:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                txt = open(os.path.join(dp, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "libspiir_oracle" not in txt and "spiir_oracle" not in txt, f

@@ -1,0 +1,309 @@
+"""-m gpu parity tests: the CUDA path, called through the C ABI, against the float64
+oracle on the same seeded inputs (tolerances in tests/parity_util.py)."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sp():
+    import paper_2011_06787_b200 as sp
+    sp.lib()                                    # fails loudly if the CUDA library is missing
+    return sp
+
+
+@pytest.fixture(scope="module")
+def U():
+    import parity_util
+    return parity_util
+
+
+def _table(cfg, nside=None, gmst=None):
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    g = workloads.strain_for_config(cfg["index"], seconds=1)["gmst"] if gmst is None else gmst
+    U2, delay = oracle.sky_table(nside or cfg["nside"], pos, resp, cfg["sigma"], g, 2048.0)
+    return U2.astype(np.float32), delay
+
+
+# ------------------------------------------------------------------ config 0, whole path
+def test_cfg0_whole_path(sp, U):
+    import torch
+    cfg = workloads.config(0)
+    bank = workloads.bank_for_config(0)
+    st = workloads.strain_for_config(0)
+    x = st["strain"]
+    z_ref = oracle.filter_bank(x, bank)
+    z, trigs, bk = U.run_bank(bank, x, 2048, peak_thr=0.0)
+    U.check_snr(z, z_ref)
+    trig, cnt = trigs[0]
+    assert cnt == 8
+    U.check_peaks_mode0(trig, z, z_ref, 0, 0.0)
+    # sky search on the bank's own ring, stage-isolated against the oracle on the same float32 z
+    u2, delay = _table(cfg, gmst=st["gmst"])
+    plan = sp.SkyPlan(u2, delay, max_slots=8)
+    tr_dev, _ = bk.peaks(0.0, 0)
+    smap = torch.empty(8, plan.n_pix, dtype=torch.float32, device="cuda")
+    res = sp.results_to_numpy(plan.search(bk.snr_view(), tr_dev, 8, skymap=smap))
+    torch.cuda.synchronize()
+    ref = U.oracle_sky_on(z, 2048, 2047, u2, delay, trig, want_map=True)
+    U.check_sky(res, z, 2048, 2047, u2, delay, trig, ref=ref)
+    # peaks within 21 samples of the chunk edge must come back as "no result"
+    edge = (trig["k"] < 21) | (trig["k"] > 2047 - 21)
+    assert np.all((res["pix"] == -1) == (ref[1][:, 0] == -1))
+    assert np.all(res["pix"][~edge] >= 0)
+    # two detectors: coh2 == tot2, null2 == 0 at every pixel (P11) -> the map is flat per delay ring
+    ok = res["pix"] >= 0
+    np.testing.assert_allclose(res["coh2"][ok], res["tot2"][ok], rtol=1e-5)
+    m = smap.cpu().numpy()
+    assert np.abs(m - ref[2]).max() <= 1e-4 * max(1.0, np.abs(ref[2]).max())
+
+
+# ------------------------------------------------------------------ single-rate bank, chunk invariance
+def test_single_rate_bank_ragged_and_split_invariant(sp, U):
+    """A bank whose templates have ragged filter counts (incl. an empty template and one larger than
+    a unit), several chunk splits: all must match the one-shot oracle (P7)."""
+    rng = np.random.default_rng(11)
+    counts = [32, 1, 0, 300, 77, 129, 8, 64, 700]
+    banks = [workloads.random_bank(rng, 1, max(c, 1), [2048]) for c in counts]
+    off = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    bank = dict(n_templates=len(counts), band_rates=[2048], out_band=0, tmpl_offset=off,
+                a=np.concatenate([b["a"][:c] for b, c in zip(banks, counts)]),
+                b=np.concatenate([b["b"][:c] for b, c in zip(banks, counts)]),
+                delay=np.concatenate([b["delay"][:c] for b, c in zip(banks, counts)]),
+                band=np.zeros(sum(counts), np.uint8), max_delay=[2047])
+    x = workloads.gaussian_strain(rng, 2, 3 * 2048)
+    z_ref = oracle.filter_bank(x, bank)
+    assert np.all(z_ref[:, 2] == 0)
+    z1, _, _ = U.run_bank(bank, x, 2048)
+    U.check_snr(z1, z_ref)
+    z2, _, _ = U.run_bank(bank, x, None, chunks=[4, 2044, 1024, 8, 3064])
+    U.check_snr(z2, z_ref)
+    z3, _, _ = U.run_bank(bank, x, 6144)
+    U.check_snr(z3, z_ref)
+    assert np.abs(z1 - z2).max() <= 1e-4 and np.abs(z1 - z3).max() <= 1e-4
+
+
+def test_long_delay_template_and_reset(sp, U):
+    """Chirp-matched template (delays up to ~24 000 samples, served beyond the shared window) next
+    to random templates; reset restores the initial state."""
+    import torch
+    bank = workloads.bank_for_config(1, n_templates=24)
+    assert bank["max_delay"][0] > 20000
+    x = workloads.strain_for_config(1)["strain"][:, :15 * 2048]
+    z_ref = oracle.filter_bank(x, bank)
+    z, trigs, bk = U.run_bank(bank, x, 2048, peak_thr=4.0)
+    U.check_snr(z, z_ref)
+    assert np.abs(z_ref[:, 0]).max() > 6.0                 # the injection is seen by template 0
+    n_near = 0
+    for c, (trig, cnt) in enumerate(trigs):
+        sl = slice(c * 2048, (c + 1) * 2048)
+        n_near += U.check_peaks_mode0(trig, z[:, :, sl], z_ref[:, :, sl], c * 2048, 4.0)
+        assert cnt == int(trig["valid"].sum())
+    bk.reset()
+    xs = torch.from_numpy(x[:, :2048].copy()).cuda()
+    out = torch.empty(3, 24, 2048, 2, dtype=torch.float32, device="cuda")
+    bk.filter_chunk(xs, out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy().view(np.complex64)[..., 0], z[:, :, :2048])
+
+
+# ------------------------------------------------------------------ multirate
+def test_multirate_streaming_matches_one_shot_oracle(sp, U):
+    rng = np.random.default_rng(5)
+    bank = workloads.random_bank(rng, 6, 83, workloads.configs.RATES8, out_band=1)
+    dec, itp = workloads.halfband_taps()
+    x = workloads.gaussian_strain(rng, 2, 5 * 4096)
+    z_ref = oracle.filter_bank(x, bank, dec, itp)
+    z, trigs, _ = U.run_bank(bank, x, 4096, taps=(dec, itp), peak_thr=4.0)
+    U.check_snr(z, z_ref)
+    for c, (trig, cnt) in enumerate(trigs):
+        sl = slice(c * 2048, (c + 1) * 2048)
+        U.check_peaks_mode0(trig, z[:, :, sl], z_ref[:, :, sl], c * 2048, 4.0)
+    z2, _, _ = U.run_bank(bank, x, None, taps=(dec, itp), chunks=[512, 4096, 1024, 3584, 4096, 4096, 3072])
+    U.check_snr(z2, z_ref)
+    # three bands with the output at the top rate (out_band = 0)
+    bank3 = workloads.random_bank(rng, 3, 40, [2048, 1024, 512], out_band=0)
+    x3 = workloads.gaussian_strain(rng, 1, 2 * 2048)
+    z3_ref = oracle.filter_bank(x3, bank3, dec, itp)
+    z3, _, _ = U.run_bank(bank3, x3, 2048, taps=(dec, itp))
+    U.check_snr(z3, z3_ref)
+
+
+def test_cfg2_shape_sample(sp, U):
+    """Config 2's layout (8 bands, 600 filters per template) on a template subset, 3 chunks."""
+    bank = workloads.bank_for_config(2, n_templates=16)
+    dec, itp = workloads.halfband_taps()
+    x = workloads.strain_for_config(2, seconds=3)["strain"]
+    z_ref = oracle.filter_bank(x, bank, dec, itp)
+    z, _, bk = U.run_bank(bank, x, 4096, taps=(dec, itp))
+    U.check_snr(z, z_ref)
+    assert bk.updates_per_chunk(4096) == 2 * 16 * 75 * 8160
+
+
+# ------------------------------------------------------------------ peaks mode 1
+def test_peaks_mode1_paper_rule(sp, U):
+    rng = np.random.default_rng(8)
+    bank = workloads.random_bank(rng, 37, 16, [2048])
+    x = workloads.gaussian_strain(rng, 2, 2048)
+    for bank_size, thr in ((10, 2.5), (37, 0.0), (1, 3.0)):
+        z, trigs, _ = U.run_bank(bank, x, 2048, bank_size=bank_size, peak_thr=thr, peak_mode=1)
+        trig, cnt = trigs[0]
+        for d in range(2):
+            k, v = oracle.peaks_mode1(z[d], thr, bank_size)
+            t = trig[d * 37:(d + 1) * 37]
+            assert np.array_equal(t["valid"], v)
+            assert np.array_equal(t["k"][v == 1], k[v == 1])
+            zz = z[d][np.arange(37), k]
+            assert np.array_equal(t["z_re"][v == 1], zz.real[v == 1])
+        assert cnt == int(trig["valid"].sum())
+
+
+# ------------------------------------------------------------------ sky search on snippets (config 3 form)
+def _snippet_case(sp, n_rows, nside, n_windows, half, seed, gmst=0.7):
+    import torch
+    cfg = workloads.config(3)
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    U2, delay = oracle.sky_table(nside, pos, resp, cfg["sigma"], gmst, 2048.0)
+    u2 = U2.astype(np.float32)
+    rng = np.random.default_rng(seed)
+    z, tdet, k, truth = workloads.snr_snippets(rng, u2, delay, n_rows, n_windows, half, 0.25)
+    zc = np.ascontiguousarray(z).view(np.complex64)[..., 0]
+    trig = np.zeros(n_rows, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1
+    trig["tmpl"] = np.arange(n_rows)
+    trig["det"] = tdet
+    trig["k"] = k
+    zd = torch.from_numpy(np.ascontiguousarray(z)).cuda()
+    return u2, delay, zc, zd, trig, truth
+
+
+def test_sky_foreground_and_signal_recovery(sp, U):
+    import torch
+    u2, delay, zc, zd, trig, truth = _snippet_case(sp, 200, 16, 1, 102, seed=21)
+    trig["valid"][::7] = 0                                   # some empty slots
+    L = zc.shape[2]
+    plan = sp.SkyPlan(u2, delay, max_slots=200)
+    assert plan.n_tuples < plan.n_pix
+    view = sp.SnrView(zd)
+    smap = torch.empty(200, plan.n_pix, dtype=torch.float32, device="cuda")
+    res = sp.results_to_numpy(plan.search(view, sp.triggers_from_numpy(trig), 200, skymap=smap))
+    torch.cuda.synchronize()
+    ref = U.oracle_sky_on(zc, L, L - 1, u2, delay, trig, want_map=True)
+    U.check_sky(res, zc, L, L - 1, u2, delay, trig, ref=ref)
+    assert np.all(res["pix"][::7] == -1)
+    m = smap.cpu().numpy()
+    tot = np.maximum(ref[0][:, 0, 2], 1.0)[:, None]
+    assert np.all(np.abs(m - ref[2]) <= 1e-4 * ref[2] + 2e-6 * tot)
+    # injected coherent signals: strong ones come back within the oracle's own arg-max set
+    sig = truth["is_signal"] & (trig["valid"] == 1)
+    assert sig.sum() > 10
+    assert np.mean(res["coh2"][sig]) > 4 * np.mean(res["coh2"][~truth["is_signal"] & (trig["valid"] == 1)])
+
+
+def test_sky_time_slides(sp, U):
+    import torch
+    n_rows, S, half = 96, 7, 102
+    W = 2 * half + 1
+    u2, delay, zc, zd, trig, truth = _snippet_case(sp, n_rows, 16, S + 1, half, seed=22)
+    L = zc.shape[2]
+    plan = sp.SkyPlan(u2, delay, max_slots=n_rows)
+    view = sp.SnrView(zd)
+    td = sp.triggers_from_numpy(trig)
+    for mult in ([1, 1, 1], [0, 0, 0]):
+        res = sp.results_to_numpy(plan.background(view, td, n_rows, S, W, mult))
+        torch.cuda.synchronize()
+        U.check_sky(res, zc, L, L - 1, u2, delay, trig, n_slides=S, step=W, mult=mult)
+    # P16: with every multiplier 0 each slide reproduces the foreground
+    fg = sp.results_to_numpy(plan.search(view, td, n_rows))
+    bg0 = sp.results_to_numpy(plan.background(view, td, n_rows, S, W, [0, 0, 0])).reshape(n_rows, S)
+    for s in range(S):
+        assert np.array_equal(bg0[:, s], fg)
+    # one slide too many leaves the view: "no result" for that slide only
+    res = sp.results_to_numpy(plan.background(view, td, n_rows, S + 1, W, [1, 1, 1])).reshape(n_rows, S + 1)
+    assert np.all(res["pix"][:, S] == -1) and np.all(res["pix"][:, :S] >= 0)
+    # a coarser background table (768 pixels) is just another plan
+    cfg = workloads.config(3)
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    U2b, delayb = oracle.sky_table(8, pos, resp, cfg["sigma"], 0.7, 2048.0)
+    planb = sp.SkyPlan(U2b.astype(np.float32), delayb, max_slots=n_rows)
+    resb = sp.results_to_numpy(planb.background(view, td, n_rows, S, W, [1, 1, 1]))
+    torch.cuda.synchronize()
+    U.check_sky(resb, zc, L, L - 1, U2b.astype(np.float32), delayb, trig, n_slides=S, step=W, mult=[1, 1, 1])
+
+
+def test_sky_ring_wraparound_and_two_detectors(sp, U):
+    """A view used as a true ring (k_newest beyond ring_len, windows wrapping the end) and a
+    two-detector network (projector = identity, P11)."""
+    import torch
+    cfg = workloads.config(0)
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    U2, delay = oracle.sky_table(8, pos, resp, cfg["sigma"], 2.1, 2048.0)
+    u2 = U2.astype(np.float32)
+    rng = np.random.default_rng(3)
+    L, rows = 500, 40
+    z = rng.standard_normal((2, rows, L, 2)).astype(np.float32)
+    zc = z.view(np.complex64)[..., 0]
+    k_newest = 3 * L + 123
+    trig = np.zeros(rows, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1
+    trig["tmpl"] = np.arange(rows)
+    trig["det"] = rng.integers(0, 2, rows)
+    trig["k"] = rng.integers(k_newest - L - 10, k_newest + 5, rows)      # some too old, some too new
+    plan = sp.SkyPlan(u2, delay, max_slots=rows)
+    view = sp.SnrView(torch.from_numpy(z).cuda(), k_newest=k_newest)
+    res = sp.results_to_numpy(plan.search(view, sp.triggers_from_numpy(trig), rows))
+    torch.cuda.synchronize()
+    U.check_sky(res, zc, L, k_newest, u2, delay, trig)
+    ok = res["pix"] >= 0
+    assert ok.sum() > 10 and (~ok).sum() > 0
+    np.testing.assert_allclose(res["coh2"][ok], res["tot2"][ok], rtol=1e-5)
+    assert np.all(res["null2"][ok] <= 1e-4 * res["tot2"][ok] + 1e-5)
+
+
+# ------------------------------------------------------------------ config 1 sample: bank -> peaks -> sky, one-chunk lag
+def test_cfg1_sample_chain(sp, U):
+    import torch
+    cfg = workloads.config(1)
+    T = 48
+    bank = workloads.bank_for_config(1, n_templates=T)
+    st = workloads.strain_for_config(1)
+    x = st["strain"]
+    NC = x.shape[1] // 2048
+    z_ref = oracle.filter_bank(x, bank)
+    u2, delay = _table(cfg, gmst=st["gmst"])
+    ring = 3 * 2048
+    bk = sp.Bank(bank, 3, 2048, ring_len=ring)
+    plan = sp.SkyPlan(u2, delay, max_slots=3 * T)
+    xs = torch.from_numpy(x).cuda()
+    z = np.zeros((3, T, NC * 2048), np.complex64)
+    prev = None
+    best = (0.0, None)
+    for c in range(NC):
+        out = torch.empty(3, T, 2048, 2, dtype=torch.float32, device="cuda")
+        bk.filter_chunk(xs[:, c * 2048:(c + 1) * 2048].contiguous(), out)
+        z[:, :, c * 2048:(c + 1) * 2048] = out.cpu().numpy().view(np.complex64)[..., 0]
+        if prev is not None:                                  # search chunk c-1 now that chunk c exists (A13)
+            res = sp.results_to_numpy(plan.search(bk.snr_view(), prev[0], 3 * T))
+            torch.cuda.synchronize()
+            k_newest = (c + 1) * 2048 - 1
+            lo = k_newest - ring + 1
+            zr = np.zeros((3, T, ring), np.complex64)
+            kk = np.arange(max(lo, 0), k_newest + 1)
+            zr[:, :, kk % ring] = z[:, :, kk]
+            U.check_sky(res, zr, ring, k_newest, u2, delay, prev[1])
+            ok = res["pix"] >= 0
+            if ok.any() and res["coh2"][ok].max() > best[0]:
+                i = np.nonzero(ok)[0][np.argmax(res["coh2"][ok])]
+                best = (float(res["coh2"][i]), (int(prev[1]["tmpl"][i]), int(res["pix"][i])))
+        tr, cnt = bk.peaks(4.0, 0)
+        torch.cuda.synchronize()
+        prev = (tr.clone(), sp.triggers_to_numpy(tr).copy())
+    U.check_snr(z, z_ref)
+    # the injection (network SNR 15) is the loudest coherent candidate, found by template 0
+    assert best[1][0] == 0 and math.sqrt(best[0]) > 10.0
