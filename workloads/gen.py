@@ -8,11 +8,16 @@ t_d), PAPER.md:162 (SNR threshold 4), PAPER.md:489/:495 (unit variance per
 quadrature, hence E|z|^2 = 2 — SURVEY.md §8(c) A8), BASELINE.json configs.
 """
 import math
+import os
+from concurrent.futures import ThreadPoolExecutor
+
 import numpy as np
+from scipy.signal import lfilter
 
 from .configs import config, streams
 
 C_LIGHT = 299792458.0
+_N_THREADS = max(1, min(32, len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)))
 
 # --------------------------------------------------------------------------
 # FIR taps for the multirate layout (BASELINE.json config 2: "32-tap Kaiser
@@ -107,7 +112,7 @@ def _split_over_bands(L, B):
     return base
 
 
-def _noise_variance(a, b, d, block_bytes=96 << 20):
+def _noise_variance(a, b, d, block_bytes=24 << 20):
     """Closed-form E|z|^2 of sum_l y_l in unit white noise, per template.
 
     a, b: complex128 [T, n]; d: int [T, n].  V = sum_{l,m} b_l conj(b_m) K_lm,
@@ -121,13 +126,24 @@ def _noise_variance(a, b, d, block_bytes=96 << 20):
         return out
     step = max(1, int(block_bytes // (n * n * 16 * 4)))
     la = np.log(a)
-    for s in range(0, T, step):
+
+    def block(s):
         e = min(T, s + step)
         dd = (d[s:e, None, :] - d[s:e, :, None]).astype(np.float64)       # d_m - d_l  [T,l,m]
         pos = dd >= 0
         ex = np.where(pos, la[s:e, :, None] * dd, np.conj(la[s:e, None, :]) * (-dd))
         K = np.exp(ex) / (1.0 - a[s:e, :, None] * np.conj(a[s:e, None, :]))
         out[s:e] = np.real(np.einsum("tl,tm,tlm->t", b[s:e], np.conj(b[s:e]), K))
+
+    # blocks are independent and their size does not depend on the thread count, so the
+    # result is the same however many threads run them (numpy releases the GIL)
+    starts = list(range(0, T, step))
+    if len(starts) > 1 and _N_THREADS > 1:
+        with ThreadPoolExecutor(_N_THREADS) as ex_:
+            list(ex_.map(block, starts))
+    else:
+        for s in starts:
+            block(s)
     return out
 
 
@@ -224,16 +240,28 @@ def chirp_matched_template(f0, tc, fs, n_filters, f_cut=1000.0):
     d = np.array([K - int(round(x[0] * fs)) for x in nd], dtype=np.int32)
     a32 = np.exp(-1.0 / tau + 1j * om).astype(np.complex64)
     a = a32.astype(np.complex128)
-    N = K + 1 + int(6 * tau.max())
-    n = np.arange(N)[:, None]
-    rel = n - d[None, :]
-    basis = np.where(rel >= 0, np.exp(np.log(a)[None, :] * np.maximum(rel, 0)), 0.0)
-    tgt = np.zeros(N, complex)
-    tgt[:K + 1] = target
-    b, *_ = np.linalg.lstsq(basis, tgt, rcond=None)
-    u = basis @ b
-    ov = abs(np.vdot(u, tgt)) / math.sqrt(np.vdot(u, u).real * np.vdot(tgt, tgt).real)
-    V = np.vdot(u, u).real                                   # E|z|^2 in unit white noise = sum |h|^2
+    # Linear least squares for b against tgt[n] = target[n] (n <= K), through the normal
+    # equations G b = r of the basis h_l[n] = a_l^(n-d_l) [n >= d_l], both in closed form:
+    #   G_lm = sum_n conj(h_l[n]) h_m[n] = conj(a_l)^(d_m-d_l) / (1 - conj(a_l) a_m)   (d_m >= d_l)
+    #                                    = a_m^(d_l-d_m)       / (1 - conj(a_l) a_m)   (d_m <  d_l)
+    #   r_l  = sum_{n >= d_l} conj(a_l)^(n-d_l) target[n]   (a backward one-pole recursion)
+    # The nodes oversample the chirp, so G is numerically singular: a tiny ridge picks the
+    # small-norm solution.
+    la = np.log(a)
+    dd = (d[None, :] - d[:, None]).astype(np.float64)                  # d_m - d_l  [l, m]
+    ex = np.where(dd >= 0, np.conj(la)[:, None] * dd, la[None, :] * (-dd))
+    G = np.exp(ex) / (1.0 - np.conj(a)[:, None] * a[None, :])
+    r = np.zeros(n_filters, complex)
+    rev = target[::-1]
+    for l in range(n_filters):
+        # s[n] = target[n] + conj(a_l) s[n+1], evaluated at n = d_l (lfilter over the reversed series)
+        seg = rev[:K + 1 - d[l]] if d[l] <= K else rev[:0]
+        if len(seg):
+            r[l] = lfilter([1.0], [1.0, -np.conj(a[l])], seg)[-1]
+    ridge = 1e-9 * float(np.mean(np.real(np.diag(G))))
+    b = np.linalg.solve(G + ridge * np.eye(n_filters), r)
+    V = float(np.real(np.vdot(b, G @ b)))                    # E|z|^2 in unit white noise = sum |h|^2
+    ov = abs(np.vdot(b, r)) / math.sqrt(V * float(np.vdot(target, target).real))
     b = b * math.sqrt(2.0 / V)
     return a32, b.astype(np.complex64), d, float(ov)
 
@@ -325,8 +353,8 @@ def bank_for_config(idx, n_templates=None, exact_norm=True):
         params = chirp_params_for_config(c, inj_rng)
         L = c["filters_per_template"]
         band_of_2048 = c["band_rates"].index(2048)
-        for t in range(n_chirp):
-            a, b, d, ov = chirp_matched_template(params[t]["f0"], params[t]["tc"], 2048.0, L)
+        fits = [chirp_matched_template(params[t]["f0"], params[t]["tc"], 2048.0, L) for t in range(n_chirp)]
+        for t, (a, b, d, ov) in enumerate(fits):
             sl = slice(t * L, (t + 1) * L)
             bank["a"][sl], bank["b"][sl], bank["delay"][sl] = a, b, d
             bank["band"][sl] = band_of_2048
