@@ -1,0 +1,523 @@
+"""bench.py — throughput of the SPIIR hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A *step* is one pass of the whole hot path over one 1-second chunk of synthetic strain
+(DESIGN.md §8): spiir_filter_chunk (decimator chain, IIR recursion, band sums, up-sample
+cascade, SNR ring, fused per-template maximum) -> spiir_peaks (threshold 4, mode 0) ->
+coherent_sky_search on the previous chunk's candidates (one-chunk lag, reading A13) ->
+timeslide_background with 100 slides of 1 s.  Workload at N = 1: BASELINE.json config 4
+(H1/L1/V1, 20 000 templates x 700 filters over 8 rate bands, HEALPix nside 32, 100
+slides), synthetic and seeded (workloads/).  N > 1: every rank runs one such template
+shard (weak scaling; the path has no exchange step).
+
+`value` = filter-sample updates/s of the whole job, all stages inside the timed region,
+inputs resident in HBM; `e2e` = the same through the C ABI with pinned HOST strain in and
+HOST candidate / result arrays out.  `--impl reference` times the float64 oracle (oracle/)
+on the host cores on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "spiir_filter_sample_updates_per_s"
+UNIT = "updates/s"
+FLOP_PER_UPDATE = 12.0          # 12 flop per filter-sample (8 FP32 instructions)
+FLOP_PER_EVAL = 11.0            # this kernel: 1 FMUL + 5 FFMA per direction (N_d = 3); the paper counts 4 N_d^2 = 36
+# FP32 ALU roofline: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md
+# unit counts and clocks.max.sm).  The recursion's instruction mix (2 FMUL + 4 FFMA + 2 FADD = 12 flop in
+# 8 issue slots) tops out at 12/16 = 75 % of it.
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+FP32_LANE_OPS_PER_S = 148 * 128 * 1.965e9
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/); None until a capture exists for the kernel.
+NCU_TRAFFIC_BYTES = {"k_bank": None, "k_sky": None}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (2 or 4 stream a bank)")
+    ap.add_argument("--templates", type=int, default=None, help="override the template count (debugging)")
+    ap.add_argument("--slides", type=int, default=None, help="override the number of time slides")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fast-norm", action="store_true",
+                    help="diagonal approximation of the bank's noise normalisation (quicker set-up)")
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.thr = [], None, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            inside = t0 - 0.1 <= ts <= t1 + 0.3
+            try:
+                if inside:
+                    sm.append(float(f[1])); pw.append(float(f[3]))
+                mx.append(float(f[2]))
+            except ValueError:
+                continue
+            if inside:
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"),
+                                     f[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+        if not sm:                                   # timed region shorter than one sample: take all samples
+            for ts, line in self.rows:
+                f = [x.strip() for x in line.split(",")]
+                try:
+                    sm.append(float(f[1]))
+                except (ValueError, IndexError):
+                    pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------- workload
+def workload_params(args):
+    import workloads
+    cfg = workloads.config(args.config)
+    if not cfg["n_templates"]:
+        raise SystemExit("config %d has no filter bank; bench streams configs 1, 2 or 4" % args.config)
+    T = args.templates or cfg["n_templates"]
+    S = cfg["n_slides"] if args.slides is None else args.slides
+    f_in = cfg["band_rates"][0]
+    return dict(cfg=cfg, T=T, S=S, D=len(cfg["dets"]), chunk=f_in, n_out=2048, nside=cfg["nside"],
+                n_pix=12 * cfg["nside"] ** 2, ring_len=(S + 3) * 2048, thr=float(cfg["threshold"]))
+
+
+def updates_per_chunk(bank, D, chunk):
+    """Filter-sample updates of one chunk: every filter advances (chunk >> band) samples, per detector."""
+    band = np.asarray(bank["band"]).astype(np.int64)
+    return int(D * np.sum(chunk >> band))
+
+
+# ----------------------------------------------------------------------------- oracle sample (CPU)
+_SAMPLE_INPUTS = {}
+# Fraction of (detector, template, second) slots above SNR 4 in steady state (SURVEY.md §8 probe: 36 %);
+# used only when the sampled seconds are still in the bank's cold-start transient and show none.
+STEADY_TRIGGER_FRACTION = 0.36
+
+
+def oracle_sample(args, n_templates, n_chunks, n_trig, repeat=1):
+    """Times the float64 oracle (oracle/, as it stands) on a bounded sample of the workload:
+    the first `n_templates` templates over `n_chunks` seconds (O1-O4) and the sky search with
+    all its slides for `n_trig` candidates on packed SNR snippets (O6-O7).  Work is linear in
+    templates and in candidates, so rates extrapolate to the full chunk."""
+    import oracle
+    import workloads
+    w = workload_params(args)
+    cfg, D, S = w["cfg"], w["D"], w["S"]
+    key = (args.config, n_templates, n_chunks)
+    if key not in _SAMPLE_INPUTS:                      # inputs are generated once, outside the timed calls
+        _SAMPLE_INPUTS[key] = (workloads.bank_for_config(args.config, n_templates=n_templates),
+                               workloads.strain_for_config(args.config, seconds=n_chunks)["strain"])
+    bank, x = _SAMPLE_INPUTS[key]
+    dec, itp = workloads.halfband_taps()
+    multirate = len(cfg["band_rates"]) > 1
+    out = dict(threads=oracle.num_threads(), n_templates=n_templates, n_chunks=n_chunks, n_trig=n_trig)
+    t_bank = t_peaks = t_sky = 0.0
+    for _ in range(repeat):
+        t0 = time.perf_counter()
+        z = oracle.filter_bank(x, bank, dec if multirate else None, itp if multirate else None)
+        t1 = time.perf_counter()
+        n_valid = 0
+        for c in range(n_chunks):
+            zc = np.ascontiguousarray(z[:, :, c * 2048:(c + 1) * 2048]).reshape(D * n_templates, 2048)
+            _, v = oracle.peaks_mode0(zc, w["thr"])
+            n_valid += int(v.sum())
+        t2 = time.perf_counter()
+        t_bank += t1 - t0
+        t_peaks += t2 - t1
+    out["updates"] = updates_per_chunk(bank, D, w["chunk"]) * n_chunks * repeat
+    out["t_bank"], out["t_peaks"] = t_bank, t_peaks
+    out["trigger_fraction"] = n_valid / float(D * n_templates * n_chunks)
+    out["evals"], out["t_sky"] = 0, 0.0
+    if w["nside"] and n_trig:
+        pos, resp = workloads.detector_geometry(cfg["dets"])
+        U2, delay = oracle.sky_table(w["nside"], pos, resp, cfg["sigma"], 1.234, 2048.0)
+        u2 = U2.astype(np.float32)
+        half = 102
+        W = 2 * half + 1
+        rng = np.random.default_rng(cfg["seed"])
+        zs, tdet, k, _ = workloads.snr_snippets(rng, u2, delay, n_trig, S + 1, half, 0.1)
+        zc = np.ascontiguousarray(zs).view(np.complex64)[..., 0]
+        L = zc.shape[2]
+        ones, rows = np.ones(n_trig, np.int32), np.arange(n_trig, dtype=np.int32)
+        for _ in range(repeat):
+            t0 = time.perf_counter()
+            oracle.sky_search(u2, delay, zc, n_trig * L, L, L, L - 1, ones, rows, tdet, k)
+            if S:
+                oracle.sky_search(u2, delay, zc, n_trig * L, L, L, L - 1, ones, rows, tdet, k,
+                                  n_slides=S, step=W, slide_mult=[1] * D)
+            t_sky += time.perf_counter() - t0
+        out["evals"] = n_trig * w["n_pix"] * (1 + S) * repeat
+        out["t_sky"] = t_sky
+    return out
+
+
+def oracle_whole_step_rate(s, updates_full, evals_full, slots_full):
+    """Whole-path updates/s of the oracle extrapolated to one full chunk from the sampled stage rates."""
+    t = updates_full / (s["updates"] / s["t_bank"])
+    t += s["t_peaks"] * slots_full / float(max(1, s["n_templates"] * s["n_chunks"]))
+    if s["evals"]:
+        t += evals_full / (s["evals"] / s["t_sky"])
+    return updates_full / t, t
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, K timed steps after W warm-ups; each step
+    is one bounded sample (64 templates x 1 s through O1-O4, 8 candidates through O6-O7)."""
+    import oracle
+    w = workload_params(args)
+    n_t, n_c, n_trig = min(64, w["T"]), 1, (8 if w["nside"] else 0)
+    for _ in range(max(0, args.warmup)):
+        oracle_sample(args, n_t, n_c, n_trig)
+    acc = None
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        s = oracle_sample(args, n_t, n_c, n_trig)
+        if acc is None:
+            acc = dict(s)
+        else:
+            for key in ("updates", "t_bank", "t_peaks", "evals", "t_sky"):
+                acc[key] += s[key]
+    wall = time.perf_counter() - t0
+    import workloads
+    per_t = updates_per_chunk(workloads.bank_for_config(args.config, n_templates=n_t), w["D"], w["chunk"]) / n_t
+    updates_full = per_t * w["T"]
+    slots_full = w["D"] * w["T"]
+    frac = acc["trigger_fraction"] if acc["trigger_fraction"] > 0.05 else STEADY_TRIGGER_FRACTION
+    evals_full = frac * slots_full * w["n_pix"] * (1 + w["S"]) if w["nside"] else 0
+    value, t_chunk = oracle_whole_step_rate(acc, updates_full, evals_full, slots_full)
+    sample = ("per step: first %d templates x %d s through O1-O4 + %d candidates x %d directions x (1+%d slides) "
+              "through O6-O7; whole-chunk rate extrapolated linearly in templates and candidates"
+              % (n_t, n_c, n_trig, w["n_pix"], w["S"]))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(args, w),
+        "bank_updates_per_s": acc["updates"] / acc["t_bank"],
+        "sky_evals_per_s": (acc["evals"] / acc["t_sky"]) if acc["evals"] else None,
+        "extrapolated_s_per_chunk": t_chunk,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def config_dict(args, w):
+    cfg = w["cfg"]
+    return {"workload": "BASELINE.json configs[%d] (%s): %d det, %d templates x %d filters, %d rate bands, "
+                        "1-s chunks of %d samples, peaks mode 0 thr %.1f, HEALPix nside %d, %d time slides of 1 s"
+                        % (args.config, cfg["name"], w["D"], w["T"], cfg["filters_per_template"],
+                           len(cfg["band_rates"]), w["chunk"], w["thr"], w["nside"], w["S"]),
+            "templates_per_gpu": w["T"], "ring_seconds": w["ring_len"] // 2048,
+            "l2": "no flush: per-step working set (coefficients, states, band sums, SNR ring segment) exceeds the 126 MB L2",
+            "parallelism": "template shards, no collective"}
+
+
+# ----------------------------------------------------------------------------- the CUDA arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import workloads
+    import paper_2011_06787_b200 as sp
+    from paper_2011_06787_b200 import shard as shd
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; --impl reference times the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    sp.lib()                                             # fails loudly if libspiir_b200.so is missing
+
+    w = workload_params(args)
+    cfg, T, S, D, chunk = w["cfg"], w["T"], w["S"], w["D"], w["chunk"]
+    multirate = len(cfg["band_rates"]) > 1
+    t_setup = time.time()
+    bank = workloads.bank_for_config(args.config, n_templates=T, exact_norm=not args.fast_norm, shard=rank)
+    st = workloads.strain_for_config(args.config)
+    x = st["strain"]
+    n_chunks = x.shape[1] // chunk
+    dec, itp = workloads.halfband_taps()
+    upd_chunk = updates_per_chunk(bank, D, chunk)
+    n_slots = D * T
+    has_sky = w["nside"] > 0
+
+    bk = sp.Bank(bank, D, chunk, ring_len=w["ring_len"], bank_size=1000,
+                 dec_taps=dec if multirate else None, int_taps=itp if multirate else None)
+    assert bk.updates_per_chunk(chunk) == upd_chunk
+    plan = None
+    if has_sky:
+        pos, resp = workloads.detector_geometry(cfg["dets"])
+        u2, delay = sp.sky_table_build(w["nside"], pos, resp, cfg["sigma"], st["gmst"], 2048.0)
+        plan = sp.SkyPlan(u2, delay, max_slots=n_slots)
+    mult = [1] * D
+    # strain chunks: [n_chunks][D][chunk], resident in HBM and as pinned host memory
+    xc = np.ascontiguousarray(x.reshape(D, n_chunks, chunk).transpose(1, 0, 2))
+    x_host = torch.from_numpy(xc).pin_memory()
+    x_dev = x_host.to(dev)
+    x_in = torch.empty(D, chunk, dtype=torch.float32, device=dev)        # e2e staging buffer
+    trig = [torch.zeros(n_slots, 40, dtype=torch.uint8, device=dev) for _ in range(2)]
+    max_steps = w["ring_len"] // 2048 + 2 * (args.warmup + args.steps) + 8
+    counts = torch.zeros(max_steps, dtype=torch.int32, device=dev)
+    fg_out = torch.zeros(n_slots, 16, dtype=torch.uint8, device=dev)
+    bg_out = torch.zeros(n_slots * max(S, 1), 16, dtype=torch.uint8, device=dev)
+    trig_host = torch.empty(n_slots, 40, dtype=torch.uint8).pin_memory()
+    fg_host = torch.empty(n_slots, 16, dtype=torch.uint8).pin_memory()
+    bg_host = torch.empty(n_slots * max(S, 1), 16, dtype=torch.uint8).pin_memory()
+    cnt_host = torch.empty(1, dtype=torch.int32).pin_memory()
+    state = {"i": 0}
+
+    def step(xin, events=None):
+        """One pass of the hot path over one chunk (every call goes through the C ABI)."""
+        i = state["i"]
+        cur, prev = trig[i & 1], trig[(i & 1) ^ 1]
+        if events is not None: events[0].record()
+        bk.filter_chunk(xin)                                           # H0-H3 (+ fused H4 maximum)
+        if events is not None: events[1].record()
+        bk.peaks(w["thr"], 0, trig=cur, count=counts[i:i + 1])         # H4
+        if events is not None: events[2].record()
+        if has_sky:
+            view = bk.snr_view()
+            plan.search(view, prev, n_slots, out=fg_out)               # H5 on the previous chunk's candidates
+            if events is not None: events[3].record()
+            if S:
+                plan.background(view, prev, n_slots, S, 2048, mult, out=bg_out)   # H6
+        elif events is not None:
+            events[3].record()
+        if events is not None: events[4].record()
+        state["i"] = i + 1
+        return cur
+
+    # ---- fill the SNR ring (set-up, untimed): the slides need S seconds of history
+    n_fill = w["ring_len"] // 2048
+    for c in range(n_fill):
+        bk.filter_chunk(x_dev[c % n_chunks])
+    torch.cuda.synchronize()
+    t_setup = time.time() - t_setup
+    c0 = n_fill
+    for j in range(args.warmup):
+        step(x_dev[(c0 + j) % n_chunks])
+    c0 += args.warmup
+    torch.cuda.synchronize()
+
+    # ---- device-timed region: K steps, inputs resident in HBM
+    K = args.steps
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    bk.timing_enable(True)
+    clocks = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = sp.spiir_launch_count()
+    i_first = state["i"]
+    wall0 = time.time()
+    e_begin, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e_begin.record()
+    for j in range(K):
+        step(x_dev[(c0 + j) % n_chunks], evs[j])
+    e_end.record()
+    torch.cuda.synchronize()
+    wall1 = time.time()
+    if world > 1:
+        dist.barrier()
+    launches = sp.spiir_launch_count() - launches0
+    ms_total = e_begin.elapsed_time(e_end)
+    ms_rec, ms_chunkcall, n_rec = bk.timing_read()
+    bk.timing_enable(False)
+    clk = clocks.stop(wall0, wall1) if clocks else None
+    c0 += K
+    stage = np.zeros(4)
+    for e in evs:
+        for q in range(4):
+            stage[q] += e[q].elapsed_time(e[q + 1])
+    cnt = counts.cpu().numpy()
+    # candidates searched in step j are those found in step j-1
+    n_cand = int(cnt[i_first - 1:i_first - 1 + K].sum()) if has_sky else 0
+    evals = n_cand * w["n_pix"] * (1 + S)
+    # every valid candidate of the last step must have been searched on every slide (ring filled, one-chunk lag)
+    searched = None
+    if has_sky:
+        prev_np = sp.triggers_to_numpy(trig[state["i"] & 1])
+        fg_np = sp.results_to_numpy(fg_out)
+        okf = fg_np["pix"][prev_np["valid"] == 1] >= 0
+        searched = float(okf.mean()) if okf.size else None
+        if S:
+            bg_np = sp.results_to_numpy(bg_out).reshape(n_slots, S)
+            okb = bg_np["pix"][prev_np["valid"] == 1] >= 0
+            searched = min(searched, float(okb.mean())) if okb.size else searched
+
+    # ---- end to end: pinned host strain in, host candidates and results out, every step
+    e2e = None
+    if not args.no_e2e:
+        torch.cuda.synchronize()
+        h2d = D * chunk * 4
+        d2h = n_slots * 40 + 4 + (n_slots * 16 + (n_slots * S * 16 if S else 0) if has_sky else 0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if world > 1:
+            dist.barrier()
+        e0.record()
+        for j in range(K):
+            x_in.copy_(x_host[(c0 + j) % n_chunks], non_blocking=True)
+            cur = step(x_in)
+            trig_host.copy_(cur, non_blocking=True)
+            cnt_host.copy_(counts[state["i"] - 1:state["i"]], non_blocking=True)
+            if has_sky:
+                fg_host.copy_(fg_out, non_blocking=True)
+                if S:
+                    bg_host.copy_(bg_out, non_blocking=True)
+            torch.cuda.current_stream().synchronize()                # the caller reads this step's results
+        e1.record()
+        torch.cuda.synchronize()
+        ms_e2e = shd.max_over_ranks(e0.elapsed_time(e1), dev)
+        e2e = {"value": world * upd_chunk * K / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e / K,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+        c0 += K
+
+    ms_total = shd.max_over_ranks(ms_total, dev)
+    upd_all = shd.sum_over_ranks(upd_chunk * K, dev)
+    evals_all = shd.sum_over_ranks(evals, dev)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (+ the other one), FP32 probe, CPU baseline
+    ffma_rate, _ = sp.fp32_peak_probe(20)
+    ms_sky = stage[2] + stage[3]
+    roof_bank = alu_roofline("k_bank (IIR recursion, H1+H2)", FLOP_PER_UPDATE * upd_chunk * n_rec, ms_rec,
+                             n_rec * len_groups(bk), ffma_rate, NCU_TRAFFIC_BYTES["k_bank"],
+                             issue_ops=8.0 * upd_chunk * n_rec)
+    roof_sky = None
+    if has_sky and evals:
+        roof_sky = alu_roofline("k_sky (coherent search + slides, H5+H6)", FLOP_PER_EVAL * evals, ms_sky,
+                                2 * D * K if S else D * K, ffma_rate, NCU_TRAFFIC_BYTES["k_sky"],
+                                issue_ops=9.0 * evals)
+    dominant, other = (roof_bank, roof_sky) if (roof_sky is None or ms_rec >= ms_sky) else (roof_sky, roof_bank)
+    line = {
+        "metric": METRIC, "value": upd_all / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": args.warmup, "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_dict(args, w),
+        "sky_evals_per_s": evals_all / (ms_total * 1e-3) if has_sky else None,
+        "chunk_latency_ms": ms_total / K,
+        "stages_ms_per_step": {"filter_chunk": stage[0] / K, "of_which_k_bank": ms_rec / max(1, n_rec),
+                               "peaks": stage[1] / K, "sky_foreground": stage[2] / K, "sky_slides": stage[3] / K},
+        "stage_rates": {"bank_updates_per_s": upd_chunk * K / (stage[0] * 1e-3),
+                        "k_bank_updates_per_s": upd_chunk * n_rec / (ms_rec * 1e-3),
+                        "sky_evals_per_s": (evals / (ms_sky * 1e-3)) if (has_sky and ms_sky > 0) else None},
+        "per_step": {"updates": upd_chunk, "candidates": n_cand / K if has_sky else None,
+                     "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
+        "roofline": dominant, "roofline_other": other,
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        s = oracle_sample(args, min(256, T), 2, 16 if has_sky else 0)
+        cpu_v, cpu_t = oracle_whole_step_rate(s, upd_chunk, evals / K if has_sky else 0, n_slots)
+        line["cpu_baseline"] = {
+            "value": cpu_v, "unit": UNIT, "cores": s["threads"], "kind": "oracle",
+            "bank_updates_per_s": s["updates"] / s["t_bank"],
+            "sky_evals_per_s": (s["evals"] / s["t_sky"]) if s["evals"] else None,
+            "extrapolated_s_per_chunk": cpu_t,
+            "sample": "first %d templates x %d s through O1-O4 (%.1f s) and %d candidates x %d directions x (1+%d "
+                      "slides) through O6-O7 (%.1f s); whole-chunk rate extrapolated linearly in templates and "
+                      "candidates" % (s["n_templates"], s["n_chunks"], s["t_bank"], s["n_trig"], w["n_pix"], S,
+                                      s["t_sky"])}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def len_groups(bk):
+    """Recursion-kernel launches per chunk (one per (lanes, filters-per-lane, delay class) group)."""
+    seen = set()
+    for b in range(bk.n_bands):
+        p = bk.band_plan(b)
+        seen.add((p["lanes_per_unit"], p["filters_per_lane"], 0))
+        if p["n_units_long"]:
+            seen.add((p["lanes_per_unit"], p["filters_per_lane"], 1))
+    return len(seen)
+
+
+def alu_roofline(name, flops, ms, n_launches, ffma_rate, traffic, issue_ops):
+    """FP32-ALU roofline entry: achieved = algorithmic flop / device time of the kernel's launches
+    (CUDA events on the launching stream, inside the timed region)."""
+    achieved = flops / (ms * 1e-3) / 1e12
+    return {"kernel": name, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
+            "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (clocks.max.sm); not in "
+                           "MEASURED_PEAKS.json",
+            "fp32_issue_frac": issue_ops / (ms * 1e-3) / FP32_LANE_OPS_PER_S,
+            "measured_ffma_tflops_same_run": 2.0 * ffma_rate / 1e12,
+            "frac_of_measured_ffma": achieved / (2.0 * ffma_rate / 1e12),
+            "ms_per_launch_set": ms / max(1, n_launches), "launches": n_launches}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -204,10 +204,13 @@ class Bank:
         _check(lib().spiir_filter_chunk(self.h, C.c_void_p(strain.data_ptr()), n,
                                         C.c_void_p(snr_out.data_ptr()) if snr_out is not None else None, _stream()))
 
-    def peaks(self, threshold, mode=0):
-        _check(lib().spiir_peaks(self.h, C.c_float(threshold), mode, C.c_void_p(self.trig.data_ptr()),
-                                 C.c_void_p(self.count.data_ptr()), _stream()))
-        return self.trig, self.count
+    def peaks(self, threshold, mode=0, trig=None, count=None):
+        """spiir_peaks into the given device buffers (default: the Bank's own)."""
+        trig = self.trig if trig is None else trig
+        count = self.count if count is None else count
+        _check(lib().spiir_peaks(self.h, C.c_float(threshold), mode, C.c_void_p(trig.data_ptr()),
+                                 C.c_void_p(count.data_ptr()), _stream()))
+        return trig, count
 
     def snr_view(self):
         v = spiir_snr_view()

@@ -339,11 +339,13 @@ def snr_snippets(rng, u2, delay, n_rows, n_windows, half, coherent_fraction,
 # Per-configuration assembly
 # --------------------------------------------------------------------------
 
-def bank_for_config(idx, n_templates=None, exact_norm=True):
+def bank_for_config(idx, n_templates=None, exact_norm=True, shard=0):
     """The filter bank of config ``idx`` (optionally with fewer templates —
-    templates are independent, so a prefix is an exact sub-problem)."""
+    templates are independent, so a prefix is an exact sub-problem).  ``shard`` > 0
+    draws the random templates of another template shard of the same shape (one
+    shard per GPU: independent nodes of 4000 templates each)."""
     c = config(idx)
-    rng = streams(c["seed"])["bank"]
+    rng = streams(c["seed"] + 7919 * int(shard))["bank"]
     T = c["n_templates"] if n_templates is None else n_templates
     bank = random_bank(rng, T, c["filters_per_template"], c["band_rates"], c["out_band"],
                        exact_norm=exact_norm)
