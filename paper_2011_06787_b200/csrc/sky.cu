@@ -8,15 +8,18 @@
 // Design — not the paper's "one thread per direction":
 //   * Eq. 28 writes rho_c^2 as the quadratic form z^H (U I U^T) z.  With
 //     integer delays only ~N_pix/14 distinct delay tuples exist at nside 64, and every
-//     direction of one tuple gathers the SAME samples.  So the plan sorts directions
-//     by tuple and stores the projector M = U2 U2^T; per tuple a thread forms the
-//     N_d(N_d+1)/2 real products q_IJ = Re(z_I conj z_J) once, and each direction then
-//     costs one N_q-term dot product (6 FP32 instructions for three detectors)
-//     plus the running arg-max.
+//     direction of one tuple gathers the SAME samples.  The plan sorts the directions
+//     of each trigger detector T by delay tuple and packs them into a stream of
+//     32-slot chunks: a header slot per tuple (shared-memory rows to gather, number of
+//     directions, which detectors' rows changed since the previous header) followed
+//     by its direction slots (the projector M = U2 U2^T in the order the kernel
+//     consumes it, and the pixel).  Per tuple a thread forms the real products
+//     q_IJ = Re(z_I conj z_J) that changed; each direction then costs one N_q-term dot
+//     product (1 FMUL + 5 FFMA for three detectors) plus the running arg-max.
 //   * thread = K (trigger, slide) pairs; a CTA owns 32 K pairs whose delay windows
 //     (the only samples any direction can touch) sit in shared memory, sample-major
-//     so that the per-tuple gather is conflict free; its warps split the direction
-//     stream and stage their records through shared memory for broadcast reads.
+//     so that the per-tuple gather is conflict free; its warps split the chunk
+//     stream and stage each chunk through shared memory for broadcast reads.
 //   * valid trigger slots are binned by trigger detector on the device (no host sync);
 //     one launch per trigger detector, persistent CTAs stride over the pair batches.
 #include <algorithm>
@@ -28,68 +31,66 @@
 
 namespace spiir {
 
-constexpr int kSkyThreads = 256;
+constexpr int kSkyThreads = 512;
 constexpr int kSkyWarps = kSkyThreads / 32;
-constexpr int kSkyK = 2;                    // pairs per thread
-constexpr int kSkyNP = 32 * kSkyK;          // pairs per CTA
-constexpr int kSkyNPS = kSkyNP + 1;         // padded row stride of the windows (float2)
-constexpr int kSkySmemMax = 200 * 1024;
+constexpr int kSkyChunk = 32;               // slots per stream chunk (one per lane when staging)
+constexpr int kSkyKMax = 4;                 // (trigger, slide) pairs per thread, at most
+constexpr int kSkySmemMax = 227 * 1024;     // opt-in dynamic shared memory per CTA on sm_100
+constexpr int kSkyEnd = 15;                 // header level that ends a chunk
 
-template <int D> struct SkyRec { static constexpr int NQ = D * (D + 1) / 2; static constexpr int RW = (NQ + 3 + 3) / 4 * 4; };
-// record words: [0, NQ) projector entries (diagonal first, then 2*M_IJ for I<J in the
-// order (0,1) (0,2) (1,2) (0,3) (1,3) (2,3)); [NQ] pixel; [NQ+1] d1 | d2 << 16; [NQ+2] d3
-// with d_I = delay[p][I] - delay[p][0].
+template <int D> struct SkyFmt {
+  static constexpr int NO = D - 1;                       // detectors other than the trigger detector
+  static constexpr int NQ = D * (D + 1) / 2;             // independent entries of the projector
+  static constexpr int SW = (NQ + 1 + 3) / 4 * 4;        // words per slot: NQ weights + pixel, padded to 16 B
+};
+// header slot : word 0..2 window row of other detector o (already offset by its window's first row),
+//               word 3 = count | level << 8 (level = first other detector whose row changed; kSkyEnd = end)
+// direction   : words [0,NQ) weights, word NQ = pixel.  Weight order (T = trigger detector, o = others in
+//               increasing detector index): M_TT; M_oo (o = 0..NO-1); 2 M_To; 2 M_o'o for o' < o,
+//               (0,1) (0,2) (1,2).
 
 struct SkyParams {
-  const float* rec; int32_t n_rec; int32_t rec_per_warp;     // stream, multiple-of-32 share per warp
-  const int32_t* pix_delta;                                   // [n_pix][4] d_I of each pixel (word 0 unused)
+  const float* stream; int32_t n_chunks, chunks_per_warp;     // this trigger detector's stream
+  const int4* slot_info;                                      // per slot: rows of the others, pixel
   int32_t n_pix;
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
   const spiir_trigger* trig;
-  const int32_t* list; const int32_t* counts;                 // this launch: list of slots of trigger detector T
-  int32_t T;                                                  // trigger detector
+  const int32_t* list; const int32_t* counts;                 // slots of trigger detector T
+  int32_t T;
   int32_t n_slides;                                           // 0 = foreground
   int64_t step; int32_t mult[SPIIR_MAX_DET];
-  int32_t lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];   // window of detector I vs T: first delta, width, row offset
-  int32_t win_rows;                                           // total rows
-  int32_t win_elems;                                          // float2 elements of the window region (even)
+  int32_t lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];   // window of detector I vs T: first delta, width, first row
+  int32_t win_elems;                                          // float2 elements of the window region
   spiir_sky_result* out; float* map;
 };
 
 struct PairInfo { int32_t slot, slide, valid, row; float2 vT; long long k; };
 
-__device__ __forceinline__ int unpack_delta(const int32_t w1, const int32_t w2, int I) {
-  if (I == 0) return 0;
-  if (I == 1) return (int)(short)(w1 & 0xFFFF);
-  if (I == 2) return (int)(short)((unsigned)w1 >> 16);
-  return w2;
-}
-
-template <int D, bool MAP>
-__global__ void __launch_bounds__(kSkyThreads, 2) k_sky(const __grid_constant__ SkyParams P) {
-  constexpr int NQ = SkyRec<D>::NQ, RW = SkyRec<D>::RW;
+template <int D, int K, bool MAP>
+__global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ SkyParams P) {
+  constexpr int NO = SkyFmt<D>::NO, NQ = SkyFmt<D>::NQ, SW = SkyFmt<D>::SW;
+  constexpr int NP = 32 * K, NPS = NP + 1;
+  constexpr int kTileWords = (kSkyChunk * SW > 2 * NP) ? kSkyChunk * SW : 2 * NP;   // a warp's chunk tile, reused for the reduction
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2* win = reinterpret_cast<float2*>(smem_raw);                              // [win_rows][NPS]
-  float* tiles = reinterpret_cast<float*>(win + P.win_elems);                     // [warps][32][RW]
-  float* red_c = tiles + kSkyWarps * 32 * RW;                                     // [warps][NP]
-  int* red_p = reinterpret_cast<int*>(red_c + kSkyWarps * kSkyNP);                // [warps][NP]
-  PairInfo* pinfo = reinterpret_cast<PairInfo*>(red_p + kSkyWarps * kSkyNP);      // [NP]
+  float2* win = reinterpret_cast<float2*>(smem_raw);                              // [rows][NPS]
+  float* tiles = reinterpret_cast<float*>(win + P.win_elems);                     // [warps][kTileWords]
+  PairInfo* pinfo = reinterpret_cast<PairInfo*>(tiles + kSkyWarps * kTileWords);  // [NP]
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int T = P.T;
   const int S1 = P.n_slides > 0 ? P.n_slides : 1;
   const long long n_pairs = (long long)P.counts[T] * S1;
-  const long long n_batches = (n_pairs + kSkyNP - 1) / kSkyNP;
+  const long long n_batches = (n_pairs + NP - 1) / NP;
   const int64_t kmin = (P.k_newest - P.ring_len + 1 > 0) ? P.k_newest - P.ring_len + 1 : 0;
-  float* mytile = tiles + warp * 32 * RW;
-  const int rbeg = min(P.n_rec, warp * P.rec_per_warp), rend = min(P.n_rec, rbeg + P.rec_per_warp);
+  float* mytile = tiles + warp * kTileWords;
+  const int c_beg = min(P.n_chunks, warp * P.chunks_per_warp), c_end = min(P.n_chunks, c_beg + P.chunks_per_warp);
 
   for (long long batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
     __syncthreads();                                   // previous batch fully consumed
     // ---- pair set-up: which trigger, which slide, is every gather inside the view
-    if (tid < kSkyNP) {
+    if (tid < NP) {
       PairInfo pi; pi.slot = -1; pi.slide = 0; pi.valid = 0; pi.row = 0; pi.vT = make_float2(0.f, 0.f); pi.k = 0;
-      const long long q = batch * kSkyNP + tid;
+      const long long q = batch * NP + tid;
       if (q < n_pairs) {
         pi.slot = P.list[q / S1];
         pi.slide = (int)(q % S1) + (P.n_slides > 0 ? 1 : 0);
@@ -108,135 +109,136 @@ __global__ void __launch_bounds__(kSkyThreads, 2) k_sky(const __grid_constant__ 
       pinfo[tid] = pi;
     }
     __syncthreads();
-    // ---- delay windows -> shared memory, [row][pair]; a warp reads 32 consecutive samples of one pair
-#pragma unroll
-    for (int I = 0; I < D; ++I) {
-      if (I == T) continue;
+    // ---- delay windows -> shared memory [row][pair]; a warp copies one (pair, detector) window,
+    //      its lanes reading consecutive samples of the ring
+    for (int task = warp; task < NP * NO; task += kSkyWarps) {
+      const int j = task / NO, o = task - j * NO;
+      const int I = o + (o >= T ? 1 : 0);
+      const PairInfo pi = pinfo[j];
       const int W = P.W[I];
-      const int Wp = (W + 31) & ~31;
-      float2* dst = win + (size_t)P.woff[I] * kSkyNPS;
-      for (int idx = tid; idx < kSkyNP * Wp; idx += kSkyThreads) {
-        const int j = idx / Wp, r = idx - j * Wp;
-        if (r >= W) continue;
-        const PairInfo pi = pinfo[j];
-        float2 v = make_float2(0.f, 0.f);
-        if (pi.valid) {
-          const int64_t k0 = pi.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I] + r;
-          v = P.z[(size_t)I * P.det_stride + (size_t)pi.row * P.row_stride + (size_t)(k0 % P.ring_len)];
+      float2* dst = win + (size_t)P.woff[I] * NPS + j;
+      if (pi.valid) {
+        const int64_t k0 = pi.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I];
+        const int64_t base = k0 % P.ring_len;
+        const float2* src = P.z + (size_t)I * P.det_stride + (size_t)pi.row * P.row_stride;
+        for (int r = lane; r < W; r += 32) {
+          int64_t idx = base + r;
+          if (idx >= P.ring_len) idx -= P.ring_len;
+          dst[(size_t)r * NPS] = src[idx];
         }
-        dst[(size_t)r * kSkyNPS + j] = v;
+      } else {
+        for (int r = lane; r < W; r += 32) dst[(size_t)r * NPS] = make_float2(0.f, 0.f);
       }
     }
     __syncthreads();
 
-    // ---- the direction stream: this warp's share, tile by tile
-    float2 vT[kSkyK];
-    float best[kSkyK]; int bpix[kSkyK];
+    // ---- the direction stream: this warp's chunks
+    float2 vT[K], v[NO][K];
+    float best[K]; int bidx[K];
+    float q[K][NQ];
+    long long mrow[K];                                  // sky-map row of each pair, -1 = none
 #pragma unroll
-    for (int a = 0; a < kSkyK; ++a) { vT[a] = pinfo[lane + 32 * a].vT; best[a] = -1.f; bpix[a] = INT_MAX; }
-    long long mrow[kSkyK];                                  // sky-map row of each pair, -1 = none
-#pragma unroll
-    for (int a = 0; a < kSkyK; ++a) {
+    for (int a = 0; a < K; ++a) {
       const PairInfo pi = pinfo[lane + 32 * a];
+      vT[a] = pi.vT; best[a] = -1.f; bidx[a] = 0;
       mrow[a] = (MAP && pi.valid) ? (long long)pi.slot * P.n_pix : -1;
-    }
-    float q[kSkyK][NQ];
-#pragma unroll
-    for (int a = 0; a < kSkyK; ++a)
 #pragma unroll
       for (int e = 0; e < NQ; ++e) q[a][e] = 0.f;
-    int cur_w1 = INT_MIN, cur_w2 = INT_MIN;
+      q[a][0] = fmaf(vT[a].x, vT[a].x, vT[a].y * vT[a].y);
+#pragma unroll
+      for (int o = 0; o < NO; ++o) v[o][a] = make_float2(0.f, 0.f);
+    }
 
-    float4 pre[RW / 4];
-    if (rbeg < rend) {
-      const int r = min(rbeg + lane, P.n_rec - 1);
+    float4 pre[SW / 4];
+    if (c_beg < c_end) {
+      const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)c_beg * kSkyChunk + lane) * SW);
 #pragma unroll
-      for (int c = 0; c < RW / 4; ++c) pre[c] = __ldg(reinterpret_cast<const float4*>(P.rec + (size_t)r * RW) + c);
+      for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
     }
-    for (int t0 = rbeg; t0 < rend; t0 += 32) {
+    for (int ch = c_beg; ch < c_end; ++ch) {
       __syncwarp();
 #pragma unroll
-      for (int c = 0; c < RW / 4; ++c) reinterpret_cast<float4*>(mytile + lane * RW)[c] = pre[c];
+      for (int c = 0; c < SW / 4; ++c) reinterpret_cast<float4*>(mytile + lane * SW)[c] = pre[c];
       __syncwarp();
-      if (t0 + 32 < rend) {                                   // prefetch the next tile while this one is consumed
-        const int r = min(t0 + 32 + lane, P.n_rec - 1);
+      if (ch + 1 < c_end) {                                   // prefetch the next chunk while this one is consumed
+        const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)(ch + 1) * kSkyChunk + lane) * SW);
 #pragma unroll
-        for (int c = 0; c < RW / 4; ++c) pre[c] = __ldg(reinterpret_cast<const float4*>(P.rec + (size_t)r * RW) + c);
+        for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
       }
-      const int cnt = min(32, rend - t0);
-      for (int r = 0; r < cnt; ++r) {
-        float w[RW];
+      int s = 0;
+      while (s < kSkyChunk) {
+        const int4 h = *reinterpret_cast<const int4*>(mytile + s * SW);          // broadcast read
+        const int count = h.w & 0xFF, level = h.w >> 8;
+        if (level == kSkyEnd) break;
+        // new delay tuple: gather the rows that changed, refresh the products they enter
 #pragma unroll
-        for (int c = 0; c < RW / 4; ++c) {
-          const float4 v = reinterpret_cast<const float4*>(mytile + r * RW)[c];   // broadcast read
-          w[4 * c] = v.x; w[4 * c + 1] = v.y; w[4 * c + 2] = v.z; w[4 * c + 3] = v.w;
-        }
-        const int pix = __float_as_int(w[NQ]);
-        const int w1 = __float_as_int(w[NQ + 1]);
-        const int w2 = (D > 3) ? __float_as_int(w[NQ + 2]) : 0;
-        if (w1 != cur_w1 || w2 != cur_w2) {                   // new delay tuple: gather once, form q_IJ once
-          cur_w1 = w1; cur_w2 = w2;
-          const int dT = unpack_delta(w1, w2, T);
+        for (int o = 0; o < NO; ++o) {
+          if (level <= o) {
+            const int row = (o == 0) ? h.x : (o == 1) ? h.y : h.z;
+            const float2* rp = win + (size_t)row * NPS + lane;
 #pragma unroll
-          for (int a = 0; a < kSkyK; ++a) {
-            float2 v[D];
+            for (int a = 0; a < K; ++a) {
+              const float2 x = rp[32 * a];
+              v[o][a] = x;
+              q[a][1 + o] = fmaf(x.x, x.x, x.y * x.y);
+              q[a][1 + NO + o] = fmaf(vT[a].x, x.x, vT[a].y * x.y);
 #pragma unroll
-            for (int I = 0; I < D; ++I) {
-              if (I == T) { v[I] = vT[a]; continue; }
-              const int row = P.woff[I] + (unpack_delta(w1, w2, I) - dT - P.lo[I]);
-              v[I] = win[(size_t)row * kSkyNPS + lane + 32 * a];
+              for (int o2 = 0; o2 < o; ++o2)
+                q[a][1 + 2 * NO + o * (o - 1) / 2 + o2] = fmaf(v[o2][a].x, x.x, v[o2][a].y * x.y);
             }
-#pragma unroll
-            for (int I = 0; I < D; ++I) q[a][I] = fmaf(v[I].x, v[I].x, v[I].y * v[I].y);
-            int e = D;
-#pragma unroll
-            for (int J = 1; J < D; ++J)
-#pragma unroll
-              for (int I = 0; I < J; ++I) { q[a][e] = fmaf(v[I].x, v[J].x, v[I].y * v[J].y); ++e; }
           }
         }
+        const float* rec = mytile + (s + 1) * SW;
+        int gs = ch * kSkyChunk + s + 1;
+        for (int i = 0; i < count; ++i, rec += SW, ++gs) {
+          float w[SW];
 #pragma unroll
-        for (int a = 0; a < kSkyK; ++a) {
-          float c = w[0] * q[a][0];
-#pragma unroll
-          for (int e = 1; e < NQ; ++e) c = fmaf(w[e], q[a][e], c);
-          if (MAP) {
-            if (mrow[a] >= 0) P.map[mrow[a] + pix] = c;
+          for (int c = 0; c < SW / 4; ++c) {
+            const float4 t = reinterpret_cast<const float4*>(rec)[c];             // broadcast read
+            w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
           }
-          if (c >= best[a]) {
-            if (c > best[a] || pix < bpix[a]) { best[a] = c; bpix[a] = pix; }
+#pragma unroll
+          for (int a = 0; a < K; ++a) {
+            float c = w[0] * q[a][0];
+#pragma unroll
+            for (int e = 1; e < NQ; ++e) c = fmaf(w[e], q[a][e], c);
+            if (MAP) {
+              if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = c;
+            }
+            if (c > best[a]) { best[a] = c; bidx[a] = gs; }
           }
         }
+        s += 1 + count;
       }
     }
+    __syncthreads();                                   // every warp is done with its tile: reuse it for the reduction
+    {
+      float* red_c = mytile; int* red_i = reinterpret_cast<int*>(mytile + NP);
 #pragma unroll
-    for (int a = 0; a < kSkyK; ++a) {
-      red_c[warp * kSkyNP + lane + 32 * a] = best[a];
-      red_p[warp * kSkyNP + lane + 32 * a] = bpix[a];
+      for (int a = 0; a < K; ++a) { red_c[lane + 32 * a] = best[a]; red_i[lane + 32 * a] = bidx[a]; }
     }
     __syncthreads();
-    // ---- across the warps, then tot2 / null2 at the winning direction (Eq. 10)
-    if (tid < kSkyNP) {
+    // ---- across the warps (first in stream order on exact ties), then tot2 / null2 at the winner (Eq. 10)
+    if (tid < NP) {
       const PairInfo pi = pinfo[tid];
       if (pi.slot >= 0) {
         spiir_sky_result res; res.coh2 = 0.f; res.null2 = 0.f; res.tot2 = 0.f; res.pix = -1;
         if (pi.valid) {
-          float bc = red_c[tid]; int bp = red_p[tid];
+          float bc = tiles[tid]; int bi = reinterpret_cast<const int*>(tiles + NP)[tid];
           for (int wv = 1; wv < kSkyWarps; ++wv) {
-            const float c = red_c[wv * kSkyNP + tid]; const int p = red_p[wv * kSkyNP + tid];
-            if (c > bc || (c == bc && p < bp)) { bc = c; bp = p; }
+            const float c = tiles[wv * kTileWords + tid];
+            const int i = reinterpret_cast<const int*>(tiles + wv * kTileWords + NP)[tid];
+            if (c > bc) { bc = c; bi = i; }
           }
-          const int4 dl = __ldg(reinterpret_cast<const int4*>(P.pix_delta) + bp);
-          const int dd[4] = {0, dl.y, dl.z, dl.w};
-          float tot = 0.f;
+          const int4 info = __ldg(P.slot_info + bi);
+          const int rows[3] = {info.x, info.y, info.z};
+          float tot = fmaf(pi.vT.x, pi.vT.x, pi.vT.y * pi.vT.y);
 #pragma unroll
-          for (int I = 0; I < D; ++I) {
-            float2 v;
-            if (I == T) v = pi.vT;
-            else v = win[(size_t)(P.woff[I] + (dd[I] - dd[T] - P.lo[I])) * kSkyNPS + tid];
-            tot += fmaf(v.x, v.x, v.y * v.y);
+          for (int o = 0; o < NO; ++o) {
+            const float2 x = win[(size_t)rows[o] * NPS + tid];
+            tot += fmaf(x.x, x.x, x.y * x.y);
           }
-          res.coh2 = bc; res.tot2 = tot; res.null2 = fmaxf(tot - bc, 0.f); res.pix = bp;
+          res.coh2 = bc; res.tot2 = tot; res.null2 = fmaxf(tot - bc, 0.f); res.pix = info.w;
         }
         P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
       }
@@ -264,30 +266,118 @@ __global__ void __launch_bounds__(256) k_sky_bin(const spiir_trigger* trig, int 
 
 using namespace spiir;
 
+struct spiir_sky_stream {                 // the direction stream of one trigger detector
+  int n_chunks = 0, n_tuples = 0, rows = 0, k_max = 0;
+  int lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];
+  size_t off_slots = 0, off_info = 0;
+};
+
 struct spiir_sky_plan {
-  int n_det = 0, n_pix = 0, max_slots = 0, n_rec = 0, n_tuples = 0, rec_per_warp = 0, RW = 0;
+  int n_det = 0, n_pix = 0, max_slots = 0, n_tuples = 0, SW = 0, cap_slots = 0;
   char* ws = nullptr;
-  size_t off_rec = 0, off_pixd = 0, off_lists = 0, off_counts = 0, bytes = 0;
-  int lo[SPIIR_MAX_DET][SPIIR_MAX_DET], hi[SPIIR_MAX_DET][SPIIR_MAX_DET];    // [T][I]
+  size_t off_lists = 0, off_counts = 0, bytes = 0;
+  spiir_sky_stream st[SPIIR_MAX_DET];
   int num_sms = 148;
 };
 
 static size_t sky_align(size_t x) { return (x + 255) / 256 * 256; }
-static int sky_win_elems(int rows) { return (rows * kSkyNPS + 1) & ~1; }
-static size_t sky_smem_bytes(int rows, int RW) {
-  return (size_t)sky_win_elems(rows) * 8 + (size_t)kSkyWarps * 32 * RW * 4 + (size_t)kSkyWarps * kSkyNP * 8 +
-         kSkyNP * sizeof(PairInfo);
+static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 1 + 3) / 4 * 4; }
+static int sky_win_elems(int rows, int K) { return (rows * (32 * K + 1) + 1) & ~1; }
+static size_t sky_smem_bytes(int rows, int SW, int K) {
+  const int NP = 32 * K, tile = std::max(kSkyChunk * SW, 2 * NP);
+  return (size_t)sky_win_elems(rows, K) * 8 + (size_t)kSkyWarps * tile * 4 + (size_t)NP * sizeof(PairInfo);
 }
 
 static void sky_layout(spiir_sky_plan* pl) {
   const int D = pl->n_det;
-  pl->RW = (D * (D + 1) / 2 + 3 + 3) / 4 * 4;
+  pl->SW = sky_slot_words(D);
+  // a chunk wastes at most one slot and repeats at most one header: slots <= 2 n_pix * 32/30 + a chunk
+  pl->cap_slots = (int)(((size_t)pl->n_pix * 2 * 16 / 15 + 2 * kSkyChunk + kSkyChunk - 1) / kSkyChunk * kSkyChunk);
   size_t cur = 0;
-  pl->off_rec = cur;    cur = sky_align(cur + (size_t)pl->n_pix * pl->RW * 4);
-  pl->off_pixd = cur;   cur = sky_align(cur + (size_t)pl->n_pix * 16);
+  for (int T = 0; T < D; ++T) {
+    pl->st[T].off_slots = cur; cur = sky_align(cur + (size_t)pl->cap_slots * pl->SW * 4);
+    pl->st[T].off_info = cur;  cur = sky_align(cur + (size_t)pl->cap_slots * 16);
+  }
   pl->off_lists = cur;  cur = sky_align(cur + (size_t)D * pl->max_slots * 4);
   pl->off_counts = cur; cur = sky_align(cur + SPIIR_MAX_DET * 4);
   pl->bytes = cur;
+}
+
+// Builds the chunked stream of trigger detector T on the host (slots + per-slot info).
+static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const int32_t* delay,
+                             std::vector<float>& slots, std::vector<int32_t>& info) {
+  const int D = pl->n_det, NO = D - 1, NQ = D * (D + 1) / 2, SW = pl->SW, n_pix = pl->n_pix;
+  spiir_sky_stream& S = pl->st[T];
+  int oth[SPIIR_MAX_DET];
+  for (int o = 0; o < NO; ++o) oth[o] = o + (o >= T ? 1 : 0);
+  std::vector<int32_t> rows((size_t)n_pix * 3, 0);
+  for (int p = 0; p < n_pix; ++p)
+    for (int o = 0; o < NO; ++o) {
+      const int I = oth[o];
+      rows[(size_t)p * 3 + o] = S.woff[I] + (delay[(size_t)p * D + I] - delay[(size_t)p * D + T] - S.lo[I]);
+    }
+  std::vector<int32_t> order(n_pix);
+  for (int p = 0; p < n_pix; ++p) order[p] = p;
+  std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
+    for (int o = 0; o < 3; ++o)
+      if (rows[(size_t)x * 3 + o] != rows[(size_t)y * 3 + o]) return rows[(size_t)x * 3 + o] < rows[(size_t)y * 3 + o];
+    return x < y;
+  });
+  slots.clear(); info.clear();
+  int used = 0;                            // slots used in the current chunk
+  bool have_prev = false; int32_t prev[3] = {0, 0, 0};
+  auto push_slot = [&]() { slots.resize(slots.size() + SW, 0.f); info.resize(info.size() + 4, 0); ++used; };
+  auto end_chunk = [&]() {
+    if (used == 0 || used == kSkyChunk) { if (used == kSkyChunk) used = 0; have_prev = false; return; }
+    push_slot();
+    const int32_t hw = kSkyEnd << 8;
+    memcpy(&slots[slots.size() - SW + 3], &hw, 4);
+    while (used < kSkyChunk) push_slot();
+    used = 0; have_prev = false;
+  };
+  S.n_tuples = 0;
+  int i = 0;
+  while (i < n_pix) {
+    int j = i + 1;
+    while (j < n_pix && memcmp(&rows[(size_t)order[j] * 3], &rows[(size_t)order[i] * 3], 12) == 0) ++j;
+    ++S.n_tuples;
+    const int32_t* rw = &rows[(size_t)order[i] * 3];
+    int remaining = j - i, at = i;
+    while (remaining > 0) {
+      if (used == kSkyChunk) { used = 0; have_prev = false; }
+      if (kSkyChunk - used < 2) end_chunk();
+      int level = 0;
+      if (have_prev) { while (level < NO && prev[level] == rw[level]) ++level; if (level >= NO) level = NO - 1; }
+      const int cnt = std::min(remaining, kSkyChunk - used - 1);
+      push_slot();
+      {
+        int32_t h[4] = {rw[0], rw[1], rw[2], cnt | (level << 8)};
+        memcpy(&slots[slots.size() - SW], h, 16);
+      }
+      for (int c = 0; c < cnt; ++c) {
+        const int p = order[at + c];
+        push_slot();
+        float* w = &slots[slots.size() - SW];
+        const float* u = u2 + (size_t)p * D * 2;
+        auto M = [&](int I, int J) { return (double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]; };
+        // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order
+        w[0] = (float)M(T, T);
+        for (int o = 0; o < NO; ++o) w[1 + o] = (float)M(oth[o], oth[o]);
+        for (int o = 0; o < NO; ++o) w[1 + NO + o] = (float)(2.0 * M(T, oth[o]));
+        for (int o = 1; o < NO; ++o)
+          for (int o2 = 0; o2 < o; ++o2) w[1 + 2 * NO + o * (o - 1) / 2 + o2] = (float)(2.0 * M(oth[o2], oth[o]));
+        const int32_t pix = p;
+        memcpy(w + NQ, &pix, 4);
+        int32_t* inf = &info[info.size() - 4];
+        inf[0] = rw[0]; inf[1] = rw[1]; inf[2] = rw[2]; inf[3] = p;
+      }
+      prev[0] = rw[0]; prev[1] = rw[1]; prev[2] = rw[2]; have_prev = true;
+      remaining -= cnt; at += cnt;
+    }
+    i = j;
+  }
+  end_chunk();
+  S.n_chunks = (int)(slots.size() / ((size_t)SW * kSkyChunk));
 }
 
 extern "C" {
@@ -311,71 +401,44 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
   pl->n_det = n_det; pl->n_pix = n_pix; pl->max_slots = max_slots;
   sky_layout(pl);
   if (bytes < pl->bytes) { set_error("workspace too small: %zu < %zu", bytes, pl->bytes); delete pl; return SPIIR_ENOMEM; }
-  const int D = n_det, NQ = D * (D + 1) / 2, RW = pl->RW;
-  for (int T = 0; T < D; ++T) for (int I = 0; I < D; ++I) { pl->lo[T][I] = INT_MAX; pl->hi[T][I] = INT_MIN; }
-  std::vector<int32_t> pixd((size_t)n_pix * 4, 0);
-  for (int p = 0; p < n_pix; ++p) {
-    for (int I = 0; I < D; ++I) {
-      const long long d = (long long)delay[(size_t)p * D + I] - delay[(size_t)p * D];
-      if (d < -32000 || d > 32000) { set_error("pixel %d: delay difference %lld does not fit the plan", p, d); delete pl; return SPIIR_EINVAL; }
-      pixd[(size_t)p * 4 + I] = (int32_t)d;
-    }
-    for (int T = 0; T < D; ++T) for (int I = 0; I < D; ++I) {
-      const int d = delay[(size_t)p * D + I] - delay[(size_t)p * D + T];
-      pl->lo[T][I] = std::min(pl->lo[T][I], d); pl->hi[T][I] = std::max(pl->hi[T][I], d);
-    }
-  }
-  // directions sorted by delay tuple, then by pixel index
-  std::vector<int32_t> order(n_pix);
-  for (int p = 0; p < n_pix; ++p) order[p] = p;
-  std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
-    for (int I = 1; I < D; ++I) {
-      const int32_t dx = pixd[(size_t)x * 4 + I], dy = pixd[(size_t)y * 4 + I];
-      if (dx != dy) return dx < dy;
-    }
-    return x < y;
-  });
-  std::vector<float> rec((size_t)n_pix * RW, 0.f);
-  int n_tuples = 0;
-  for (int r = 0; r < n_pix; ++r) {
-    const int p = order[r];
-    float* w = rec.data() + (size_t)r * RW;
-    const float* u = u2 + (size_t)p * D * 2;
-    // projector M = U2 U2^T in float64 from the float32 table, rounded once
-    for (int I = 0; I < D; ++I) w[I] = (float)((double)u[2 * I] * u[2 * I] + (double)u[2 * I + 1] * u[2 * I + 1]);
-    int e = D;
-    for (int J = 1; J < D; ++J)
-      for (int I = 0; I < J; ++I)
-        w[e++] = (float)(2.0 * ((double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]));
-    int32_t iw[3];
-    iw[0] = p;
-    iw[1] = (int32_t)(((uint32_t)(uint16_t)(int16_t)pixd[(size_t)p * 4 + 1]) |
-                      ((uint32_t)(uint16_t)(int16_t)(D > 2 ? pixd[(size_t)p * 4 + 2] : 0) << 16));
-    iw[2] = D > 3 ? pixd[(size_t)p * 4 + 3] : 0;
-    memcpy(w + NQ, iw, sizeof(iw));
-    if (r == 0 || memcmp(&pixd[(size_t)p * 4], &pixd[(size_t)order[r - 1] * 4], 16) != 0) ++n_tuples;
-  }
-  pl->n_rec = n_pix; pl->n_tuples = n_tuples;
-  pl->rec_per_warp = ((n_pix + kSkyWarps - 1) / kSkyWarps + 31) / 32 * 32;
-  // shared-memory need of the widest trigger detector
-  for (int T = 0; T < D; ++T) {
-    int rows = 0;
-    for (int I = 0; I < D; ++I) if (I != T) rows += pl->hi[T][I] - pl->lo[T][I] + 1;
-    const size_t smem = sky_smem_bytes(rows, RW);
-    if (smem > (size_t)kSkySmemMax) {
-      set_error("delay span of trigger detector %d needs %zu bytes of shared memory (> %d)", T, smem, kSkySmemMax);
-      delete pl; return SPIIR_EINVAL;
-    }
-  }
+  const int D = n_det;
   pl->ws = (char*)dev_workspace;
   cudaStream_t st = (cudaStream_t)stream;
-  cudaError_t e = cudaMemcpyAsync(pl->ws + pl->off_rec, rec.data(), rec.size() * 4, cudaMemcpyHostToDevice, st);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(pl->ws + pl->off_pixd, pixd.data(), pixd.size() * 4, cudaMemcpyHostToDevice, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  std::vector<float> slots; std::vector<int32_t> info;
+  for (int T = 0; T < D; ++T) {
+    spiir_sky_stream& S = pl->st[T];
+    int rows = 0;
+    for (int I = 0; I < D; ++I) {
+      int lo = INT_MAX, hi = INT_MIN;
+      for (int p = 0; p < n_pix; ++p) {
+        const long long d = (long long)delay[(size_t)p * D + I] - delay[(size_t)p * D + T];
+        if (d < -1000000 || d > 1000000) { set_error("pixel %d: delay difference %lld out of range", p, d); delete pl; return SPIIR_EINVAL; }
+        lo = std::min(lo, (int)d); hi = std::max(hi, (int)d);
+      }
+      S.lo[I] = lo; S.W[I] = hi - lo + 1; S.woff[I] = rows;
+      if (I != T) rows += S.W[I];
+    }
+    S.rows = rows;
+    S.k_max = 0;
+    for (int K = kSkyKMax; K >= 1; --K)
+      if (sky_smem_bytes(rows, pl->SW, K) <= (size_t)kSkySmemMax) { S.k_max = K; break; }
+    if (S.k_max == 0) {
+      set_error("delay span of trigger detector %d needs %zu bytes of shared memory (> %d)", T,
+                sky_smem_bytes(rows, pl->SW, 1), kSkySmemMax);
+      delete pl; return SPIIR_EINVAL;
+    }
+    sky_build_stream(pl, T, u2, delay, slots, info);
+    if ((int)(slots.size() / pl->SW) > pl->cap_slots) { set_error("stream of detector %d exceeds its bound", T); delete pl; return SPIIR_EOVERFLOW; }
+    cudaError_t e = cudaMemcpyAsync(pl->ws + S.off_slots, slots.data(), slots.size() * 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->ws + S.off_info, info.data(), info.size() * 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);     // the host images are reused for the next detector
+    if (e != cudaSuccess) { set_error("sky plan upload failed: %s", cudaGetErrorString(e)); delete pl; return SPIIR_ECUDA; }
+    pl->n_tuples = std::max(pl->n_tuples, S.n_tuples);
+  }
   int dev = 0, sms = 0;
-  if (e == cudaSuccess) e = cudaGetDevice(&dev);
+  cudaError_t e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (e != cudaSuccess) { set_error("sky plan upload failed: %s", cudaGetErrorString(e)); delete pl; return SPIIR_ECUDA; }
+  if (e != cudaSuccess) { set_error("device query failed: %s", cudaGetErrorString(e)); delete pl; return SPIIR_ECUDA; }
   pl->num_sms = sms > 0 ? sms : 148;
   *out = pl;
   return SPIIR_OK;
@@ -391,17 +454,29 @@ int32_t spiir_sky_plan_tuples(const spiir_sky_plan* pl) { return pl ? pl->n_tupl
 
 }  // extern "C"
 
-template <int D, bool MAP>
-static int sky_launch_one(const SkyParams& P, int grid, size_t smem, cudaStream_t st) {
-  static size_t configured = 0;
-  if (smem > configured) {
-    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_sky<D, MAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSkySmemMax));
-    configured = kSkySmemMax;
+template <int D, int K, bool MAP>
+static int sky_launch_one(const SkyParams& P, long long max_batches, int num_sms, size_t smem, cudaStream_t st) {
+  static bool configured = false;
+  if (!configured) {
+    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_sky<D, K, MAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSkySmemMax));
+    configured = true;
   }
-  k_sky<D, MAP><<<grid, kSkyThreads, smem, st>>>(P);
+  const int grid = (int)std::max<long long>(1, std::min<long long>(max_batches, num_sms));
+  k_sky<D, K, MAP><<<grid, kSkyThreads, smem, st>>>(P);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());
   return SPIIR_OK;
+}
+
+template <int D, bool MAP>
+static int sky_launch_k(int K, const SkyParams& P, long long max_pairs, int num_sms, size_t smem, cudaStream_t st) {
+  const long long nb = (max_pairs + 32 * K - 1) / (32 * K);
+  switch (K) {
+    case 1: return sky_launch_one<D, 1, MAP>(P, nb, num_sms, smem, st);
+    case 2: return sky_launch_one<D, 2, MAP>(P, nb, num_sms, smem, st);
+    case 3: return sky_launch_one<D, 3, MAP>(P, nb, num_sms, smem, st);
+    default: return sky_launch_one<D, 4, MAP>(P, nb, num_sms, smem, st);
+  }
 }
 
 static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_trigger* trig, int32_t n_slots,
@@ -422,31 +497,33 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
   k_sky_bin<<<(n_slots + 255) / 256, 256, 0, st>>>(trig, n_slots, D, S1, lists, counts, pl->max_slots, out);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());
+  // pairs one launch can see at most (the real count is on the device): all slots of one detector
+  const long long max_pairs = (long long)n_slots * S1;
   for (int T = 0; T < D; ++T) {
+    const spiir_sky_stream& S = pl->st[T];
     SkyParams P;
     memset(&P, 0, sizeof(P));
-    P.rec = (const float*)(pl->ws + pl->off_rec); P.n_rec = pl->n_rec; P.rec_per_warp = pl->rec_per_warp;
-    P.pix_delta = (const int32_t*)(pl->ws + pl->off_pixd); P.n_pix = pl->n_pix;
+    P.stream = (const float*)(pl->ws + S.off_slots); P.n_chunks = S.n_chunks;
+    P.chunks_per_warp = (S.n_chunks + kSkyWarps - 1) / kSkyWarps;
+    P.slot_info = (const int4*)(pl->ws + S.off_info); P.n_pix = pl->n_pix;
     P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;
     P.ring_len = view->ring_len; P.k_newest = view->k_newest;
     P.trig = trig; P.list = lists + (size_t)T * pl->max_slots; P.counts = counts; P.T = T;
     P.n_slides = n_slides; P.step = step;
-    int rows = 0;
     for (int I = 0; I < D; ++I) {
       P.mult[I] = (mult && I != T) ? mult[I] : 0;
-      P.lo[I] = pl->lo[T][I]; P.W[I] = pl->hi[T][I] - pl->lo[T][I] + 1;
-      P.woff[I] = rows;
-      if (I != T) rows += P.W[I];
+      P.lo[I] = S.lo[I]; P.W[I] = S.W[I]; P.woff[I] = S.woff[I];
     }
-    P.win_rows = rows; P.win_elems = sky_win_elems(rows);
+    // pairs per thread: as many as shared memory allows, fewer when the launch could not fill the SMs
+    int K = S.k_max;
+    while (K > 1 && max_pairs / D < (long long)pl->num_sms * 32 * K) --K;
+    P.win_elems = sky_win_elems(S.rows, K);
     P.out = out; P.map = map;
-    const size_t smem = sky_smem_bytes(rows, pl->RW);
-    const long long max_batches = ((long long)n_slots * S1 + kSkyNP - 1) / kSkyNP;
-    const int grid = (int)std::min<long long>(max_batches, (long long)pl->num_sms * 2);
+    const size_t smem = sky_smem_bytes(S.rows, pl->SW, K);
     int rc;
-    if (D == 2)      rc = map ? sky_launch_one<2, true>(P, grid, smem, st) : sky_launch_one<2, false>(P, grid, smem, st);
-    else if (D == 3) rc = map ? sky_launch_one<3, true>(P, grid, smem, st) : sky_launch_one<3, false>(P, grid, smem, st);
-    else             rc = map ? sky_launch_one<4, true>(P, grid, smem, st) : sky_launch_one<4, false>(P, grid, smem, st);
+    if (D == 2)      rc = map ? sky_launch_k<2, true>(K, P, max_pairs, pl->num_sms, smem, st) : sky_launch_k<2, false>(K, P, max_pairs, pl->num_sms, smem, st);
+    else if (D == 3) rc = map ? sky_launch_k<3, true>(K, P, max_pairs, pl->num_sms, smem, st) : sky_launch_k<3, false>(K, P, max_pairs, pl->num_sms, smem, st);
+    else             rc = map ? sky_launch_k<4, true>(K, P, max_pairs, pl->num_sms, smem, st) : sky_launch_k<4, false>(K, P, max_pairs, pl->num_sms, smem, st);
     if (rc) return rc;
   }
   return SPIIR_OK;
