@@ -36,22 +36,23 @@ constexpr int kSkyWarps = kSkyThreads / 32;
 constexpr int kSkyChunk = 32;               // slots per stream chunk (one per lane when staging)
 constexpr int kSkyKMax = 4;                 // (trigger, slide) pairs per thread, at most
 constexpr int kSkySmemMax = 227 * 1024;     // opt-in dynamic shared memory per CTA on sm_100
-constexpr int kSkyEnd = 15;                 // header level that ends a chunk
 
 template <int D> struct SkyFmt {
   static constexpr int NO = D - 1;                       // detectors other than the trigger detector
   static constexpr int NQ = D * (D + 1) / 2;             // independent entries of the projector
-  static constexpr int SW = (NQ + 1 + 3) / 4 * 4;        // words per slot: NQ weights + pixel, padded to 16 B
+  static constexpr int SW = (NQ + 1 + 3) / 4 * 4;        // words per slot: NQ weights + tag, padded to 16 B
 };
-// header slot : word 0..2 window row of other detector o (already offset by its window's first row),
-//               word 3 = count | level << 8 (level = first other detector whose row changed; kSkyEnd = end)
-// direction   : words [0,NQ) weights, word NQ = pixel.  Weight order (T = trigger detector, o = others in
-//               increasing detector index): M_TT; M_oo (o = 0..NO-1); 2 M_To; 2 M_o'o for o' < o,
+// Every slot is SW words; word NQ is its tag.
+//   header slot (tag < 0): words 0..NO-1 = window row of other detector o (already offset by its window's
+//               first row); tag = -1 - level, level = first other detector whose row differs from the
+//               previous header of the SAME chunk (0 for a chunk's first header: refresh everything).
+//   direction   (tag >= 0): words [0,NQ) weights, tag = pixel.  Weight order (T = trigger detector, o = others
+//               in increasing detector index): M_TT; M_oo (o = 0..NO-1); 2 M_To; 2 M_o'o for o' < o,
 //               (0,1) (0,2) (1,2).
+// A chunk always starts with a header and is padded at its end with copies of its last direction.
 
 struct SkyParams {
   const float* stream; int32_t n_chunks, chunks_per_warp;     // this trigger detector's stream
-  const int4* slot_info;                                      // per slot: rows of the others, pixel
   int32_t n_pix;
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
   const spiir_trigger* trig;
@@ -65,6 +66,24 @@ struct SkyParams {
 };
 
 struct PairInfo { int32_t slot, slide, valid, row; float2 vT; long long k; };
+
+__device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src_gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)),
+               "l"(src_gmem)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// q_IJ = Re(v_I conj v_J), the same two roundings wherever it is formed (main loop and rescan)
+__device__ __forceinline__ float re_prod(float2 x, float2 y) { return __fmaf_rn(x.x, y.x, __fmul_rn(x.y, y.y)); }
+
+template <int NQ>
+__device__ __forceinline__ float quad_form(const float* __restrict__ w, const float (&q)[NQ]) {
+  float c = __fmul_rn(w[0], q[0]);
+#pragma unroll
+  for (int e = 1; e < NQ; ++e) c = __fmaf_rn(w[e], q[e], c);
+  return c;
+}
 
 template <int D, int K, bool MAP>
 __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ SkyParams P) {
@@ -109,8 +128,8 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       pinfo[tid] = pi;
     }
     __syncthreads();
-    // ---- delay windows -> shared memory [row][pair]; a warp copies one (pair, detector) window,
-    //      its lanes reading consecutive samples of the ring
+    // ---- delay windows -> shared memory [row][pair] with cp.async (all copies of the batch in flight at
+    //      once); a warp copies one (pair, detector) window, its lanes reading consecutive ring samples
     for (int task = warp; task < NP * NO; task += kSkyWarps) {
       const int j = task / NO, o = task - j * NO;
       const int I = o + (o >= T ? 1 : 0);
@@ -124,27 +143,29 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         for (int r = lane; r < W; r += 32) {
           int64_t idx = base + r;
           if (idx >= P.ring_len) idx -= P.ring_len;
-          dst[(size_t)r * NPS] = src[idx];
+          cp_async_8(dst + (size_t)r * NPS, src + idx);
         }
       } else {
         for (int r = lane; r < W; r += 32) dst[(size_t)r * NPS] = make_float2(0.f, 0.f);
       }
     }
+    cp_async_wait_all();
     __syncthreads();
 
-    // ---- the direction stream: this warp's chunks
+    // ---- the direction stream: this warp's chunks.  Only the running maximum is kept per direction
+    //      (one FMNMX); which chunk raised it last is noted per chunk, and that chunk is rescanned below.
     float2 vT[K], v[NO][K];
-    float best[K]; int bidx[K];
+    float best[K], seen[K]; int bch[K];
     float q[K][NQ];
     long long mrow[K];                                  // sky-map row of each pair, -1 = none
 #pragma unroll
     for (int a = 0; a < K; ++a) {
       const PairInfo pi = pinfo[lane + 32 * a];
-      vT[a] = pi.vT; best[a] = -1.f; bidx[a] = 0;
+      vT[a] = pi.vT; best[a] = -1.f; seen[a] = -1.f; bch[a] = c_beg;
       mrow[a] = (MAP && pi.valid) ? (long long)pi.slot * P.n_pix : -1;
 #pragma unroll
       for (int e = 0; e < NQ; ++e) q[a][e] = 0.f;
-      q[a][0] = fmaf(vT[a].x, vT[a].x, vT[a].y * vT[a].y);
+      q[a][0] = re_prod(vT[a], vT[a]);
 #pragma unroll
       for (int o = 0; o < NO; ++o) v[o][a] = make_float2(0.f, 0.f);
     }
@@ -165,60 +186,57 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
       }
-      int s = 0;
-      while (s < kSkyChunk) {
-        const int4 h = *reinterpret_cast<const int4*>(mytile + s * SW);          // broadcast read
-        const int count = h.w & 0xFF, level = h.w >> 8;
-        if (level == kSkyEnd) break;
-        // new delay tuple: gather the rows that changed, refresh the products they enter
+#pragma unroll 4
+      for (int s = 0; s < kSkyChunk; ++s) {
+        float w[SW];
 #pragma unroll
-        for (int o = 0; o < NO; ++o) {
-          if (level <= o) {
-            const int row = (o == 0) ? h.x : (o == 1) ? h.y : h.z;
-            const float2* rp = win + (size_t)row * NPS + lane;
+        for (int c = 0; c < SW / 4; ++c) {
+          const float4 t = reinterpret_cast<const float4*>(mytile + s * SW)[c];   // broadcast read
+          w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
+        }
+        const int tag = __float_as_int(w[NQ]);
+        if (tag < 0) {
+          // new delay tuple: gather the rows that changed, refresh the products they enter
+          const int level = -1 - tag;
 #pragma unroll
-            for (int a = 0; a < K; ++a) {
-              const float2 x = rp[32 * a];
-              v[o][a] = x;
-              q[a][1 + o] = fmaf(x.x, x.x, x.y * x.y);
-              q[a][1 + NO + o] = fmaf(vT[a].x, x.x, vT[a].y * x.y);
+          for (int o = 0; o < NO; ++o) {
+            if (level <= o) {
+              const float2* rp = win + (size_t)__float_as_int(w[o]) * NPS + lane;
 #pragma unroll
-              for (int o2 = 0; o2 < o; ++o2)
-                q[a][1 + 2 * NO + o * (o - 1) / 2 + o2] = fmaf(v[o2][a].x, x.x, v[o2][a].y * x.y);
+              for (int a = 0; a < K; ++a) {
+                const float2 x = rp[32 * a];
+                v[o][a] = x;
+                q[a][1 + o] = re_prod(x, x);
+                q[a][1 + NO + o] = re_prod(vT[a], x);
+#pragma unroll
+                for (int o2 = 0; o2 < o; ++o2) q[a][1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(v[o2][a], x);
+              }
             }
           }
-        }
-        const float* rec = mytile + (s + 1) * SW;
-        int gs = ch * kSkyChunk + s + 1;
-        for (int i = 0; i < count; ++i, rec += SW, ++gs) {
-          float w[SW];
-#pragma unroll
-          for (int c = 0; c < SW / 4; ++c) {
-            const float4 t = reinterpret_cast<const float4*>(rec)[c];             // broadcast read
-            w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
-          }
+        } else {
 #pragma unroll
           for (int a = 0; a < K; ++a) {
-            float c = w[0] * q[a][0];
-#pragma unroll
-            for (int e = 1; e < NQ; ++e) c = fmaf(w[e], q[a][e], c);
+            const float c = quad_form<NQ>(w, q[a]);
             if (MAP) {
-              if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = c;
+              if (mrow[a] >= 0) P.map[mrow[a] + tag] = c;
             }
-            if (c > best[a]) { best[a] = c; bidx[a] = gs; }
+            best[a] = fmaxf(best[a], c);
           }
         }
-        s += 1 + count;
       }
+#pragma unroll
+      for (int a = 0; a < K; ++a)
+        if (best[a] > seen[a]) { seen[a] = best[a]; bch[a] = ch; }
     }
     __syncthreads();                                   // every warp is done with its tile: reuse it for the reduction
     {
       float* red_c = mytile; int* red_i = reinterpret_cast<int*>(mytile + NP);
 #pragma unroll
-      for (int a = 0; a < K; ++a) { red_c[lane + 32 * a] = best[a]; red_i[lane + 32 * a] = bidx[a]; }
+      for (int a = 0; a < K; ++a) { red_c[lane + 32 * a] = best[a]; red_i[lane + 32 * a] = bch[a]; }
     }
     __syncthreads();
-    // ---- across the warps (first in stream order on exact ties), then tot2 / null2 at the winner (Eq. 10)
+    // ---- across the warps (first in stream order on exact ties), rescan of the winning chunk for the
+    //      direction, then tot2 / null2 there (Eq. 10)
     if (tid < NP) {
       const PairInfo pi = pinfo[tid];
       if (pi.slot >= 0) {
@@ -230,15 +248,38 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
             const int i = reinterpret_cast<const int*>(tiles + wv * kTileWords + NP)[tid];
             if (c > bc) { bc = c; bi = i; }
           }
-          const int4 info = __ldg(P.slot_info + bi);
-          const int rows[3] = {info.x, info.y, info.z};
-          float tot = fmaf(pi.vT.x, pi.vT.x, pi.vT.y * pi.vT.y);
+          const float4* sp = reinterpret_cast<const float4*>(P.stream + (size_t)bi * kSkyChunk * SW);
+          float qq[NQ]; float2 vv[NO];
 #pragma unroll
-          for (int o = 0; o < NO; ++o) {
-            const float2 x = win[(size_t)rows[o] * NPS + tid];
-            tot += fmaf(x.x, x.x, x.y * x.y);
+          for (int e = 0; e < NQ; ++e) qq[e] = 0.f;
+          qq[0] = re_prod(pi.vT, pi.vT);
+          float rb = -2.f, rtot = 0.f, tot = 0.f; int rpix = -1;
+          for (int s = 0; s < kSkyChunk; ++s) {
+            float w[SW];
+#pragma unroll
+            for (int c = 0; c < SW / 4; ++c) {
+              const float4 t = __ldg(sp + s * (SW / 4) + c);
+              w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
+            }
+            const int tag = __float_as_int(w[NQ]);
+            if (tag < 0) {
+              tot = qq[0];
+#pragma unroll
+              for (int o = 0; o < NO; ++o) {
+                const float2 x = win[(size_t)__float_as_int(w[o]) * NPS + tid];
+                vv[o] = x;
+                qq[1 + o] = re_prod(x, x);
+                qq[1 + NO + o] = re_prod(pi.vT, x);
+#pragma unroll
+                for (int o2 = 0; o2 < o; ++o2) qq[1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(vv[o2], x);
+                tot += qq[1 + o];
+              }
+            } else {
+              const float c = quad_form<NQ>(w, qq);
+              if (c > rb) { rb = c; rpix = tag; rtot = tot; }
+            }
           }
-          res.coh2 = bc; res.tot2 = tot; res.null2 = fmaxf(tot - bc, 0.f); res.pix = info.w;
+          res.coh2 = rb; res.tot2 = rtot; res.null2 = fmaxf(rtot - rb, 0.f); res.pix = rpix;
         }
         P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
       }
@@ -269,7 +310,7 @@ using namespace spiir;
 struct spiir_sky_stream {                 // the direction stream of one trigger detector
   int n_chunks = 0, n_tuples = 0, rows = 0, k_max = 0;
   int lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];
-  size_t off_slots = 0, off_info = 0;
+  size_t off_slots = 0;
 };
 
 struct spiir_sky_plan {
@@ -296,16 +337,15 @@ static void sky_layout(spiir_sky_plan* pl) {
   size_t cur = 0;
   for (int T = 0; T < D; ++T) {
     pl->st[T].off_slots = cur; cur = sky_align(cur + (size_t)pl->cap_slots * pl->SW * 4);
-    pl->st[T].off_info = cur;  cur = sky_align(cur + (size_t)pl->cap_slots * 16);
   }
   pl->off_lists = cur;  cur = sky_align(cur + (size_t)D * pl->max_slots * 4);
   pl->off_counts = cur; cur = sky_align(cur + SPIIR_MAX_DET * 4);
   pl->bytes = cur;
 }
 
-// Builds the chunked stream of trigger detector T on the host (slots + per-slot info).
+// Builds the chunked stream of trigger detector T on the host.
 static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const int32_t* delay,
-                             std::vector<float>& slots, std::vector<int32_t>& info) {
+                             std::vector<float>& slots) {
   const int D = pl->n_det, NO = D - 1, NQ = D * (D + 1) / 2, SW = pl->SW, n_pix = pl->n_pix;
   spiir_sky_stream& S = pl->st[T];
   int oth[SPIIR_MAX_DET];
@@ -316,6 +356,7 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
       const int I = oth[o];
       rows[(size_t)p * 3 + o] = S.woff[I] + (delay[(size_t)p * D + I] - delay[(size_t)p * D + T] - S.lo[I]);
     }
+  // directions sorted by delay tuple, then by pixel index
   std::vector<int32_t> order(n_pix);
   for (int p = 0; p < n_pix; ++p) order[p] = p;
   std::sort(order.begin(), order.end(), [&](int32_t x, int32_t y) {
@@ -323,16 +364,15 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
       if (rows[(size_t)x * 3 + o] != rows[(size_t)y * 3 + o]) return rows[(size_t)x * 3 + o] < rows[(size_t)y * 3 + o];
     return x < y;
   });
-  slots.clear(); info.clear();
+  slots.clear();
   int used = 0;                            // slots used in the current chunk
   bool have_prev = false; int32_t prev[3] = {0, 0, 0};
-  auto push_slot = [&]() { slots.resize(slots.size() + SW, 0.f); info.resize(info.size() + 4, 0); ++used; };
-  auto end_chunk = [&]() {
-    if (used == 0 || used == kSkyChunk) { if (used == kSkyChunk) used = 0; have_prev = false; return; }
-    push_slot();
-    const int32_t hw = kSkyEnd << 8;
-    memcpy(&slots[slots.size() - SW + 3], &hw, 4);
-    while (used < kSkyChunk) push_slot();
+  auto push_slot = [&]() -> float* { slots.resize(slots.size() + SW, 0.f); ++used; return &slots[slots.size() - SW]; };
+  auto pad_chunk = [&]() {                 // fill the rest of the chunk with copies of its last direction
+    while (used > 0 && used < kSkyChunk) {
+      float* w = push_slot();
+      memcpy(w, w - SW, (size_t)SW * 4);
+    }
     used = 0; have_prev = false;
   };
   S.n_tuples = 0;
@@ -344,20 +384,20 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
     const int32_t* rw = &rows[(size_t)order[i] * 3];
     int remaining = j - i, at = i;
     while (remaining > 0) {
-      if (used == kSkyChunk) { used = 0; have_prev = false; }
-      if (kSkyChunk - used < 2) end_chunk();
+      if (kSkyChunk - used < 2) pad_chunk();               // a header needs at least one direction after it
       int level = 0;
-      if (have_prev) { while (level < NO && prev[level] == rw[level]) ++level; if (level >= NO) level = NO - 1; }
+      if (have_prev) { while (level < NO - 1 && prev[level] == rw[level]) ++level; }
       const int cnt = std::min(remaining, kSkyChunk - used - 1);
-      push_slot();
       {
-        int32_t h[4] = {rw[0], rw[1], rw[2], cnt | (level << 8)};
-        memcpy(&slots[slots.size() - SW], h, 16);
+        float* w = push_slot();
+        int32_t h[3] = {rw[0], rw[1], rw[2]};
+        memcpy(w, h, (size_t)NO * 4);
+        const int32_t tag = -1 - level;
+        memcpy(w + NQ, &tag, 4);
       }
       for (int c = 0; c < cnt; ++c) {
         const int p = order[at + c];
-        push_slot();
-        float* w = &slots[slots.size() - SW];
+        float* w = push_slot();
         const float* u = u2 + (size_t)p * D * 2;
         auto M = [&](int I, int J) { return (double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]; };
         // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order
@@ -368,15 +408,14 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
           for (int o2 = 0; o2 < o; ++o2) w[1 + 2 * NO + o * (o - 1) / 2 + o2] = (float)(2.0 * M(oth[o2], oth[o]));
         const int32_t pix = p;
         memcpy(w + NQ, &pix, 4);
-        int32_t* inf = &info[info.size() - 4];
-        inf[0] = rw[0]; inf[1] = rw[1]; inf[2] = rw[2]; inf[3] = p;
       }
       prev[0] = rw[0]; prev[1] = rw[1]; prev[2] = rw[2]; have_prev = true;
       remaining -= cnt; at += cnt;
+      if (used == kSkyChunk) { used = 0; have_prev = false; }
     }
     i = j;
   }
-  end_chunk();
+  pad_chunk();
   S.n_chunks = (int)(slots.size() / ((size_t)SW * kSkyChunk));
 }
 
@@ -404,7 +443,7 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
   const int D = n_det;
   pl->ws = (char*)dev_workspace;
   cudaStream_t st = (cudaStream_t)stream;
-  std::vector<float> slots; std::vector<int32_t> info;
+  std::vector<float> slots;
   for (int T = 0; T < D; ++T) {
     spiir_sky_stream& S = pl->st[T];
     int rows = 0;
@@ -427,10 +466,9 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
                 sky_smem_bytes(rows, pl->SW, 1), kSkySmemMax);
       delete pl; return SPIIR_EINVAL;
     }
-    sky_build_stream(pl, T, u2, delay, slots, info);
+    sky_build_stream(pl, T, u2, delay, slots);
     if ((int)(slots.size() / pl->SW) > pl->cap_slots) { set_error("stream of detector %d exceeds its bound", T); delete pl; return SPIIR_EOVERFLOW; }
     cudaError_t e = cudaMemcpyAsync(pl->ws + S.off_slots, slots.data(), slots.size() * 4, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->ws + S.off_info, info.data(), info.size() * 4, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);     // the host images are reused for the next detector
     if (e != cudaSuccess) { set_error("sky plan upload failed: %s", cudaGetErrorString(e)); delete pl; return SPIIR_ECUDA; }
     pl->n_tuples = std::max(pl->n_tuples, S.n_tuples);
@@ -505,7 +543,7 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
     memset(&P, 0, sizeof(P));
     P.stream = (const float*)(pl->ws + S.off_slots); P.n_chunks = S.n_chunks;
     P.chunks_per_warp = (S.n_chunks + kSkyWarps - 1) / kSkyWarps;
-    P.slot_info = (const int4*)(pl->ws + S.off_info); P.n_pix = pl->n_pix;
+    P.n_pix = pl->n_pix;
     P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;
     P.ring_len = view->ring_len; P.k_newest = view->k_newest;
     P.trig = trig; P.list = lists + (size_t)T * pl->max_slots; P.counts = counts; P.T = T;
