@@ -186,14 +186,18 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
       }
+      float4 nxt[SW / 4];
+#pragma unroll
+      for (int c = 0; c < SW / 4; ++c) nxt[c] = reinterpret_cast<const float4*>(mytile)[c];
 #pragma unroll 4
       for (int s = 0; s < kSkyChunk; ++s) {
         float w[SW];
 #pragma unroll
-        for (int c = 0; c < SW / 4; ++c) {
-          const float4 t = reinterpret_cast<const float4*>(mytile + s * SW)[c];   // broadcast read
-          w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
-        }
+        for (int c = 0; c < SW / 4; ++c) { w[4 * c] = nxt[c].x; w[4 * c + 1] = nxt[c].y; w[4 * c + 2] = nxt[c].z; w[4 * c + 3] = nxt[c].w; }
+        // the next slot is fetched (broadcast read) before this one is consumed
+#pragma unroll
+        for (int c = 0; c < SW / 4; ++c)
+          nxt[c] = reinterpret_cast<const float4*>(mytile + ((s + 1) & (kSkyChunk - 1)) * SW)[c];
         const int tag = __float_as_int(w[NQ]);
         if (tag < 0) {
           // new delay tuple: gather the rows that changed, refresh the products they enter
@@ -235,54 +239,61 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       for (int a = 0; a < K; ++a) { red_c[lane + 32 * a] = best[a]; red_i[lane + 32 * a] = bch[a]; }
     }
     __syncthreads();
-    // ---- across the warps (first in stream order on exact ties), rescan of the winning chunk for the
-    //      direction, then tot2 / null2 there (Eq. 10)
-    if (tid < NP) {
-      const PairInfo pi = pinfo[tid];
-      if (pi.slot >= 0) {
-        spiir_sky_result res; res.coh2 = 0.f; res.null2 = 0.f; res.tot2 = 0.f; res.pix = -1;
-        if (pi.valid) {
-          float bc = tiles[tid]; int bi = reinterpret_cast<const int*>(tiles + NP)[tid];
-          for (int wv = 1; wv < kSkyWarps; ++wv) {
-            const float c = tiles[wv * kTileWords + tid];
-            const int i = reinterpret_cast<const int*>(tiles + wv * kTileWords + NP)[tid];
-            if (c > bc) { bc = c; bi = i; }
-          }
-          const float4* sp = reinterpret_cast<const float4*>(P.stream + (size_t)bi * kSkyChunk * SW);
-          float qq[NQ]; float2 vv[NO];
-#pragma unroll
-          for (int e = 0; e < NQ; ++e) qq[e] = 0.f;
-          qq[0] = re_prod(pi.vT, pi.vT);
-          float rb = -2.f, rtot = 0.f, tot = 0.f; int rpix = -1;
-          for (int s = 0; s < kSkyChunk; ++s) {
-            float w[SW];
-#pragma unroll
-            for (int c = 0; c < SW / 4; ++c) {
-              const float4 t = __ldg(sp + s * (SW / 4) + c);
-              w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
-            }
-            const int tag = __float_as_int(w[NQ]);
-            if (tag < 0) {
-              tot = qq[0];
-#pragma unroll
-              for (int o = 0; o < NO; ++o) {
-                const float2 x = win[(size_t)__float_as_int(w[o]) * NPS + tid];
-                vv[o] = x;
-                qq[1 + o] = re_prod(x, x);
-                qq[1 + NO + o] = re_prod(pi.vT, x);
-#pragma unroll
-                for (int o2 = 0; o2 < o; ++o2) qq[1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(vv[o2], x);
-                tot += qq[1 + o];
-              }
-            } else {
-              const float c = quad_form<NQ>(w, qq);
-              if (c > rb) { rb = c; rpix = tag; rtot = tot; }
-            }
-          }
-          res.coh2 = rb; res.tot2 = rtot; res.null2 = fmaxf(rtot - rb, 0.f); res.pix = rpix;
+    // ---- across the warps (first in stream order on exact ties); then a warp rescans the winning chunk
+    //      of one pair, lane = slot: every direction lane refreshes its tuple's products itself, the
+    //      first lane holding the maximum gives the direction, tot2 and null2 there (Eq. 10)
+    for (int j = warp; j < NP; j += kSkyWarps) {
+      const PairInfo pi = pinfo[j];
+      if (pi.slot < 0) continue;
+      spiir_sky_result res; res.coh2 = 0.f; res.null2 = 0.f; res.tot2 = 0.f; res.pix = -1;
+      if (pi.valid) {
+        float bc = -2.f; int bi = 0;
+        if (lane < kSkyWarps) {
+          bc = tiles[lane * kTileWords + j];
+          bi = reinterpret_cast<const int*>(tiles + lane * kTileWords + NP)[j];
         }
-        P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
+        float m = bc;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        const unsigned who = __ballot_sync(0xffffffffu, bc == m);
+        bi = __shfl_sync(0xffffffffu, bi, __ffs(who) - 1);
+        float w[SW];
+        {
+          const float4* sp = reinterpret_cast<const float4*>(P.stream + ((size_t)bi * kSkyChunk + lane) * SW);
+#pragma unroll
+          for (int c = 0; c < SW / 4; ++c) {
+            const float4 t = __ldg(sp + c);
+            w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
+          }
+        }
+        const int tag = __float_as_int(w[NQ]);
+        const unsigned hmask = __ballot_sync(0xffffffffu, tag < 0);
+        const int hl = 31 - __clz((int)(hmask & (0xffffffffu >> (31 - lane))));     // this slot's header (slot 0 is one)
+        float qq[NQ]; float2 vv[NO];
+        qq[0] = re_prod(pi.vT, pi.vT);
+        float tot = qq[0];
+#pragma unroll
+        for (int o = 0; o < NO; ++o) {
+          const int row = __shfl_sync(0xffffffffu, __float_as_int(w[o]), hl);
+          const float2 x = win[(size_t)row * NPS + j];
+          vv[o] = x;
+          qq[1 + o] = re_prod(x, x);
+          qq[1 + NO + o] = re_prod(pi.vT, x);
+#pragma unroll
+          for (int o2 = 0; o2 < o; ++o2) qq[1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(vv[o2], x);
+          tot += qq[1 + o];
+        }
+        const float c = (tag >= 0) ? quad_form<NQ>(w, qq) : -2.f;
+        float cm = c;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) cm = fmaxf(cm, __shfl_xor_sync(0xffffffffu, cm, o));
+        const int src = __ffs(__ballot_sync(0xffffffffu, c == cm)) - 1;
+        res.coh2 = cm;
+        res.tot2 = __shfl_sync(0xffffffffu, tot, src);
+        res.pix = __shfl_sync(0xffffffffu, tag, src);
+        res.null2 = fmaxf(res.tot2 - cm, 0.f);
       }
+      if (lane == 0) P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
     }
   }
 }
