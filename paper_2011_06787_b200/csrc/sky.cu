@@ -40,19 +40,20 @@ constexpr int kSkySmemMax = 227 * 1024;     // opt-in dynamic shared memory per 
 template <int D> struct SkyFmt {
   static constexpr int NO = D - 1;                       // detectors other than the trigger detector
   static constexpr int NQ = D * (D + 1) / 2;             // independent entries of the projector
-  static constexpr int SW = (NQ + 1 + 3) / 4 * 4;        // words per slot: NQ weights + tag, padded to 16 B
+  static constexpr int SW = (NQ + 2 + 3) / 4 * 4;        // words per slot: NQ weights + pixel + control, padded to 16 B
 };
-// Every slot is SW words; word NQ is its tag.
-//   header slot (tag < 0): words 0..NO-1 = window row of other detector o (already offset by its window's
-//               first row); tag = -1 - level, level = first other detector whose row differs from the
-//               previous header of the SAME chunk (0 for a chunk's first header: refresh everything).
-//   direction   (tag >= 0): words [0,NQ) weights, tag = pixel.  Weight order (T = trigger detector, o = others
-//               in increasing detector index): M_TT; M_oo (o = 0..NO-1); 2 M_To; 2 M_o'o for o' < o,
-//               (0,1) (0,2) (1,2).
-// A chunk always starts with a header and is padded at its end with copies of its last direction.
+// One slot per direction, SW words: words [0,NQ) weights, word NQ = pixel, word NQ+1 = control.
+//   Weight order (T = trigger detector, o = others in increasing detector index): M_TT; M_oo (o = 0..NO-1);
+//   2 M_To; 2 M_o'o for o' < o, (0,1) (0,2) (1,2).
+//   control = level | row_0 << 2 | row_1 << 12 | row_2 << 22: row_o = shared-memory window row of other
+//   detector o (already offset by its window's first row, < 1024); level = first other detector whose row
+//   differs from the previous slot of the SAME chunk (0 for a chunk's first slot: refresh everything;
+//   NO: same delay tuple, nothing to refresh).
+// The last chunk is padded with copies of the last direction (level NO).
+constexpr int kSkyRowBits = 10;
 
 struct SkyParams {
-  const float* stream; int32_t n_chunks, chunks_per_warp;     // this trigger detector's stream
+  const float* stream; int32_t n_chunks;                      // this trigger detector's stream
   int32_t n_pix;
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
   const spiir_trigger* trig;
@@ -102,7 +103,8 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
   const long long n_batches = (n_pairs + NP - 1) / NP;
   const int64_t kmin = (P.k_newest - P.ring_len + 1 > 0) ? P.k_newest - P.ring_len + 1 : 0;
   float* mytile = tiles + warp * kTileWords;
-  const int c_beg = min(P.n_chunks, warp * P.chunks_per_warp), c_end = min(P.n_chunks, c_beg + P.chunks_per_warp);
+  // chunks are dealt round-robin to the warps (tuple sizes vary slowly along the stream)
+  const int c_beg = warp, c_end = P.n_chunks;
 
   for (long long batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
     __syncthreads();                                   // previous batch fully consumed
@@ -176,13 +178,13 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
       for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
     }
-    for (int ch = c_beg; ch < c_end; ++ch) {
+    for (int ch = c_beg; ch < c_end; ch += kSkyWarps) {
       __syncwarp();
 #pragma unroll
       for (int c = 0; c < SW / 4; ++c) reinterpret_cast<float4*>(mytile + lane * SW)[c] = pre[c];
       __syncwarp();
-      if (ch + 1 < c_end) {                                   // prefetch the next chunk while this one is consumed
-        const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)(ch + 1) * kSkyChunk + lane) * SW);
+      if (ch + kSkyWarps < c_end) {                           // prefetch the next chunk while this one is consumed
+        const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)(ch + kSkyWarps) * kSkyChunk + lane) * SW);
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
       }
@@ -198,14 +200,15 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c)
           nxt[c] = reinterpret_cast<const float4*>(mytile + ((s + 1) & (kSkyChunk - 1)) * SW)[c];
-        const int tag = __float_as_int(w[NQ]);
-        if (tag < 0) {
+        const int ctrl = __float_as_int(w[NQ + 1]);
+        const int level = ctrl & 3;
+        if (level < NO) {
           // new delay tuple: gather the rows that changed, refresh the products they enter
-          const int level = -1 - tag;
 #pragma unroll
           for (int o = 0; o < NO; ++o) {
             if (level <= o) {
-              const float2* rp = win + (size_t)__float_as_int(w[o]) * NPS + lane;
+              const int row = (ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1);
+              const float2* rp = win + (size_t)row * NPS + lane;
 #pragma unroll
               for (int a = 0; a < K; ++a) {
                 const float2 x = rp[32 * a];
@@ -217,15 +220,14 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
               }
             }
           }
-        } else {
+        }
 #pragma unroll
-          for (int a = 0; a < K; ++a) {
-            const float c = quad_form<NQ>(w, q[a]);
-            if (MAP) {
-              if (mrow[a] >= 0) P.map[mrow[a] + tag] = c;
-            }
-            best[a] = fmaxf(best[a], c);
+        for (int a = 0; a < K; ++a) {
+          const float c = quad_form<NQ>(w, q[a]);
+          if (MAP) {
+            if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = c;
           }
+          best[a] = fmaxf(best[a], c);
         }
       }
 #pragma unroll
@@ -240,7 +242,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     }
     __syncthreads();
     // ---- across the warps (first in stream order on exact ties); then a warp rescans the winning chunk
-    //      of one pair, lane = slot: every direction lane refreshes its tuple's products itself, the
+    //      of one pair, lane = slot: every lane forms its own direction's products from scratch, the
     //      first lane holding the maximum gives the direction, tot2 and null2 there (Eq. 10)
     for (int j = warp; j < NP; j += kSkyWarps) {
       const PairInfo pi = pinfo[j];
@@ -255,8 +257,9 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         float m = bc;
 #pragma unroll
         for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-        const unsigned who = __ballot_sync(0xffffffffu, bc == m);
-        bi = __shfl_sync(0xffffffffu, bi, __ffs(who) - 1);
+        bi = (bc == m) ? bi : INT_MAX;                       // exact ties: the earliest chunk of the stream
+#pragma unroll
+        for (int o = 16; o; o >>= 1) bi = min(bi, __shfl_xor_sync(0xffffffffu, bi, o));
         float w[SW];
         {
           const float4* sp = reinterpret_cast<const float4*>(P.stream + ((size_t)bi * kSkyChunk + lane) * SW);
@@ -266,15 +269,13 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
             w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
           }
         }
-        const int tag = __float_as_int(w[NQ]);
-        const unsigned hmask = __ballot_sync(0xffffffffu, tag < 0);
-        const int hl = 31 - __clz((int)(hmask & (0xffffffffu >> (31 - lane))));     // this slot's header (slot 0 is one)
+        const int ctrl = __float_as_int(w[NQ + 1]);
         float qq[NQ]; float2 vv[NO];
         qq[0] = re_prod(pi.vT, pi.vT);
         float tot = qq[0];
 #pragma unroll
         for (int o = 0; o < NO; ++o) {
-          const int row = __shfl_sync(0xffffffffu, __float_as_int(w[o]), hl);
+          const int row = (ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1);
           const float2 x = win[(size_t)row * NPS + j];
           vv[o] = x;
           qq[1 + o] = re_prod(x, x);
@@ -283,14 +284,14 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
           for (int o2 = 0; o2 < o; ++o2) qq[1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(vv[o2], x);
           tot += qq[1 + o];
         }
-        const float c = (tag >= 0) ? quad_form<NQ>(w, qq) : -2.f;
+        const float c = quad_form<NQ>(w, qq);
         float cm = c;
 #pragma unroll
         for (int o = 16; o; o >>= 1) cm = fmaxf(cm, __shfl_xor_sync(0xffffffffu, cm, o));
         const int src = __ffs(__ballot_sync(0xffffffffu, c == cm)) - 1;
         res.coh2 = cm;
         res.tot2 = __shfl_sync(0xffffffffu, tot, src);
-        res.pix = __shfl_sync(0xffffffffu, tag, src);
+        res.pix = __shfl_sync(0xffffffffu, __float_as_int(w[NQ]), src);
         res.null2 = fmaxf(res.tot2 - cm, 0.f);
       }
       if (lane == 0) P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
@@ -333,7 +334,7 @@ struct spiir_sky_plan {
 };
 
 static size_t sky_align(size_t x) { return (x + 255) / 256 * 256; }
-static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 1 + 3) / 4 * 4; }
+static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 2 + 3) / 4 * 4; }
 static int sky_win_elems(int rows, int K) { return (rows * (32 * K + 1) + 1) & ~1; }
 static size_t sky_smem_bytes(int rows, int SW, int K) {
   const int NP = 32 * K, tile = std::max(kSkyChunk * SW, 2 * NP);
@@ -343,8 +344,7 @@ static size_t sky_smem_bytes(int rows, int SW, int K) {
 static void sky_layout(spiir_sky_plan* pl) {
   const int D = pl->n_det;
   pl->SW = sky_slot_words(D);
-  // a chunk wastes at most one slot and repeats at most one header: slots <= 2 n_pix * 32/30 + a chunk
-  pl->cap_slots = (int)(((size_t)pl->n_pix * 2 * 16 / 15 + 2 * kSkyChunk + kSkyChunk - 1) / kSkyChunk * kSkyChunk);
+  pl->cap_slots = (pl->n_pix + kSkyChunk - 1) / kSkyChunk * kSkyChunk;       // one slot per direction, whole chunks
   size_t cur = 0;
   for (int T = 0; T < D; ++T) {
     pl->st[T].off_slots = cur; cur = sky_align(cur + (size_t)pl->cap_slots * pl->SW * 4);
@@ -375,59 +375,43 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
       if (rows[(size_t)x * 3 + o] != rows[(size_t)y * 3 + o]) return rows[(size_t)x * 3 + o] < rows[(size_t)y * 3 + o];
     return x < y;
   });
-  slots.clear();
-  int used = 0;                            // slots used in the current chunk
-  bool have_prev = false; int32_t prev[3] = {0, 0, 0};
-  auto push_slot = [&]() -> float* { slots.resize(slots.size() + SW, 0.f); ++used; return &slots[slots.size() - SW]; };
-  auto pad_chunk = [&]() {                 // fill the rest of the chunk with copies of its last direction
-    while (used > 0 && used < kSkyChunk) {
-      float* w = push_slot();
-      memcpy(w, w - SW, (size_t)SW * 4);
-    }
-    used = 0; have_prev = false;
-  };
+  slots.assign((size_t)pl->cap_slots * SW, 0.f);
   S.n_tuples = 0;
-  int i = 0;
-  while (i < n_pix) {
-    int j = i + 1;
-    while (j < n_pix && memcmp(&rows[(size_t)order[j] * 3], &rows[(size_t)order[i] * 3], 12) == 0) ++j;
-    ++S.n_tuples;
-    const int32_t* rw = &rows[(size_t)order[i] * 3];
-    int remaining = j - i, at = i;
-    while (remaining > 0) {
-      if (kSkyChunk - used < 2) pad_chunk();               // a header needs at least one direction after it
-      int level = 0;
-      if (have_prev) { while (level < NO - 1 && prev[level] == rw[level]) ++level; }
-      const int cnt = std::min(remaining, kSkyChunk - used - 1);
-      {
-        float* w = push_slot();
-        int32_t h[3] = {rw[0], rw[1], rw[2]};
-        memcpy(w, h, (size_t)NO * 4);
-        const int32_t tag = -1 - level;
-        memcpy(w + NQ, &tag, 4);
-      }
-      for (int c = 0; c < cnt; ++c) {
-        const int p = order[at + c];
-        float* w = push_slot();
-        const float* u = u2 + (size_t)p * D * 2;
-        auto M = [&](int I, int J) { return (double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]; };
-        // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order
-        w[0] = (float)M(T, T);
-        for (int o = 0; o < NO; ++o) w[1 + o] = (float)M(oth[o], oth[o]);
-        for (int o = 0; o < NO; ++o) w[1 + NO + o] = (float)(2.0 * M(T, oth[o]));
-        for (int o = 1; o < NO; ++o)
-          for (int o2 = 0; o2 < o; ++o2) w[1 + 2 * NO + o * (o - 1) / 2 + o2] = (float)(2.0 * M(oth[o2], oth[o]));
-        const int32_t pix = p;
-        memcpy(w + NQ, &pix, 4);
-      }
-      prev[0] = rw[0]; prev[1] = rw[1]; prev[2] = rw[2]; have_prev = true;
-      remaining -= cnt; at += cnt;
-      if (used == kSkyChunk) { used = 0; have_prev = false; }
+  for (int r = 0; r < pl->cap_slots; ++r) {
+    float* w = &slots[(size_t)r * SW];
+    if (r >= n_pix) {                      // padding: the last direction again, nothing to refresh
+      memcpy(w, w - SW, (size_t)SW * 4);
+      int32_t ctrl; memcpy(&ctrl, w + NQ + 1, 4);
+      ctrl = (ctrl & ~3) | NO;
+      memcpy(w + NQ + 1, &ctrl, 4);
+      continue;
     }
-    i = j;
+    const int p = order[r];
+    const int32_t* rw = &rows[(size_t)p * 3];
+    int level = 0;
+    if (r > 0) {
+      const int32_t* pr = &rows[(size_t)order[r - 1] * 3];
+      while (level < NO && pr[level] == rw[level]) ++level;
+      if (level < NO) ++S.n_tuples;
+    } else {
+      ++S.n_tuples;
+    }
+    if (r % kSkyChunk == 0) level = 0;     // chunks are processed independently of each other
+    const float* u = u2 + (size_t)p * D * 2;
+    auto M = [&](int I, int J) { return (double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]; };
+    // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order
+    w[0] = (float)M(T, T);
+    for (int o = 0; o < NO; ++o) w[1 + o] = (float)M(oth[o], oth[o]);
+    for (int o = 0; o < NO; ++o) w[1 + NO + o] = (float)(2.0 * M(T, oth[o]));
+    for (int o = 1; o < NO; ++o)
+      for (int o2 = 0; o2 < o; ++o2) w[1 + 2 * NO + o * (o - 1) / 2 + o2] = (float)(2.0 * M(oth[o2], oth[o]));
+    const int32_t pix = p;
+    memcpy(w + NQ, &pix, 4);
+    int32_t ctrl = level;
+    for (int o = 0; o < NO; ++o) ctrl |= rw[o] << (2 + kSkyRowBits * o);
+    memcpy(w + NQ + 1, &ctrl, 4);
   }
-  pad_chunk();
-  S.n_chunks = (int)(slots.size() / ((size_t)SW * kSkyChunk));
+  S.n_chunks = pl->cap_slots / kSkyChunk;
 }
 
 extern "C" {
@@ -477,8 +461,8 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
                 sky_smem_bytes(rows, pl->SW, 1), kSkySmemMax);
       delete pl; return SPIIR_EINVAL;
     }
+    if (rows >= (1 << kSkyRowBits)) { set_error("delay span of trigger detector %d: %d window rows (>= %d)", T, rows, 1 << kSkyRowBits); delete pl; return SPIIR_EINVAL; }
     sky_build_stream(pl, T, u2, delay, slots);
-    if ((int)(slots.size() / pl->SW) > pl->cap_slots) { set_error("stream of detector %d exceeds its bound", T); delete pl; return SPIIR_EOVERFLOW; }
     cudaError_t e = cudaMemcpyAsync(pl->ws + S.off_slots, slots.data(), slots.size() * 4, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);     // the host images are reused for the next detector
     if (e != cudaSuccess) { set_error("sky plan upload failed: %s", cudaGetErrorString(e)); delete pl; return SPIIR_ECUDA; }
@@ -553,7 +537,6 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
     SkyParams P;
     memset(&P, 0, sizeof(P));
     P.stream = (const float*)(pl->ws + S.off_slots); P.n_chunks = S.n_chunks;
-    P.chunks_per_warp = (S.n_chunks + kSkyWarps - 1) / kSkyWarps;
     P.n_pix = pl->n_pix;
     P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;
     P.ring_len = view->ring_len; P.k_newest = view->k_newest;
