@@ -489,9 +489,7 @@ def len_groups(bk):
     seen = set()
     for b in range(bk.n_bands):
         p = bk.band_plan(b)
-        seen.add((p["lanes_per_unit"], p["filters_per_lane"], 0))
-        if p["n_units_long"]:
-            seen.add((p["lanes_per_unit"], p["filters_per_lane"], 1))
+        seen.add((p["lanes_per_unit"], p["filters_per_lane"]))
     return len(seen)
 
 

@@ -95,7 +95,7 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
 
   // per band: filters of each template
   std::vector<std::vector<int64_t>> ids((size_t)T);
-  std::map<std::tuple<int, int, int>, size_t> group_of;
+  std::map<std::pair<int, int>, size_t> group_of;
   for (int b = 0; b < B; ++b) {
     spiir_bank_host_band& hb = bk->band[b];
     hb = spiir_bank_host_band();
@@ -141,20 +141,24 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
     const size_t slots = (size_t)hb.n_units * cap_unit;
     hb.off_coef = take(slots * sizeof(float4));
     hb.off_off = take(slots * sizeof(int32_t));
-    // launch groups, one per (G, F, class); CTAs listed band by band (heaviest band first)
-    for (int cls = 0; cls < 2; ++cls) {
+    // launch groups, one per (G, F); the long-delay CTAs of a group are listed first (they start first
+    // and overlap the rest instead of forming a tail)
+    for (int cls = 1; cls >= 0; --cls) {
       const int nwu = cls ? hb.n_wu_long : hb.n_wu_short;
       if (!nwu) continue;
-      auto key = std::make_tuple(G, F, cls);
+      auto key = std::make_pair(G, F);
       if (!group_of.count(key)) {
         group_of[key] = bk->groups.size();
-        spiir_launch_group g; g.G = G; g.F = F; g.xg = cls;
+        spiir_launch_group g; g.G = G; g.F = F;
         bk->groups.push_back(g);
       }
       spiir_launch_group& g = bk->groups[group_of[key]];
       const int wu0 = cls ? hb.n_wu_short : 0;
+      std::vector<CtaWork> add;
       for (int w = 0; w < nwu; w += kBankWarps)
-        g.work.push_back(CtaWork{b, wu0 + w, wu0 + std::min(nwu, w + kBankWarps), 0});
+        add.push_back(CtaWork{b, wu0 + w, wu0 + std::min(nwu, w + kBankWarps), cls});
+      if (cls) g.work.insert(g.work.begin(), add.begin(), add.end());
+      else     g.work.insert(g.work.end(), add.begin(), add.end());
       if (!cls) g.smem_bytes = std::max(g.smem_bytes, kReplicas * hb.reps * 4 + 16);
     }
     if (img) {
@@ -382,6 +386,7 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     bd.S_det_stride = (int64_t)hb.n_units * hb.nmax;
     bd.n = n; bd.nmax = hb.nmax; bd.Hcap = hb.Hcap; bd.Hs = hb.Hs; bd.cap = hb.cap; bd.reps = hb.reps;
     bd.nsub = std::min(n, std::min(hb.nmax, kSubChunkMax));
+    bd.odd = (b == 0 && d.out_band == 1) ? 1 : 0;
   }
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   if (bk->timing) {
@@ -398,8 +403,8 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
   SPIIR_CUDA_OK(cudaGetLastError());
   if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[1], st));
   for (auto& g : bk->groups) {
-    int rc = launch_bank_group(g.G, g.F, g.xg, P, (const CtaWork*)(bk->ws + g.off_work), (int)g.work.size(), D,
-                               g.xg ? 0 : g.smem_bytes, st);
+    int rc = launch_bank_group(g.G, g.F, P, (const CtaWork*)(bk->ws + g.off_work), (int)g.work.size(), D,
+                               g.smem_bytes, st);
     if (rc) return rc;
   }
   if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[2], st));

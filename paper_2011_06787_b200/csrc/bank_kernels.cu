@@ -127,6 +127,29 @@ __device__ __forceinline__ float reduce8(float (&s)[8], int lane) {
   return t;
 }
 
+// Same for 4 per-lane values (2 complex samples): after two halving steps and one
+// butterfly lanes g and g^1 both hold element (g >> 1) & 3 summed over their 8-lane group.
+template <int G>
+__device__ __forceinline__ float reduce4(float (&s)[4], int lane) {
+  float w[2], u, t;
+  const bool b4 = lane & 4, b2 = lane & 2;
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const float send = b4 ? s[j] : s[j + 2];
+    const float keep = b4 ? s[j + 2] : s[j];
+    w[j] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+  }
+  {
+    const float send = b2 ? w[0] : w[1];
+    const float keep = b2 ? w[1] : w[0];
+    u = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+  }
+  t = u + __shfl_xor_sync(0xffffffffu, u, 1);
+  if (G >= 16) t += __shfl_xor_sync(0xffffffffu, t, 8);
+  if (G >= 32) t += __shfl_xor_sync(0xffffffffu, t, 16);
+  return t;
+}
+
 template <int F>
 struct FilterRegs {
   float ar[F], ai[F], br[F], bi[F], yr[F], yi[F];
@@ -135,11 +158,54 @@ struct FilterRegs {
 
 // Four consecutive samples of all F filters of this lane; s[] receives the lane's
 // partial sums (re0, im0, re1, im1, ...).  Per update: FMUL + 2 FFMA per component
-// and one FADD per component into the sum = 8 FP32 instructions (12 flop).
-template <int F, bool XG>
-__device__ __forceinline__ void step4(FilterRegs<F>& r, const float* __restrict__ x, int i, float (&s)[8]) {
+// and one FADD per component into the sum = 8 FP32 lane-operations (12 flop,
+// PAPER.md:135).  Filters are taken two at a time so that the FFMAs and FADDs issue
+// as packed FFMA2 / FADD2 (sm_100 f32x2: same FP32-pipe cycles, half the issue
+// slots): per two updates 4 FMUL + 4 FFMA2 + 2 FADD2.  An odd last filter runs scalar.
+// ODD: only samples 1 and 3 of the four enter a sum (a band running at twice the output
+// rate contributes z[m] += s_0[2m+1] only, reading M5); s[] = (re1, im1, re3, im3).
+template <int F, bool XG, bool ODD>
+__device__ __forceinline__ void step4(FilterRegs<F>& r, const float* __restrict__ x, int i, float (&s)[ODD ? 4 : 8]) {
+  float2 sr[4], si[4];                       // (sum over even filters, sum over odd filters)
 #pragma unroll
-  for (int f = 0; f < F; ++f) {
+  for (int f = 0; f + 1 < F; f += 2) {
+    float4 xa, xb;
+    if (XG) {
+      xa = __ldg(reinterpret_cast<const float4*>(x + r.off[f] + i));
+      xb = __ldg(reinterpret_cast<const float4*>(x + r.off[f + 1] + i));
+    } else {
+      xa = *reinterpret_cast<const float4*>(x + r.off[f] + i);
+      xb = *reinterpret_cast<const float4*>(x + r.off[f + 1] + i);
+    }
+    const float xsa[4] = {xa.x, xa.y, xa.z, xa.w}, xsb[4] = {xb.x, xb.y, xb.z, xb.w};
+    const float2 ar = make_float2(r.ar[f], r.ar[f + 1]), ai = make_float2(r.ai[f], r.ai[f + 1]);
+    const float2 nai = make_float2(-r.ai[f], -r.ai[f + 1]);
+    float2 yr = make_float2(r.yr[f], r.yr[f + 1]), yi = make_float2(r.yi[f], r.yi[f + 1]);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const float2 pr = make_float2(r.br[f] * xsa[q], r.br[f + 1] * xsb[q]);
+      const float2 pi = make_float2(r.bi[f] * xsa[q], r.bi[f + 1] * xsb[q]);
+      const float2 tr = __ffma2_rn(nai, yi, pr);
+      const float2 ti = __ffma2_rn(ai, yr, pi);
+      const float2 nr = __ffma2_rn(ar, yr, tr);
+      const float2 ni = __ffma2_rn(ar, yi, ti);
+      yr = nr; yi = ni;
+      if (!ODD || (q & 1)) {
+        if (f == 0) { sr[q] = yr; si[q] = yi; }
+        else        { sr[q] = __fadd2_rn(sr[q], yr); si[q] = __fadd2_rn(si[q], yi); }
+      }
+    }
+    r.yr[f] = yr.x; r.yr[f + 1] = yr.y; r.yi[f] = yi.x; r.yi[f + 1] = yi.y;
+  }
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    if (ODD && !(q & 1)) continue;
+    const int o = ODD ? (q >> 1) : q;
+    s[2 * o] = (F > 1) ? sr[q].x + sr[q].y : 0.f;
+    s[2 * o + 1] = (F > 1) ? si[q].x + si[q].y : 0.f;
+  }
+  if (F & 1) {
+    constexpr int f = F - 1;
     float4 xv;
     if (XG) xv = __ldg(reinterpret_cast<const float4*>(x + r.off[f] + i));
     else    xv = *reinterpret_cast<const float4*>(x + r.off[f] + i);
@@ -152,14 +218,35 @@ __device__ __forceinline__ void step4(FilterRegs<F>& r, const float* __restrict_
       const float nr = fmaf(r.ar[f], yr, tr);
       const float ni = fmaf(r.ar[f], yi, ti);
       yr = nr; yi = ni;
-      if (f == 0) { s[2 * q] = yr; s[2 * q + 1] = yi; }
-      else        { s[2 * q] += yr; s[2 * q + 1] += yi; }
+      if (!ODD || (q & 1)) {
+        const int o = ODD ? (q >> 1) : q;
+        s[2 * o] += yr; s[2 * o + 1] += yi;
+      }
     }
     r.yr[f] = yr; r.yi[f] = yi;
   }
 }
 
-template <int G, int F, bool XG>
+// One sub-chunk of `len` samples for this lane's filters: recursion, unit sums, store.
+template <int G, int F, bool XG, bool ODD>
+__device__ __forceinline__ void run_samples(FilterRegs<F>& r, const float* __restrict__ x, int len, float* __restrict__ So,
+                                            int lane, int g) {
+  for (int i = 0; i < len; i += 4) {
+    if (ODD) {
+      float s[4];
+      step4<F, XG, true>(r, x, i, s);
+      const float t = reduce4<G>(s, lane);
+      if (g < 8 && !(g & 1)) So[i + (g >> 1)] = t;          // 2 complex samples per 4 inputs
+    } else {
+      float s[8];
+      step4<F, XG, false>(r, x, i, s);
+      const float t = reduce8<G>(s, lane);
+      if (g < 8) So[2 * i + g] = t;
+    }
+  }
+}
+
+template <int G, int F>
 __global__ void __launch_bounds__(kBankThreads, 2)
 k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
   extern __shared__ __align__(128) float xs[];
@@ -169,6 +256,7 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int wu = w.wu_begin + warp;
   const bool active = wu < w.wu_end;
+  const bool odd = B.odd != 0;                       // CTA-uniform
 
   FilterRegs<F> r;
   const size_t slot0 = ((size_t)wu * F) * 32 + lane;
@@ -189,16 +277,13 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
   float* Sout = reinterpret_cast<float*>(B.S + (size_t)det * B.S_det_stride + (size_t)unit * B.nmax);
   const int n = B.n;
 
-  if (XG) {
-    // long-delay units: read the replicas straight from global memory (L1/L2 resident)
+  if (w.xg) {
+    // long-delay units (same launch, listed first): the replicas are read straight from
+    // global memory (L1/L2 resident)
     if (active) {
       const float* x = B.xrep + (size_t)det * B.x_det_stride;
-      for (int i = 0; i < n; i += 4) {
-        float s[8];
-        step4<F, true>(r, x, i, s);
-        const float t = reduce8<G>(s, lane);
-        if (g < 8) Sout[2 * i + g] = t;
-      }
+      if (odd) run_samples<G, F, true, true>(r, x, n, Sout, lane, g);
+      else     run_samples<G, F, true, false>(r, x, n, Sout, lane, g);
     }
   } else {
     uint64_t* bar = reinterpret_cast<uint64_t*>(xs + kReplicas * B.reps);
@@ -219,13 +304,8 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
       mbar_wait(bar, phase);
       phase ^= 1u;
       if (active) {
-        float* So = Sout + 2 * m0;
-        for (int i = 0; i < len; i += 4) {
-          float s[8];
-          step4<F, false>(r, xs, i, s);
-          const float t = reduce8<G>(s, lane);
-          if (g < 8) So[2 * i + g] = t;
-        }
+        if (odd) run_samples<G, F, false, true>(r, xs, len, Sout + m0, lane, g);
+        else     run_samples<G, F, false, false>(r, xs, len, Sout + 2 * m0, lane, g);
       }
     }
   }
@@ -235,44 +315,38 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
   }
 }
 
-template <int G, int F, bool XG>
+template <int G, int F>
 static int launch_one(const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det, int smem, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_bank<G, F, XG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_bank<G, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     configured = true;
   }
-  k_bank<G, F, XG><<<dim3(n_cta, n_det), kBankThreads, smem, st>>>(P, dev_work);
+  k_bank<G, F><<<dim3(n_cta, n_det), kBankThreads, smem, st>>>(P, dev_work);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());
   return SPIIR_OK;
 }
 
-#define SPIIR_F_CASES(G, XG)                                                          \
-  switch (F) {                                                                        \
-    case 4:  return launch_one<G, 4, XG>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 5:  return launch_one<G, 5, XG>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 6:  return launch_one<G, 6, XG>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 7:  return launch_one<G, 7, XG>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 8:  return launch_one<G, 8, XG>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 9:  return launch_one<G, 9, XG>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 10: return launch_one<G, 10, XG>(P, dev_work, n_cta, n_det, smem, st);       \
-    case 11: return launch_one<G, 11, XG>(P, dev_work, n_cta, n_det, smem, st);       \
-    case 12: return launch_one<G, 12, XG>(P, dev_work, n_cta, n_det, smem, st);       \
-    default: break;                                                                   \
+#define SPIIR_F_CASES(G)                                                          \
+  switch (F) {                                                                    \
+    case 4:  return launch_one<G, 4>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 5:  return launch_one<G, 5>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 6:  return launch_one<G, 6>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 7:  return launch_one<G, 7>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 8:  return launch_one<G, 8>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 9:  return launch_one<G, 9>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 10: return launch_one<G, 10>(P, dev_work, n_cta, n_det, smem, st);       \
+    case 11: return launch_one<G, 11>(P, dev_work, n_cta, n_det, smem, st);       \
+    case 12: return launch_one<G, 12>(P, dev_work, n_cta, n_det, smem, st);       \
+    default: break;                                                               \
   }
 
-int launch_bank_group(int G, int F, int xg, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
+int launch_bank_group(int G, int F, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
                       int smem, cudaStream_t st) {
-  if (!xg) {
-    if (G == 8) { SPIIR_F_CASES(8, false) }
-    else if (G == 16) { SPIIR_F_CASES(16, false) }
-    else if (G == 32) { SPIIR_F_CASES(32, false) }
-  } else {
-    if (G == 8) { SPIIR_F_CASES(8, true) }
-    else if (G == 16) { SPIIR_F_CASES(16, true) }
-    else if (G == 32) { SPIIR_F_CASES(32, true) }
-  }
+  if (G == 8) { SPIIR_F_CASES(8) }
+  else if (G == 16) { SPIIR_F_CASES(16) }
+  else if (G == 32) { SPIIR_F_CASES(32) }
   set_error("no kernel instance for G=%d F=%d", G, F);
   return SPIIR_EINVAL;
 }
@@ -340,7 +414,7 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
   for (int m = tid; m < n_out; m += kCombineThreads) {
     float2 z = acc[m];
     if (ob == 1) {                                             // band 0 runs at twice the output rate (M5)
-      const float2 v = unit_sum(S0, p.nmax[0], first0, count0, 2 * m + 1);
+      const float2 v = unit_sum(S0, p.nmax[0], first0, count0, m);   // k_bank stored s_0[2m+1] at index m
       z.x += v.x; z.y += v.y;
     }
     ring[(p.k0 + m) % p.ring_len] = z;

@@ -54,13 +54,14 @@ struct BandDev {
   int32_t cap;            // floats per replica in global memory
   int32_t reps;           // floats per replica in shared memory ( = Hs + sub-chunk capacity )
   int32_t nsub;           // sub-chunk length for this call
+  int32_t odd;            // 1: only odd samples are summed and stored, S[..][m] = s[2m+1] (band above the output rate)
 };
 
 struct BankParams {
   BandDev band[SPIIR_MAX_BANDS];
 };
 
-struct CtaWork { int32_t band, wu_begin, wu_end, _pad; };
+struct CtaWork { int32_t band, wu_begin, wu_end, xg; };   // xg: long-delay units, input read from global memory
 
 // Kernel parameter blocks (bank_kernels.cu), filled by the host code in bank.cu.
 struct PrepParams {
@@ -92,7 +93,7 @@ struct CombineParams {
 };
 
 void launch_prep(const PrepParams& p, int n_det, cudaStream_t st);
-int launch_bank_group(int G, int F, int xg, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
+int launch_bank_group(int G, int F, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
                       int smem, cudaStream_t st);
 void launch_combine(const CombineParams& p, int n_det, cudaStream_t st);
 
@@ -122,7 +123,7 @@ struct spiir_bank_host_band {
 };
 
 struct spiir_launch_group {
-  int G, F, xg;
+  int G, F;
   std::vector<spiir::CtaWork> work;
   size_t off_work = 0;
   int smem_bytes = 0;
