@@ -427,8 +427,15 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
   cp.k0 = bk->k_next;
   cp.peak = (PeakRec*)(bk->ws + bk->off_peak);
   cp.B = B; cp.out_band = d.out_band; cp.T = T;
-  cp.bufA = kUpHist + (d.max_chunk_samples >> d.out_band);
-  cp.bufB = (B - 1 > d.out_band) ? kUpHist + (d.max_chunk_samples >> (d.out_band + 1)) : 0;
+  cp.bufA = (kUpHist + (d.max_chunk_samples >> d.out_band) + 4) & ~1;   // even, and room for the 17-sample window reads
+  cp.bufB = (B - 1 > d.out_band) ? (kUpHist + (d.max_chunk_samples >> (d.out_band + 1)) + 4) & ~1 : 0;
+  cp.sb_total = 0;
+  for (int b = 0; b < B; ++b) {
+    const int n = n_samples >> b;
+    cp.sb_n[b] = (b == 0 && d.out_band == 1) ? n / 2 : n;
+    cp.sb_off[b] = cp.sb_total;
+    cp.sb_total += (cp.sb_n[b] + 1) & ~1;
+  }
   launch_combine(cp, D, st);
   SPIIR_CUDA_OK(cudaGetLastError());
   if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[3], st));

@@ -364,39 +364,74 @@ __device__ __forceinline__ float2 unit_sum(const float2* __restrict__ S, int nma
   return a;
 }
 
+__device__ __forceinline__ void cp_async_16(void* dst_smem, const void* src_gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+
 __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_constant__ CombineParams p) {
   extern __shared__ __align__(16) float2 cbuf[];
-  __shared__ float h[SPIIR_FIR_TAPS];
   __shared__ float red_m2[kCombineThreads / 32];
   __shared__ int red_k[kCombineThreads / 32];
   const int t = blockIdx.x, det = blockIdx.y, tid = threadIdx.x;
-  if (tid < SPIIR_FIR_TAPS) h[tid] = p.taps_int[tid];
-  float2* buf[2] = {cbuf, cbuf + p.bufA};
+  float hr[SPIIR_FIR_TAPS];                            // interpolation taps, in registers
+#pragma unroll
+  for (int j = 0; j < SPIIR_FIR_TAPS; ++j) hr[j] = __ldg(p.taps_int + j);
+  float2* buf[2] = {cbuf, cbuf + p.bufA};              // bufA, bufB even: 16-byte aligned windows
+  float2* sbuf = cbuf + ((p.bufA + p.bufB + 1) & ~1);   // the template's band sums of this chunk, all bands (16-byte aligned)
   const int B = p.B, ob = p.out_band;
+
+  // stage every band's sums at once (one round of HBM latency for the whole template): a template with
+  // one unit in a band is copied asynchronously, more units are added up on the way
+  for (int b = 0; b < B; ++b) {
+    const int ns = p.sb_n[b];                           // samples k_bank stored for this band (n, or n/2 if odd-only)
+    const float2* S = p.S[b] + (size_t)det * p.S_det_stride[b];
+    const int first = p.tb_first[t * B + b], count = p.tb_count[t * B + b];
+    float2* dst = sbuf + p.sb_off[b];
+    if (count == 1) {
+      const float2* row = S + (size_t)first * p.nmax[b];
+      for (int j = tid; j < ns / 2; j += kCombineThreads) cp_async_16(dst + 2 * j, row + 2 * j);
+    } else {
+      for (int m = tid; m < ns; m += kCombineThreads) dst[m] = unit_sum(S, p.nmax[b], first, count, m);
+    }
+  }
+  asm volatile("cp.async.wait_all;" ::: "memory");
+  __syncthreads();
 
   // acc_{B-1} = s_{B-1}, then acc_b = s_b + up2(acc_{b+1}) down to the output band
   for (int b = B - 1; b >= ob; --b) {
     float2* cur = buf[(b - ob) & 1];
     const int n = p.n[b];
-    const float2* S = p.S[b] + (size_t)det * p.S_det_stride[b];
-    const int first = p.tb_first[t * B + b], count = p.tb_count[t * B + b];
+    const float2* sb = sbuf + p.sb_off[b];
     float2* hist = (b > ob) ? p.uphist[b] + ((size_t)det * p.T + t) * kUpHist : nullptr;
     if (hist && tid < kUpHist) cur[tid] = hist[tid];
     if (b == B - 1) {
-      for (int m = tid; m < n; m += kCombineThreads) cur[kUpHist + m] = unit_sum(S, p.nmax[b], first, count, m);
+      for (int m = tid; m < n; m += kCombineThreads) cur[kUpHist + m] = sb[m];
     } else {
+      // four outputs per thread from one 17-sample window of acc_{b+1} held in registers:
+      // m = 2j, 2j+1 share the window ending at acc[j], m = 2j+2, 2j+3 the one ending at acc[j+1]
       const float2* src = buf[(b + 1 - ob) & 1];
-      for (int m = tid; m < n; m += kCombineThreads) {
-        float2 a = unit_sum(S, p.nmax[b], first, count, m);
-        const int par = m & 1, c = kUpHist + (m >> 1);
+      for (int j0 = 2 * tid; 2 * j0 < n; j0 += 2 * kCombineThreads) {
+        float2 w[18];
+#pragma unroll
+        for (int i = 0; i < 9; ++i) {
+          const float4 v = *reinterpret_cast<const float4*>(src + j0 + 2 * i);     // src[j0 + i] = acc[j0 + i - 15]
+          w[2 * i] = make_float2(v.x, v.y); w[2 * i + 1] = make_float2(v.z, v.w);
+        }
+        const float4 s01 = *reinterpret_cast<const float4*>(sb + 2 * j0);
+        const float4 s23 = *reinterpret_cast<const float4*>(sb + 2 * j0 + 2);
+        float2 a0 = make_float2(s01.x, s01.y), a1 = make_float2(s01.z, s01.w);
+        float2 a2 = make_float2(s23.x, s23.y), a3 = make_float2(s23.z, s23.w);
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
-          const float hv = h[2 * q + par];
-          const float2 v = src[c - q];
-          a.x = fmaf(hv, v.x, a.x);
-          a.y = fmaf(hv, v.y, a.y);
+          const float2 he = make_float2(hr[2 * q], hr[2 * q]), ho = make_float2(hr[2 * q + 1], hr[2 * q + 1]);
+          const float2 u = w[15 - q], v = w[16 - q];
+          a0 = __ffma2_rn(he, u, a0);                       // packed (re, im): half the issue slots
+          a1 = __ffma2_rn(ho, u, a1);
+          a2 = __ffma2_rn(he, v, a2);
+          a3 = __ffma2_rn(ho, v, a3);
         }
-        cur[kUpHist + m] = a;
+        float2* o = cur + kUpHist + 2 * j0;
+        o[0] = a0; o[1] = a1; o[2] = a2; o[3] = a3;
       }
     }
     __syncthreads();
@@ -406,18 +441,20 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
   // output samples, ring append, fused per-template maximum (H4 mode 0)
   const float2* acc = buf[0] + kUpHist;
   const int n_out = p.n_out;
-  const float2* S0 = (ob == 1) ? p.S[0] + (size_t)det * p.S_det_stride[0] : nullptr;
-  const int first0 = (ob == 1) ? p.tb_first[t * B] : 0, count0 = (ob == 1) ? p.tb_count[t * B] : 0;
+  const float2* s0 = sbuf + p.sb_off[0];                        // ob == 1: s_0[2m+1] stored at index m
   float2* ring = p.ring + (size_t)det * p.ring_det_stride + (size_t)t * p.ring_len;
   float2* out = p.snr_out ? p.snr_out + ((size_t)det * p.T + t) * n_out : nullptr;
   float best = -1.f; int bk = 0; float2 bz = make_float2(0.f, 0.f);
+  const long long kbase = p.k0 % p.ring_len;           // n_out <= ring_len: one conditional wrap per sample
   for (int m = tid; m < n_out; m += kCombineThreads) {
     float2 z = acc[m];
     if (ob == 1) {                                             // band 0 runs at twice the output rate (M5)
-      const float2 v = unit_sum(S0, p.nmax[0], first0, count0, m);   // k_bank stored s_0[2m+1] at index m
+      const float2 v = s0[m];
       z.x += v.x; z.y += v.y;
     }
-    ring[(p.k0 + m) % p.ring_len] = z;
+    long long kk = kbase + m;
+    if (kk >= p.ring_len) kk -= p.ring_len;
+    ring[kk] = z;
     if (out) out[m] = z;
     const float m2 = __fadd_rn(__fmul_rn(z.x, z.x), __fmul_rn(z.y, z.y));
     if (m2 > best) { best = m2; bk = m; bz = z; }
@@ -445,10 +482,10 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
 void launch_combine(const CombineParams& p, int n_det, cudaStream_t st) {
   static bool configured = false;
   if (!configured) {
-    cudaFuncSetAttribute(k_combine, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    cudaFuncSetAttribute(k_combine, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     configured = true;
   }
-  const size_t smem = (size_t)(p.bufA + p.bufB) * sizeof(float2);
+  const size_t smem = (size_t)(((p.bufA + p.bufB + 1) & ~1) + p.sb_total) * sizeof(float2);
   k_combine<<<dim3(p.T, n_det), kCombineThreads, smem, st>>>(p);
   count_launch();
 }

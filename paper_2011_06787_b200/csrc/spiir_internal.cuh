@@ -90,6 +90,7 @@ struct CombineParams {
   PeakRec* peak;                        // [det][T]
   int32_t B, out_band, T;
   int32_t bufA, bufB;                   // capacities in float2 (incl. history prefix)
+  int32_t sb_off[SPIIR_MAX_BANDS], sb_n[SPIIR_MAX_BANDS], sb_total;   // staged band sums in shared memory (float2)
 };
 
 void launch_prep(const PrepParams& p, int n_det, cudaStream_t st);
