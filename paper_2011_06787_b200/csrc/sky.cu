@@ -158,7 +158,8 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     //      (one FMNMX); which chunk raised it last is noted per chunk, and that chunk is rescanned below.
     float2 vT[K], v[NO][K];
     float best[K], seen[K]; int bch[K];
-    float q[K][NQ];
+    float2 qp[(K + 1) / 2][NQ];                          // products of pairs (2i, 2i+1) side by side: packed FFMA2 operands
+#define SKY_Q(a, e) (((a) & 1) ? qp[(a) >> 1][e].y : qp[(a) >> 1][e].x)
     long long mrow[K];                                  // sky-map row of each pair, -1 = none
 #pragma unroll
     for (int a = 0; a < K; ++a) {
@@ -166,8 +167,8 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       vT[a] = pi.vT; best[a] = -1.f; seen[a] = -1.f; bch[a] = c_beg;
       mrow[a] = (MAP && pi.valid) ? (long long)pi.slot * P.n_pix : -1;
 #pragma unroll
-      for (int e = 0; e < NQ; ++e) q[a][e] = 0.f;
-      q[a][0] = re_prod(vT[a], vT[a]);
+      for (int e = 0; e < NQ; ++e) SKY_Q(a, e) = 0.f;
+      SKY_Q(a, 0) = re_prod(vT[a], vT[a]);
 #pragma unroll
       for (int o = 0; o < NO; ++o) v[o][a] = make_float2(0.f, 0.f);
     }
@@ -213,23 +214,39 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
               for (int a = 0; a < K; ++a) {
                 const float2 x = rp[32 * a];
                 v[o][a] = x;
-                q[a][1 + o] = re_prod(x, x);
-                q[a][1 + NO + o] = re_prod(vT[a], x);
+                SKY_Q(a, 1 + o) = re_prod(x, x);
+                SKY_Q(a, 1 + NO + o) = re_prod(vT[a], x);
 #pragma unroll
-                for (int o2 = 0; o2 < o; ++o2) q[a][1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(v[o2][a], x);
+                for (int o2 = 0; o2 < o; ++o2) SKY_Q(a, 1 + 2 * NO + o * (o - 1) / 2 + o2) = re_prod(v[o2][a], x);
               }
             }
           }
         }
+        // the quadratic form of two pairs at a time: scalar weight x packed products (FFMA2, the same
+        // per-component roundings as quad_form in the rescan)
+        float cval[K];
+#pragma unroll
+        for (int i = 0; i < K / 2; ++i) {
+          float2 c2 = __fmul2_rn(make_float2(w[0], w[0]), qp[i][0]);
+#pragma unroll
+          for (int e = 1; e < NQ; ++e) c2 = __ffma2_rn(make_float2(w[e], w[e]), qp[i][e], c2);
+          cval[2 * i] = c2.x; cval[2 * i + 1] = c2.y;
+        }
+        if (K & 1) {
+          float c = __fmul_rn(w[0], qp[K / 2][0].x);
+#pragma unroll
+          for (int e = 1; e < NQ; ++e) c = __fmaf_rn(w[e], qp[K / 2][e].x, c);
+          cval[K - 1] = c;
+        }
 #pragma unroll
         for (int a = 0; a < K; ++a) {
-          const float c = quad_form<NQ>(w, q[a]);
           if (MAP) {
-            if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = c;
+            if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = cval[a];
           }
-          best[a] = fmaxf(best[a], c);
+          best[a] = fmaxf(best[a], cval[a]);
         }
       }
+#undef SKY_Q
 #pragma unroll
       for (int a = 0; a < K; ++a)
         if (best[a] > seen[a]) { seen[a] = best[a]; bch[a] = ch; }
