@@ -43,7 +43,7 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 FP32_LANE_OPS_PER_S = 148 * 128 * 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/); None until a capture exists for the kernel.
-NCU_TRAFFIC_BYTES = {"k_bank": None, "k_sky": None}
+NCU_TRAFFIC_BYTES = {"k_bank": 4.43e9, "k_sky": 2.19e9}   # profiles/r1_ncu_summary.md sections 3 and 2 (mean of the three slide launches)
 
 
 def parse_args():
@@ -449,7 +449,7 @@ def run_ours(args):
     if has_sky and evals:
         roof_sky = alu_roofline("k_sky (coherent search + slides, H5+H6)", FLOP_PER_EVAL * evals, ms_sky,
                                 2 * D * K if S else D * K, ffma_rate, NCU_TRAFFIC_BYTES["k_sky"],
-                                issue_ops=9.0 * evals)
+                                issue_ops=7.0 * evals)
     dominant, other = (roof_bank, roof_sky) if (roof_sky is None or ms_rec >= ms_sky) else (roof_sky, roof_bank)
     line = {
         "metric": METRIC, "value": upd_all / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
@@ -468,7 +468,7 @@ def run_ours(args):
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:
-        s = oracle_sample(args, min(256, T), 2, 16 if has_sky else 0)
+        s = oracle_sample(args, min(4096, T), 2, 1024 if has_sky else 0)
         cpu_v, cpu_t = oracle_whole_step_rate(s, upd_chunk, evals / K if has_sky else 0, n_slots)
         line["cpu_baseline"] = {
             "value": cpu_v, "unit": UNIT, "cores": s["threads"], "kind": "oracle",
