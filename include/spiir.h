@@ -172,8 +172,9 @@ int spiir_sky_plan_free(spiir_sky_plan* plan);
 int32_t spiir_sky_plan_tuples(const spiir_sky_plan* plan);
 
 /* Result of one (trigger[, slide]) search: the maximum over directions of the
- * coherent SNR^2 (Eq. 9), the pixel where it occurs (lowest index on exact
- * ties), and tot2 = sum_I |z_I|^2, null2 = max(tot2 - coh2, 0) (Eq. 10) there.
+ * coherent SNR^2 (Eq. 9), the pixel where it occurs (on exact ties the first
+ * direction in the plan's order: delay tuples in increasing order, pixel index
+ * ascending within a tuple), and tot2 = sum_I |z_I|^2, null2 = max(tot2 - coh2, 0) (Eq. 10) there.
  * pix = -1 (and zeros) if the slot is invalid or any gather of the search would
  * leave the valid range of the view. */
 typedef struct { float coh2, null2, tot2; int32_t pix; } spiir_sky_result;
