@@ -307,3 +307,109 @@ def test_cfg1_sample_chain(sp, U):
     U.check_snr(z, z_ref)
     # the injection (network SNR 15) is the loudest coherent candidate, found by template 0
     assert best[1][0] == 0 and math.sqrt(best[0]) > 10.0
+
+
+# ------------------------------------------------------------------ config 4 at FULL size, sampled outputs
+def test_cfg4_full_size_sampled(sp, U):
+    """BASELINE.json config 4 in the launch configuration bench.py times (20 000 templates x 700
+    filters, 8 bands, 3 detectors: k_bank grid 5005 x 3, k_combine 20000 x 3, k_sky on 60 000 slots at
+    nside 32), three 1-s chunks.  The oracle cannot run 14 M filters, so outputs are SAMPLED: the SNR
+    series of 16 templates (3 chirp-matched long-delay ones, the first / last random ones, 11 seeded)
+    against the float64 oracle of exactly those templates (templates are independent), every peak of
+    the last chunk stage-isolated against O4 on the GPU's own z, and the sky search / one time slide of
+    the sampled templates' candidates against O6 / O7 (one-chunk lag, A13)."""
+    import torch
+    cfg = workloads.config(4)
+    T, D, NC = cfg["n_templates"], 3, 3
+    THR = 1.5          # the stream is 3 s old: the low-rate bands are still filling, threshold 4 would give ~no candidates
+    bank = workloads.bank_for_config(4)
+    st = workloads.strain_for_config(4, seconds=NC)
+    x = st["strain"]
+    dec, itp = workloads.halfband_taps()
+    rng = np.random.default_rng(4)
+    sel = np.unique(np.concatenate([[0, 7, 19, 20, T - 1], rng.integers(21, T - 1, 11)])).astype(np.int64)
+    z_ref = oracle.filter_bank(x, bank, dec, itp, templates=sel)             # [D][n_sel][NC*2048]
+    ring = 4 * 2048
+    bk = sp.Bank(bank, D, 4096, ring_len=ring, bank_size=1000, dec_taps=dec, int_taps=itp)
+    assert bk.band_plan(1)["n_units_long"] > 0                               # the long-delay class is exercised
+    xs = torch.from_numpy(x).cuda()
+    out = torch.empty(D, T, 2048, 2, dtype=torch.float32, device="cuda")
+    z_sel = np.zeros((D, len(sel), NC * 2048), np.complex64)
+    trig_prev = None
+    sel_dev = torch.from_numpy(sel).cuda()
+    for c in range(NC):
+        bk.filter_chunk(xs[:, c * 4096:(c + 1) * 4096].contiguous(), out)
+        z_sel[:, :, c * 2048:(c + 1) * 2048] = out[:, sel_dev].cpu().numpy().view(np.complex64)[..., 0]
+        tr, cnt = bk.peaks(THR, 0)
+        torch.cuda.synchronize()
+        if c == NC - 2:
+            trig_prev = (tr.clone(), sp.triggers_to_numpy(tr).copy())
+    U.check_snr(z_sel, z_ref)
+    # every peak of the last chunk, bit-exact against O4 on the GPU's own float32 z
+    z_last = out.cpu().numpy().view(np.complex64)[..., 0]
+    trig = sp.triggers_to_numpy(tr)
+    k_iso, v_iso = oracle.peaks_mode0(z_last.reshape(D * T, 2048), THR)
+    assert np.array_equal(trig["k"] - (NC - 1) * 2048, k_iso) and np.array_equal(trig["valid"], v_iso)
+    assert int(cnt.cpu()[0]) == int(v_iso.sum()) and v_iso.sum() > 0.2 * D * T
+    # end to end on the sampled templates (near-tie rule A12)
+    rows = (np.arange(D)[:, None] * T + sel[None, :]).reshape(-1)
+    U.check_peaks_mode0(_subset_trig(trig[rows], sel, D), z_sel[:, :, -2048:], z_ref[:, :, -2048:],
+                        (NC - 1) * 2048, THR)
+    # sky search + one slide over all 60 000 slots; compare the sampled templates' candidates
+    u2, delay = _table(cfg, gmst=st["gmst"])
+    plan = sp.SkyPlan(u2, delay, max_slots=D * T)
+    view = bk.snr_view()
+    fg = sp.results_to_numpy(plan.search(view, trig_prev[0], D * T))
+    bg = sp.results_to_numpy(plan.background(view, trig_prev[0], D * T, 1, 2048, [1, 1, 1]))
+    torch.cuda.synchronize()
+    tp = trig_prev[1]
+    assert np.all((fg["pix"] >= 0) == (tp["valid"] == 1))                    # every candidate searched, nothing else
+    assert np.all(bg["pix"][tp["valid"] == 0] == -1)                         # (a slide may leave the stream's start)
+    k_newest = NC * 2048 - 1
+    zr = np.zeros((D, len(sel), ring), np.complex64)
+    zr[:, :, :NC * 2048] = z_sel                                             # ring index = k (k < ring_len)
+    sub = _subset_trig(tp[rows], sel, D)
+    assert sub["valid"].sum() >= 8
+    U.check_sky(fg[rows], zr, ring, k_newest, u2, delay, sub)
+    U.check_sky(bg[rows], zr, ring, k_newest, u2, delay, sub, n_slides=1, step=2048, mult=[1, 1, 1])
+
+
+def _subset_trig(trig_rows, sel, D):
+    """Trigger slots of the selected templates with `tmpl` renumbered to rows of the sampled view."""
+    t = trig_rows.copy()
+    t["tmpl"] = np.tile(np.arange(len(sel)), D)
+    return t
+
+
+# ------------------------------------------------------------------ degenerate inputs
+def test_sky_degenerate_inputs(sp, U):
+    """No slots, no valid slot, and an all-zero SNR view (every direction ties exactly)."""
+    import torch
+    cfg = workloads.config(1)
+    u2, delay = _table(cfg, nside=4, gmst=0.3)
+    plan = sp.SkyPlan(u2, delay, max_slots=16)
+    L = 400
+    zd = torch.zeros(3, 16, L, 2, dtype=torch.float32, device="cuda")
+    view = sp.SnrView(zd)
+    trig = np.zeros(16, sp.TRIGGER_DTYPE)
+    trig["tmpl"] = np.arange(16); trig["det"] = np.arange(16) % 3; trig["k"] = 200
+    td = sp.triggers_from_numpy(trig)
+    # n_slots = 0: nothing is launched, nothing is written
+    sentinel = torch.full((16, 16), 7, dtype=torch.uint8, device="cuda")
+    plan.search(view, td, 0, out=sentinel)
+    torch.cuda.synchronize()
+    assert int(sentinel.min()) == 7
+    # no valid slot: every result is "none", for the foreground and for every slide
+    res = sp.results_to_numpy(plan.search(view, td, 16))
+    bg = sp.results_to_numpy(plan.background(view, td, 16, 3, 50, [1, 1, 1]))
+    torch.cuda.synchronize()
+    for r in (res, bg):
+        assert np.all(r["pix"] == -1) and np.all(r["coh2"] == 0) and np.all(r["tot2"] == 0)
+    # all-zero SNR: coh2 = tot2 = null2 = 0 and a valid pixel (A19: every pixel is an arg-max)
+    trig["valid"] = 1
+    res = sp.results_to_numpy(plan.search(view, sp.triggers_from_numpy(trig), 16))
+    torch.cuda.synchronize()
+    assert np.all((res["pix"] >= 0) & (res["pix"] < plan.n_pix))
+    assert np.all(res["coh2"] == 0) and np.all(res["tot2"] == 0) and np.all(res["null2"] == 0)
+    zc = np.zeros((3, 16, L), np.complex64)
+    U.check_sky(res, zc, L, L - 1, u2, delay, trig)
