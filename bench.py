@@ -468,7 +468,7 @@ def run_ours(args):
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:
-        s = oracle_sample(args, min(4096, T), 2, 1024 if has_sky else 0)
+        s = oracle_sample(args, min(8192, T), 2, 4096 if has_sky else 0)        # about 10-15 s of host work at config 4
         cpu_v, cpu_t = oracle_whole_step_rate(s, upd_chunk, evals / K if has_sky else 0, n_slots)
         line["cpu_baseline"] = {
             "value": cpu_v, "unit": UNIT, "cores": s["threads"], "kind": "oracle",
