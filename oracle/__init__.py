@@ -176,3 +176,52 @@ def sky_eval(u2, delay, z, det_stride, row_stride, ring_len, k_newest, row, det,
                                      C.c_int32(row), C.c_int32(det), C.c_int64(k),
                                      C.c_int(s), C.c_int64(step), _p(sm), C.c_int64(p), _p(res))
     return bool(ok), res[0], res[1], res[2]
+
+
+def template_autocorr(bank, t, nj, n_response=None):
+    """Normalised autocorrelation A[j] = sum_n h[n+j] conj(h[n]) / sum_n |h[n]|^2, j = -nj..nj, of the
+    impulse response h of template ``t`` (a single-band template at the output rate)
+    ("the correlation function of a template with itself").  h is obtained by running the oracle's
+    own recursion (O2+O3) on a unit impulse; the sums are written out directly.  complex128[2*nj+1]."""
+    off = np.asarray(bank["tmpl_offset"])
+    sl = slice(int(off[t]), int(off[t + 1]))
+    a, b, d = np.asarray(bank["a"])[sl], np.asarray(bank["b"])[sl], np.asarray(bank["delay"])[sl]
+    if len(set(np.asarray(bank["band"])[sl].tolist())) > 1:
+        raise ValueError("template_autocorr: single-band templates only")
+    if n_response is None:
+        tau = -1.0 / np.log(np.abs(a.astype(np.complex128)))
+        n_response = int(d.max() + 25.0 * tau.max()) + nj + 8
+    x = np.zeros(n_response)
+    x[0] = 1.0
+    h = band_sum(x, a, b, d)
+    norm = np.sum(np.abs(h) ** 2)
+    A = np.zeros(2 * nj + 1, np.complex128)
+    for j in range(-nj, nj + 1):
+        if j >= 0:
+            A[j + nj] = np.sum(h[j:] * np.conj(h[:len(h) - j]))
+        else:
+            A[j + nj] = np.sum(h[:len(h) + j] * np.conj(h[-j:]))
+    return A / norm
+
+
+def xi2(delay, z, det_stride, row_stride, ring_len, k_newest, trig_valid, trig_row, trig_det, trig_k, pix,
+        acorr, nj):
+    """O8 (Eq. 11, 12).  acorr complex128 [rows][2*nj+1].  Returns float64 [n_trig][n_det+2] =
+    xi_I^2 per detector, xi_C^2, used flag."""
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    n_det = delay.shape[1]
+    n_trig = len(trig_k)
+    tv = np.ascontiguousarray(trig_valid, dtype=np.int32)
+    tr = np.ascontiguousarray(trig_row, dtype=np.int32)
+    td = np.ascontiguousarray(trig_det, dtype=np.int32)
+    tk = np.ascontiguousarray(trig_k, dtype=np.int64)
+    px = np.ascontiguousarray(pix, dtype=np.int32)
+    ac = np.ascontiguousarray(acorr, dtype=np.complex128)
+    assert ac.shape[1] == 2 * nj + 1
+    out = np.zeros((n_trig, n_det + 2))
+    buf, va = _view_args(z, det_stride, row_stride, ring_len, k_newest)
+    rc = lib().spiir_oracle_xi2(C.c_int(n_det), _p(delay), *va, C.c_int64(n_trig), _p(tv), _p(tr), _p(td),
+                                _p(tk), _p(px), _p(ac.view(np.float64)), C.c_int(nj), _p(out))
+    if rc != 0:
+        raise ValueError("spiir_oracle_xi2: bad arguments")
+    return out

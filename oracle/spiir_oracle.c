@@ -16,6 +16,7 @@
  *   O4 peaks
  *   O6 coherent / null PAPER.md:147-157 (Eq. 9, 10), PAPER.md:483-495 (Eq. 28-30)
  *   O7 time slides
+ *   O8 xi^2 (NEXT-1)   PAPER.md:177-188 (Eq. 11, 12)
  * (O5, the look-up table build, is in oracle/sky.py because it uses numpy's SVD.)
  *
  * Pins (tests/test_oracle_pins.py): P1 impulse response, P2 brute-force
@@ -348,6 +349,61 @@ EXPORT int spiir_oracle_sky_eval(int n_det, int64_t n_pix, const float* u2, cons
     if (!eval_pixel(&c, row, trig_det, k, shift, p, &coh2, &tot2)) { res[0] = res[1] = res[2] = 0; return 0; }
     res[0] = coh2; res[1] = tot2 - coh2; res[2] = tot2;
     return 1;
+}
+
+/* ---------------------------------------------------------------- O8 ---- */
+/* Signal-consistency statistic, PAPER.md:177-188 (Eq. 11, 12):
+ *   xi_I^2 = sum_{j=-nj}^{nj} |z_I[c_I + j] - z_I[c_I] A[j]|^2 / sum_j (2 - 2 |A[j]|^2),
+ *   xi_C^2 = (1/N_d) sum_I xi_I^2,
+ * with A = acorr[row][j + nj] the template's normalised autocorrelation (A[0] = 1)
+ * and c_I = k + delay[pix][I] - delay[pix][T] the sample of detector I aligned with
+ * the trigger at the direction `pix` found by the coherent search (reading X1 in
+ * DESIGN.md).  out[n_trig][n_det + 2] = xi_I^2 ..., xi_C^2, used (1/0).  A slot that
+ * is invalid, has pix < 0, or whose window leaves the view in any detector gives zeros. */
+EXPORT int spiir_oracle_xi2(int n_det, const int32_t* delay,
+                            const void* z, int z_is_f32, int64_t det_stride, int64_t row_stride,
+                            int64_t ring_len, int64_t k_newest,
+                            int64_t n_trig, const int32_t* trig_valid, const int32_t* trig_row,
+                            const int32_t* trig_det, const int64_t* trig_k, const int32_t* pix,
+                            const double* acorr, int nj, double* out)
+{
+    if (n_det < 1 || n_det > 8 || nj < 1) return -1;
+    const sky_ctx c = { n_det, 0, NULL, delay, z, z_is_f32, det_stride, row_stride, ring_len, k_newest };
+    const int W = 2 * nj + 1;
+    #pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < n_trig; ++i) {
+        double* o = out + (size_t)i * (n_det + 2);
+        for (int q = 0; q < n_det + 2; ++q) o[q] = 0.0;
+        if (!trig_valid[i] || pix[i] < 0) continue;
+        const int32_t* dl = delay + (size_t)pix[i] * n_det;
+        const double* A = acorr + (size_t)trig_row[i] * W * 2;
+        int ok = 1;
+        for (int I = 0; I < n_det; ++I) {
+            const int64_t ci = trig_k[i] + (int64_t)dl[I] - (int64_t)dl[trig_det[i]];
+            if (!in_range(&c, ci - nj) || !in_range(&c, ci + nj)) ok = 0;
+        }
+        if (!ok) continue;
+        double den = 0.0;
+        for (int j = 0; j < W; ++j) den += 2.0 - 2.0 * (A[2 * j] * A[2 * j] + A[2 * j + 1] * A[2 * j + 1]);
+        double mean = 0.0;
+        for (int I = 0; I < n_det; ++I) {
+            const int64_t ci = trig_k[i] + (int64_t)dl[I] - (int64_t)dl[trig_det[i]];
+            double z0r, z0i, num = 0.0;
+            z_at(&c, I, trig_row[i], ci, &z0r, &z0i);
+            for (int j = -nj; j <= nj; ++j) {
+                double zr, zi;
+                z_at(&c, I, trig_row[i], ci + j, &zr, &zi);
+                const double ar = A[2 * (j + nj)], ai = A[2 * (j + nj) + 1];
+                const double er = zr - (z0r * ar - z0i * ai), ei = zi - (z0r * ai + z0i * ar);
+                num += er * er + ei * ei;
+            }
+            o[I] = den > 0.0 ? num / den : 0.0;
+            mean += o[I];
+        }
+        o[n_det] = mean / n_det;
+        o[n_det + 1] = 1.0;
+    }
+    return 0;
 }
 
 EXPORT int spiir_oracle_num_threads(void)

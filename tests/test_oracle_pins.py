@@ -471,3 +471,92 @@ def test_generator_is_seeded_and_shaped():
     assert list(cnt) == [75] * 8 and np.all(np.diff(b2["band"][:600].astype(int)) >= 0)
     from workloads.gen import _split_over_bands
     assert _split_over_bands(700, 8) == [87, 87, 87, 87, 88, 88, 88, 88]
+
+
+# ---- O8 (NEXT-1): signal-consistency statistic, PAPER.md:177-188 (Eq. 11, 12) -------------
+def _one_template_bank(a, b, d):
+    return dict(n_templates=1, band_rates=[2048], out_band=0, tmpl_offset=np.array([0, len(a)], np.int64),
+                a=a, b=b, delay=d, band=np.zeros(len(a), np.uint8), max_delay=[int(d.max())])
+
+
+def test_p18_autocorrelation_closed_forms():
+    # one filter: h[n] = b a^(n-d)  ->  A[j] = a^j (j >= 0), conj(a)^|j| (j < 0), whatever b and d
+    a = np.array([np.exp(-1 / 37.0 + 0.83j)], np.complex64)
+    b = np.array([0.3 - 1.1j], np.complex64)
+    bank = _one_template_bank(a, b, np.array([11], np.int32))
+    A = oracle.template_autocorr(bank, 0, 20)
+    a64 = complex(a[0])
+    for j in range(-20, 21):
+        ref = a64 ** j if j >= 0 else np.conj(a64) ** (-j)
+        assert abs(A[j + 20] - ref) < 1e-12
+    # several filters with delays: the double sum over filter pairs of geometric series (P3's kernel at lag j)
+    rng = np.random.default_rng(18)
+    a, b, d = _rand_filters(rng, 6, dmax=25)
+    A = oracle.template_autocorr(_one_template_bank(a, b, d), 0, 45)
+    aa, bb = a.astype(np.complex128), b.astype(np.complex128)
+    def R(j):
+        tot = 0.0
+        for l in range(6):
+            for m in range(6):
+                n0 = max(int(d[l]) - j, int(d[m]))
+                tot += bb[l] * np.conj(bb[m]) * aa[l] ** (n0 + j - int(d[l])) * np.conj(aa[m]) ** (n0 - int(d[m])) \
+                       / (1 - aa[l] * np.conj(aa[m]))
+        return tot
+    r0 = R(0)
+    for j in (-45, -7, -1, 0, 1, 3, 40):
+        assert abs(A[j + 45] - R(j) / r0) < 1e-10
+    assert abs(A[45] - 1) < 1e-14 and np.allclose(A[::-1], np.conj(A))       # Hermitian, A[0] = 1
+
+
+def test_p19_xi2_exact_signal_and_single_outlier():
+    """z_I[c_I + j] = z0_I A[j] gives xi^2 = 0; one extra sample e at lag j1 != 0 in one detector gives
+    xi_I^2 = |e|^2 / sum_j (2 - 2|A[j]|^2) there and xi_C^2 = that / N_d (Eq. 11, 12 by hand)."""
+    nj, D, L = 12, 3, 200
+    rng = np.random.default_rng(19)
+    A = np.zeros((2, 2 * nj + 1), np.complex128)
+    for r in range(2):
+        aa = np.exp(-1 / (5.0 + 3 * r) + 1j * (0.4 + 0.5 * r))
+        A[r] = [aa ** j if j >= 0 else np.conj(aa) ** (-j) for j in range(-nj, nj + 1)]
+    delay = np.array([[0, 3, -5], [2, -4, 1]], np.int32)                     # two "pixels"
+    z = np.zeros((D, 2, L), np.complex128)
+    k, T, pix, row = 100, 1, 1, 1
+    z0 = rng.standard_normal(D) + 1j * rng.standard_normal(D)
+    for I in range(D):
+        c = k + delay[pix, I] - delay[pix, T]
+        z[I, row, c - nj:c + nj + 1] = z0[I] * A[row]
+    args = dict(trig_valid=[1], trig_row=[row], trig_det=[T], trig_k=[k], pix=[pix], acorr=A, nj=nj)
+    out = oracle.xi2(delay, z, 2 * L, L, L, L - 1, **args)
+    assert np.all(np.abs(out[0, :D + 1]) < 1e-28) and out[0, D + 1] == 1
+    e, j1, I1 = 0.7 - 0.2j, 5, 2
+    z[I1, row, k + delay[pix, I1] - delay[pix, T] + j1] += e
+    out = oracle.xi2(delay, z, 2 * L, L, L, L - 1, **args)
+    den = np.sum(2 - 2 * np.abs(A[row]) ** 2)
+    assert abs(out[0, I1] - abs(e) ** 2 / den) < 1e-14 and abs(out[0, D] - abs(e) ** 2 / den / D) < 1e-14
+    assert out[0, 0] < 1e-28 and out[0, 1] < 1e-28
+    # wrong pixel (other delays) no longer lines the windows up: the statistic is large
+    bad = dict(args); bad["pix"] = [0]
+    assert oracle.xi2(delay, z, 2 * L, L, L, L - 1, **bad)[0, D] > 1e-3
+    # invalid slot, no pixel, window leaving the view: zeros and used = 0
+    for kw in (dict(trig_valid=[0]), dict(pix=[-1]), dict(trig_k=[L - 3]), dict(trig_k=[nj - 1])):
+        a2 = dict(args); a2.update(kw)
+        assert np.all(oracle.xi2(delay, z, 2 * L, L, L, L - 1, **a2) == 0)
+
+
+def test_p20_xi2_has_mean_one_in_gaussian_noise():
+    """"a reduced chi^2 with a mean value of 1" - unit white noise through the oracle's own
+    bank, A from the oracle's autocorrelation of the same templates."""
+    rng = np.random.default_rng(20)
+    bank = workloads.random_bank(rng, 6, 24, [2048], tau_range=(5.0, 60.0), max_delay=100)
+    n, nj = 60000, 60
+    x = rng.standard_normal((2, n)).astype(np.float32)
+    z = oracle.filter_bank(x, bank)                                           # E|z|^2 = 2 (A8)
+    A = np.stack([oracle.template_autocorr(bank, t, nj) for t in range(6)])
+    ks = np.arange(2000, n - 200, 150)
+    rows = np.repeat(np.arange(6), len(ks)); kk = np.tile(ks, 6)
+    m = len(kk)
+    delay = np.zeros((1, 2), np.int32)
+    out = oracle.xi2(delay, z, 6 * n, n, n, n - 1, np.ones(m, np.int32), rows, np.zeros(m, np.int32), kk,
+                     np.zeros(m, np.int32), A, nj)
+    assert np.all(out[:, 3] == 1)
+    assert abs(out[:, :2].mean() - 1.0) < 0.03                               # ~4600 windows of ~120 dof each
+    assert np.allclose(out[:, 2], out[:, :2].mean(axis=1))                   # Eq. 12
