@@ -404,6 +404,35 @@ def run_ours(args):
             okb = bg_np["pix"][prev_np["valid"] == 1] >= 0
             searched = min(searched, float(okb.mean())) if okb.size else searched
 
+    # ---- NEXT-1 (outside the timed step): xi^2 of the last step's candidates (Eq. 11, 12), n_j = 175, on a
+    #      seeded synthetic autocorrelation table (the arithmetic and the traffic do not depend on its values)
+    xi2_info = None
+    if has_sky:
+        nj = 175
+        g = torch.Generator(device="cpu").manual_seed(cfg["seed"])
+        lag = torch.arange(-nj, nj + 1, dtype=torch.float32)
+        tau = 5.0 + 40.0 * torch.rand(T, 1, generator=g)
+        om = 0.1 + 1.2 * torch.rand(T, 1, generator=g)
+        env = torch.exp(-lag.abs()[None, :] / tau)
+        ac = torch.stack([env * torch.cos(om * lag[None, :]), env * torch.sin(om * lag[None, :])], dim=-1).contiguous().to(dev)
+        dl_dev = torch.from_numpy(np.ascontiguousarray(delay, dtype=np.int32)).to(dev)
+        prev = trig[state["i"] & 1]
+        view = bk.snr_view()
+        xi_out = torch.empty(n_slots, 24, dtype=torch.uint8, device=dev)
+        ex = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        for rep in range(4):
+            if rep == 1: ex[0].record()
+            sp.signal_consistency(view, dl_dev, prev, fg_out, n_slots, ac, nj, out=xi_out)
+        ex[1].record()
+        torch.cuda.synchronize()
+        xi = sp.xi2_to_numpy(xi_out)
+        n_used = int(xi["used"].sum())
+        ms_xi = ex[0].elapsed_time(ex[1]) / 3.0
+        by = n_used * (D + 1) * (2 * nj + 1) * 8.0
+        xi2_info = {"ms": ms_xi, "candidates": n_used, "algorithmic_GBps": by / (ms_xi * 1e-3) / 1e9,
+                    "median_xi2_c": float(np.median(xi["xi2_c"][xi["used"] == 1])) if n_used else None,
+                    "note": "not part of the timed step; synthetic autocorrelation table"}
+
     # ---- end to end: pinned host strain in, host candidates and results out, every step
     e2e = None
     if not args.no_e2e:
@@ -465,6 +494,7 @@ def run_ours(args):
         "per_step": {"updates": upd_chunk, "candidates": n_cand / K if has_sky else None,
                      "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
         "roofline": dominant, "roofline_other": other,
+        "next_rows": {"xi2": xi2_info},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:

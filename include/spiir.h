@@ -197,6 +197,27 @@ int timeslide_background(spiir_sky_plan* bg_plan, const spiir_snr_view* view,
                          const spiir_trigger* dev_trig, int32_t n_slots,
                          int32_t n_slides, int64_t step_samples, const int32_t* host_slide_mult,
                          spiir_sky_result* dev_out, void* stream);
+/* NEXT-1 — signal-consistency statistic (Eq. 11 and 12), the second
+ * half of the paper's ranking pair (rho_C, xi_C^2).  For every trigger slot with a sky
+ * result (pix >= 0):
+ *   c_I    = k + delay[pix][I] - delay[pix][T]     (sample of detector I aligned with the trigger)
+ *   xi_I^2 = sum_{j=-n_j}^{n_j} |z_I[c_I + j] - z_I[c_I] A[j]|^2 / sum_j (2 - 2 |A[j]|^2)
+ *   xi_C^2 = (1/n_det) sum_I xi_I^2
+ * with A = dev_autocorr[tmpl][j + n_j], the template's normalised autocorrelation (A[0] = 1).
+ * used = 0 and zeros if the slot is invalid, has no pixel, or a window leaves the view.  24 bytes. */
+typedef struct { float xi2_c; int32_t used; float xi2[SPIIR_MAX_DET]; } spiir_xi2_result;
+/*   dev_delay    [n_pix][n_det] int32, the table handed to spiir_sky_plan_init, on the device
+ *   dev_sky      [n_slots] results of coherent_sky_search for the same dev_trig
+ *   dev_autocorr [rows of the view][2 n_j + 1] complex;  dev_out [n_slots] */
+int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t n_pix, const int32_t* dev_delay,
+                             const spiir_trigger* dev_trig, const spiir_sky_result* dev_sky, int32_t n_slots,
+                             const spiir_c32* dev_autocorr, int32_t n_j, spiir_xi2_result* dev_out, void* stream);
+/* Host helper (float64 inside, set-up only): A[j] = sum_n h[n+j] conj(h[n]) / sum_n |h[n]|^2, j = -n_j..n_j,
+ * of the impulse response h[n] = sum_l b_l a_l^(n - d_l) [n >= d_l] of ONE template whose filters all run at
+ * the output rate.  host_out [2 n_j + 1]. */
+int spiir_template_autocorr(int64_t n_filters, const spiir_c32* host_a, const spiir_c32* host_b,
+                            const int32_t* host_delay, int32_t n_j, spiir_c32* host_out);
+
 /* Introspection: the layout chosen for a band (lanes per unit G, filters per lane
  * F, units, padded slots, shared-memory history depth) and counters for bench. */
 typedef struct {

@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     spiir_bank_desc, spiir_snr_view, spiir_band_plan, TRIGGER_DTYPE, RESULT_DTYPE,
     make_desc, Bank, SkyPlan, SnrView, sky_table_build,
     triggers_to_numpy, triggers_from_numpy, results_to_numpy, fp32_peak_probe,
+    XI2_DTYPE, template_autocorr, signal_consistency, xi2_to_numpy,
     SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EOVERFLOW,
 )
 from . import binding as _b

@@ -53,7 +53,8 @@ class spiir_band_plan(C.Structure):
 TRIGGER_DTYPE = np.dtype([("valid", "<i4"), ("tmpl", "<i4"), ("det", "<i4"), ("_pad", "<i4"), ("k", "<i8"),
                           ("z_re", "<f4"), ("z_im", "<f4"), ("snr", "<f4"), ("_pad2", "<f4")])
 RESULT_DTYPE = np.dtype([("coh2", "<f4"), ("null2", "<f4"), ("tot2", "<f4"), ("pix", "<i4")])
-assert TRIGGER_DTYPE.itemsize == 40 and RESULT_DTYPE.itemsize == 16
+XI2_DTYPE = np.dtype([("xi2_c", "<f4"), ("used", "<i4"), ("xi2", "<f4", (SPIIR_MAX_DET,))])
+assert TRIGGER_DTYPE.itemsize == 40 and RESULT_DTYPE.itemsize == 16 and XI2_DTYPE.itemsize == 24
 
 _SIGNATURES = {
     "spiir_bank_workspace_bytes": (C.c_int, [C.POINTER(spiir_bank_desc), C.POINTER(C.c_size_t)]),
@@ -81,6 +82,9 @@ _SIGNATURES = {
     "spiir_bank_timing_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                          C.POINTER(C.c_int32)]),
     "spiir_fp32_peak_probe": (C.c_int, [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
+    "spiir_signal_consistency": (C.c_int, [C.POINTER(spiir_snr_view), C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
+                                           C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
+    "spiir_template_autocorr": (C.c_int, [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]),
     "spiir_last_error": (C.c_char_p, []),
 }
 EXPORTS = sorted(_SIGNATURES)
@@ -328,3 +332,36 @@ def fp32_peak_probe(reps=20):
     ms, fma = C.c_double(0), C.c_double(0)
     _check(lib().spiir_fp32_peak_probe(reps, C.byref(ms), C.byref(fma), _stream()))
     return fma.value * reps / (ms.value * 1e-3), ms.value
+
+
+def template_autocorr(bank, t, n_j):
+    """spiir_template_autocorr for template ``t`` of a bank dict: complex64 [2 n_j + 1]."""
+    off = np.asarray(bank["tmpl_offset"])
+    sl = slice(int(off[t]), int(off[t + 1]))
+    a = np.ascontiguousarray(np.asarray(bank["a"])[sl], dtype=np.complex64)
+    b = np.ascontiguousarray(np.asarray(bank["b"])[sl], dtype=np.complex64)
+    d = np.ascontiguousarray(np.asarray(bank["delay"])[sl], dtype=np.int32)
+    out = np.zeros(2 * n_j + 1, np.complex64)
+    _check(lib().spiir_template_autocorr(len(d), _hp(a), _hp(b), _hp(d), n_j, _hp(out)))
+    return out
+
+
+def signal_consistency(view, delay_dev, trig, sky, n_slots, autocorr_dev, n_j, out=None):
+    """spiir_signal_consistency; delay_dev int32 cuda [n_pix][n_det], trig uint8 cuda [n_slots][40],
+    sky uint8 cuda [n_slots][16], autocorr_dev float32 cuda [rows][2 n_j + 1][2]; returns uint8 cuda
+    [n_slots][24] (XI2_DTYPE)."""
+    import torch
+    n_pix, n_det = delay_dev.shape
+    assert delay_dev.is_cuda and delay_dev.dtype == torch.int32 and delay_dev.is_contiguous()
+    assert autocorr_dev.is_cuda and autocorr_dev.is_contiguous() and autocorr_dev.shape[-2] == 2 * n_j + 1
+    if out is None:
+        out = torch.empty(n_slots, 24, dtype=torch.uint8, device="cuda")
+    _check(lib().spiir_signal_consistency(C.byref(view.c), n_det, n_pix, C.c_void_p(delay_dev.data_ptr()),
+                                          C.c_void_p(trig.data_ptr()), C.c_void_p(sky.data_ptr()), n_slots,
+                                          C.c_void_p(autocorr_dev.data_ptr()), n_j, C.c_void_p(out.data_ptr()),
+                                          _stream()))
+    return out
+
+
+def xi2_to_numpy(out):
+    return out.cpu().numpy().view(XI2_DTYPE).reshape(-1)

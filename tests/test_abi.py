@@ -42,7 +42,7 @@ def test_every_declared_symbol_is_exported(sp):
 def test_struct_sizes_match_the_header(sp):
     assert C.sizeof(sp.spiir_snr_view) == 40
     assert C.sizeof(sp.spiir_bank_desc) == 16 + 32 + 32 + 8 + 7 * 8 + 8 + 8
-    assert sp.TRIGGER_DTYPE.itemsize == 40 and sp.RESULT_DTYPE.itemsize == 16
+    assert sp.TRIGGER_DTYPE.itemsize == 40 and sp.RESULT_DTYPE.itemsize == 16 and sp.XI2_DTYPE.itemsize == 24
 
 
 def test_workspace_query_and_bad_arguments(sp):
@@ -110,3 +110,18 @@ def test_product_package_never_imports_the_oracle():
                 txt = open(os.path.join(dp, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
                 assert "libspiir_oracle" not in txt and "spiir_oracle" not in txt, f
+
+
+def test_host_autocorrelation_matches_the_oracle(sp):
+    """spiir_template_autocorr (library, float64 host helper) against the oracle's own autocorrelation of the
+    same templates, and its refusal of unstable filters."""
+    import oracle
+    bank = workloads.bank_for_config(0)
+    for t in range(bank["n_templates"]):
+        A = sp.template_autocorr(bank, t, 60)
+        ref = oracle.template_autocorr(bank, t, 60)
+        assert abs(A[60] - 1) < 1e-6 and np.abs(A - ref).max() < 5e-7
+    a = np.array([1.0 + 0j], np.complex64); b = np.array([1.0 + 0j], np.complex64); d = np.zeros(1, np.int32)
+    out = np.zeros(3, np.complex64)
+    rc = sp.spiir_template_autocorr(1, a.ctypes.data, b.ctypes.data, d.ctypes.data, 1, out.ctypes.data)
+    assert rc == sp.SPIIR_EINVAL and sp.last_error()

@@ -458,3 +458,61 @@ def test_cfg3_full_size_sampled(sp, U):
     strong = sig[truth["rho"][sig] > 12]
     assert len(strong) > 50
     assert np.median(fg["coh2"][strong] / np.median(bg["coh2"][strong], axis=1)) > 2   # (the slid background keeps |z_T|^2)
+
+
+# ------------------------------------------------------------------ NEXT-1: signal-consistency statistic (Eq. 11, 12)
+def test_xi2_signal_consistency(sp, U):
+    """Bank -> peaks -> sky search -> xi^2 on the bank's own ring (one-chunk lag), against the oracle's O8
+    on the same float32 SNR, the same pixels and the same float32 autocorrelation table.  Tolerance: 1e-4
+    relative + 1e-5 (351 float32 terms of order 1 per sum)."""
+    import torch
+    cfg = workloads.config(1)
+    T, D, NC, nj = 24, 3, 4, 175
+    bank = workloads.bank_for_config(1, n_templates=T)
+    bank_A = dict(bank)
+    st = workloads.strain_for_config(1, seconds=NC)
+    x = st["strain"]
+    u2, delay = _table(cfg, gmst=st["gmst"])
+    ring = NC * 2048
+    bk = sp.Bank(bank, D, 2048, ring_len=ring)
+    plan = sp.SkyPlan(u2, delay, max_slots=D * T)
+    # template 0 is chirp-matched with delays up to 24 576: its autocorrelation needs a long response
+    acorr = np.stack([sp.template_autocorr(bank_A, t, nj) for t in range(T)])
+    ac_dev = torch.from_numpy(acorr.view(np.float32).reshape(T, 2 * nj + 1, 2)).cuda()
+    dl_dev = torch.from_numpy(np.ascontiguousarray(delay, dtype=np.int32)).cuda()
+    xs = torch.from_numpy(x).cuda()
+    z = np.zeros((D, T, NC * 2048), np.complex64)
+    out = torch.empty(D, T, 2048, 2, dtype=torch.float32, device="cuda")
+    trig_dev = None
+    for c in range(NC):
+        bk.filter_chunk(xs[:, c * 2048:(c + 1) * 2048].contiguous(), out)
+        z[:, :, c * 2048:(c + 1) * 2048] = out.cpu().numpy().view(np.complex64)[..., 0]
+        if c == NC - 2:
+            tr, cnt = bk.peaks(2.5, 0)
+            torch.cuda.synchronize()
+            trig_dev, trig = tr.clone(), sp.triggers_to_numpy(tr).copy()
+    view = bk.snr_view()
+    sky = plan.search(view, trig_dev, D * T)
+    xi = sp.xi2_to_numpy(sp.signal_consistency(view, dl_dev, trig_dev, sky, D * T, ac_dev, nj))
+    torch.cuda.synchronize()
+    res = sp.results_to_numpy(sky)
+    k_newest = NC * 2048 - 1
+    ref = oracle.xi2(delay, z, T * ring, ring, ring, k_newest, trig["valid"], trig["tmpl"], trig["det"], trig["k"],
+                     res["pix"], acorr.astype(np.complex128), nj)
+    used = ref[:, D + 1] == 1
+    assert used.sum() >= 20 and np.array_equal(xi["used"], used.astype(np.int32))
+    assert np.array_equal(used, (trig["valid"] == 1) & (res["pix"] >= 0))
+    for I in range(D):
+        assert np.all(np.abs(xi["xi2"][:, I] - ref[:, I]) <= 1e-4 * ref[:, I] + 1e-5)
+    assert np.all(np.abs(xi["xi2_c"] - ref[:, D]) <= 1e-4 * ref[:, D] + 1e-5)
+    assert np.all(xi["xi2"][~used] == 0) and np.all(xi["xi2_c"][~used] == 0)
+    # noise candidates: a reduced chi^2 of order 1 (PAPER.md:182); not exactly 1, the windows are centred on maxima
+    assert 0.5 < np.median(xi["xi2_c"][used]) < 1.5
+    # a window that leaves the view (candidates of the newest chunk, k + 175 > k_newest for some) is refused
+    tr2, _ = bk.peaks(0.0, 0)
+    sky2 = plan.search(view, tr2, D * T)
+    xi2b = sp.xi2_to_numpy(sp.signal_consistency(view, dl_dev, tr2, sky2, D * T, ac_dev, nj))
+    t2, r2 = sp.triggers_to_numpy(tr2), sp.results_to_numpy(sky2)
+    ref2 = oracle.xi2(delay, z, T * ring, ring, ring, k_newest, t2["valid"], t2["tmpl"], t2["det"], t2["k"],
+                      r2["pix"], acorr.astype(np.complex128), nj)
+    assert np.array_equal(xi2b["used"], ref2[:, D + 1].astype(np.int32)) and (xi2b["used"] == 0).any()
