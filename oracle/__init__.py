@@ -205,23 +205,27 @@ def template_autocorr(bank, t, nj, n_response=None):
 
 
 def xi2(delay, z, det_stride, row_stride, ring_len, k_newest, trig_valid, trig_row, trig_det, trig_k, pix,
-        acorr, nj):
-    """O8 (Eq. 11, 12).  acorr complex128 [rows][2*nj+1].  Returns float64 [n_trig][n_det+2] =
+        acorr, nj, n_slides=0, step=0, slide_mult=None):
+    """O8 (Eq. 11, 12).  acorr complex128 [rows][2*nj+1]; pix int32 [n_trig] (foreground) or
+    [n_trig][n_slides].  Returns float64 [n_trig][n_det+2] (or [n_trig][n_slides][n_det+2]) =
     xi_I^2 per detector, xi_C^2, used flag."""
     delay = np.ascontiguousarray(delay, dtype=np.int32)
     n_det = delay.shape[1]
     n_trig = len(trig_k)
+    S = max(1, n_slides)
     tv = np.ascontiguousarray(trig_valid, dtype=np.int32)
     tr = np.ascontiguousarray(trig_row, dtype=np.int32)
     td = np.ascontiguousarray(trig_det, dtype=np.int32)
     tk = np.ascontiguousarray(trig_k, dtype=np.int64)
-    px = np.ascontiguousarray(pix, dtype=np.int32)
+    px = np.ascontiguousarray(pix, dtype=np.int32).reshape(n_trig, S)
+    sm = np.ascontiguousarray(slide_mult if slide_mult is not None else np.zeros(n_det), dtype=np.int32)
     ac = np.ascontiguousarray(acorr, dtype=np.complex128)
     assert ac.shape[1] == 2 * nj + 1
-    out = np.zeros((n_trig, n_det + 2))
+    out = np.zeros((n_trig, S, n_det + 2))
     buf, va = _view_args(z, det_stride, row_stride, ring_len, k_newest)
     rc = lib().spiir_oracle_xi2(C.c_int(n_det), _p(delay), *va, C.c_int64(n_trig), _p(tv), _p(tr), _p(td),
-                                _p(tk), _p(px), _p(ac.view(np.float64)), C.c_int(nj), _p(out))
+                                _p(tk), _p(px), C.c_int(n_slides), C.c_int64(step), _p(sm),
+                                _p(ac.view(np.float64)), C.c_int(nj), _p(out))
     if rc != 0:
         raise ValueError("spiir_oracle_xi2: bad arguments")
-    return out
+    return out if n_slides > 0 else out[:, 0]

@@ -358,50 +358,59 @@ EXPORT int spiir_oracle_sky_eval(int n_det, int64_t n_pix, const float* u2, cons
  * with A = acorr[row][j + nj] the template's normalised autocorrelation (A[0] = 1)
  * and c_I = k + delay[pix][I] - delay[pix][T] the sample of detector I aligned with
  * the trigger at the direction `pix` found by the coherent search (reading X1 in
- * DESIGN.md).  out[n_trig][n_det + 2] = xi_I^2 ..., xi_C^2, used (1/0).  A slot that
- * is invalid, has pix < 0, or whose window leaves the view in any detector gives zeros. */
+ * DESIGN.md).  n_slides = 0: foreground, pix[n_trig]; n_slides >= 1: the same for the
+ * time-slid companions of O7, pix[n_trig][n_slides].  out[n_trig][S][n_det + 2] =
+ * xi_I^2 ..., xi_C^2, used (1/0).  A slot that is invalid, has pix < 0, or whose window
+ * leaves the view in any detector gives zeros. */
 EXPORT int spiir_oracle_xi2(int n_det, const int32_t* delay,
                             const void* z, int z_is_f32, int64_t det_stride, int64_t row_stride,
                             int64_t ring_len, int64_t k_newest,
                             int64_t n_trig, const int32_t* trig_valid, const int32_t* trig_row,
                             const int32_t* trig_det, const int64_t* trig_k, const int32_t* pix,
+                            int n_slides, int64_t step, const int32_t* slide_mult,
                             const double* acorr, int nj, double* out)
 {
     if (n_det < 1 || n_det > 8 || nj < 1) return -1;
     const sky_ctx c = { n_det, 0, NULL, delay, z, z_is_f32, det_stride, row_stride, ring_len, k_newest };
     const int W = 2 * nj + 1;
+    const int S = n_slides > 0 ? n_slides : 1;
     #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t i = 0; i < n_trig; ++i) {
-        double* o = out + (size_t)i * (n_det + 2);
-        for (int q = 0; q < n_det + 2; ++q) o[q] = 0.0;
-        if (!trig_valid[i] || pix[i] < 0) continue;
-        const int32_t* dl = delay + (size_t)pix[i] * n_det;
-        const double* A = acorr + (size_t)trig_row[i] * W * 2;
-        int ok = 1;
-        for (int I = 0; I < n_det; ++I) {
-            const int64_t ci = trig_k[i] + (int64_t)dl[I] - (int64_t)dl[trig_det[i]];
-            if (!in_range(&c, ci - nj) || !in_range(&c, ci + nj)) ok = 0;
-        }
-        if (!ok) continue;
-        double den = 0.0;
-        for (int j = 0; j < W; ++j) den += 2.0 - 2.0 * (A[2 * j] * A[2 * j] + A[2 * j + 1] * A[2 * j + 1]);
-        double mean = 0.0;
-        for (int I = 0; I < n_det; ++I) {
-            const int64_t ci = trig_k[i] + (int64_t)dl[I] - (int64_t)dl[trig_det[i]];
-            double z0r, z0i, num = 0.0;
-            z_at(&c, I, trig_row[i], ci, &z0r, &z0i);
-            for (int j = -nj; j <= nj; ++j) {
-                double zr, zi;
-                z_at(&c, I, trig_row[i], ci + j, &zr, &zi);
-                const double ar = A[2 * (j + nj)], ai = A[2 * (j + nj) + 1];
-                const double er = zr - (z0r * ar - z0i * ai), ei = zi - (z0r * ai + z0i * ar);
-                num += er * er + ei * ei;
+        for (int s = 0; s < S; ++s) {
+            double* o = out + ((size_t)i * S + s) * (n_det + 2);
+            const int32_t px = pix[(size_t)i * S + s];
+            for (int q = 0; q < n_det + 2; ++q) o[q] = 0.0;
+            if (!trig_valid[i] || px < 0) continue;
+            const int32_t* dl = delay + (size_t)px * n_det;
+            const double* A = acorr + (size_t)trig_row[i] * W * 2;
+            int64_t ci[8];
+            int ok = 1;
+            for (int I = 0; I < n_det; ++I) {
+                /* time slide s+1 reads detector I != T at k - (s+1) step m_I + Delta (O7) */
+                const int64_t shift = (n_slides > 0 && I != trig_det[i]) ? (int64_t)(s + 1) * step * slide_mult[I] : 0;
+                ci[I] = trig_k[i] - shift + (int64_t)dl[I] - (int64_t)dl[trig_det[i]];
+                if (!in_range(&c, ci[I] - nj) || !in_range(&c, ci[I] + nj)) ok = 0;
             }
-            o[I] = den > 0.0 ? num / den : 0.0;
-            mean += o[I];
+            if (!ok) continue;
+            double den = 0.0;
+            for (int j = 0; j < W; ++j) den += 2.0 - 2.0 * (A[2 * j] * A[2 * j] + A[2 * j + 1] * A[2 * j + 1]);
+            double mean = 0.0;
+            for (int I = 0; I < n_det; ++I) {
+                double z0r, z0i, num = 0.0;
+                z_at(&c, I, trig_row[i], ci[I], &z0r, &z0i);
+                for (int j = -nj; j <= nj; ++j) {
+                    double zr, zi;
+                    z_at(&c, I, trig_row[i], ci[I] + j, &zr, &zi);
+                    const double ar = A[2 * (j + nj)], ai = A[2 * (j + nj) + 1];
+                    const double er = zr - (z0r * ar - z0i * ai), ei = zi - (z0r * ai + z0i * ar);
+                    num += er * er + ei * ei;
+                }
+                o[I] = den > 0.0 ? num / den : 0.0;
+                mean += o[I];
+            }
+            o[n_det] = mean / n_det;
+            o[n_det + 1] = 1.0;
         }
-        o[n_det] = mean / n_det;
-        o[n_det + 1] = 1.0;
     }
     return 0;
 }

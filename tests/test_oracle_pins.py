@@ -560,3 +560,37 @@ def test_p20_xi2_has_mean_one_in_gaussian_noise():
     assert np.all(out[:, 3] == 1)
     assert abs(out[:, :2].mean() - 1.0) < 0.03                               # ~4600 windows of ~120 dof each
     assert np.allclose(out[:, 2], out[:, :2].mean(axis=1))                   # Eq. 12
+
+
+def test_p21_xi2_on_time_slides():
+    """O8 on the time-slid companions of O7: multipliers 0 reproduce the foreground on every slide; an exact
+    signal whose companions sit s*step earlier gives 0 on slide s only; out-of-range slides are unused."""
+    nj, D, L, step = 8, 3, 400, 50
+    rng = np.random.default_rng(21)
+    aa = np.exp(-1 / 4.0 + 0.7j)
+    A = np.array([[aa ** j if j >= 0 else np.conj(aa) ** (-j) for j in range(-nj, nj + 1)]])
+    delay = np.array([[1, -2, 4]], np.int32)
+    z = (rng.standard_normal((D, 1, L)) + 1j * rng.standard_normal((D, 1, L)))
+    k, T, S = 300, 0, 5
+    base = dict(trig_valid=[1], trig_row=[0], trig_det=[T], trig_k=[k], acorr=A, nj=nj)
+    fg = oracle.xi2(delay, z, L, L, L, L - 1, pix=[0], **base)
+    bg0 = oracle.xi2(delay, z, L, L, L, L - 1, pix=np.zeros((1, S), np.int32), n_slides=S, step=step,
+                     slide_mult=[0, 0, 0], **base)
+    for s in range(S):
+        assert np.array_equal(bg0[0, s], fg[0])
+    # plant an exact signal: trigger detector at k, companions 3 slides earlier
+    s0 = 3
+    z0 = rng.standard_normal(D) + 1j * rng.standard_normal(D)
+    for I in range(D):
+        c = k + delay[0, I] - delay[0, T] - (s0 * step if I != T else 0)
+        z[I, 0, c - nj:c + nj + 1] = z0[I] * A[0]
+    bg = oracle.xi2(delay, z, L, L, L, L - 1, pix=np.zeros((1, S), np.int32), n_slides=S, step=step,
+                    slide_mult=[1, 1, 1], **base)
+    assert bg[0, s0 - 1, D] < 1e-28 and bg[0, s0 - 1, D + 1] == 1
+    others = [s for s in range(S) if s != s0 - 1]
+    assert np.all(bg[0, others, D] > 0.05)
+    assert np.all(bg[0, :, T] < 1e-28)                                       # the trigger detector does not move
+    # the sixth slide of step 50 from k = 300 with nj = 8 and delay -2 needs sample 300-300-2-8 < 0: unused
+    bg6 = oracle.xi2(delay, z, L, L, L, L - 1, pix=np.zeros((1, 6), np.int32), n_slides=6, step=step,
+                     slide_mult=[1, 1, 1], **base)
+    assert bg6[0, 5, D + 1] == 0 and np.all(bg6[0, 5] == 0) and np.all(bg6[0, :5, D + 1] == 1)
