@@ -207,10 +207,15 @@ int timeslide_background(spiir_sky_plan* bg_plan, const spiir_snr_view* view,
  * used = 0 and zeros if the slot is invalid, has no pixel, or a window leaves the view.  24 bytes. */
 typedef struct { float xi2_c; int32_t used; float xi2[SPIIR_MAX_DET]; } spiir_xi2_result;
 /*   dev_delay    [n_pix][n_det] int32, the table handed to spiir_sky_plan_init, on the device
- *   dev_sky      [n_slots] results of coherent_sky_search for the same dev_trig
- *   dev_autocorr [rows of the view][2 n_j + 1] complex;  dev_out [n_slots] */
+ *   n_slides = 0 : foreground; dev_sky [n_slots] = results of coherent_sky_search for the same dev_trig;
+ *                  dev_out [n_slots]
+ *   n_slides >= 1: background events; dev_sky [n_slots][n_slides] = results of timeslide_background with the
+ *                  same step_samples / host_slide_mult; detector I != T is read n_slides*... earlier exactly as
+ *                  there, c_I = k - s*step*mult[I] + delay difference; dev_out [n_slots][n_slides]
+ *   dev_autocorr [rows of the view][2 n_j + 1] complex */
 int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t n_pix, const int32_t* dev_delay,
                              const spiir_trigger* dev_trig, const spiir_sky_result* dev_sky, int32_t n_slots,
+                             int32_t n_slides, int64_t step_samples, const int32_t* host_slide_mult,
                              const spiir_c32* dev_autocorr, int32_t n_j, spiir_xi2_result* dev_out, void* stream);
 /* Host helper (float64 inside, set-up only): A[j] = sum_n h[n+j] conj(h[n]) / sum_n |h[n]|^2, j = -n_j..n_j,
  * of the impulse response h[n] = sum_l b_l a_l^(n - d_l) [n >= d_l] of ONE template whose filters all run at

@@ -83,7 +83,8 @@ _SIGNATURES = {
                                          C.POINTER(C.c_int32)]),
     "spiir_fp32_peak_probe": (C.c_int, [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
     "spiir_signal_consistency": (C.c_int, [C.POINTER(spiir_snr_view), C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
-                                           C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
+                                           C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p,
+                                           C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
     "spiir_template_autocorr": (C.c_int, [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]),
     "spiir_last_error": (C.c_char_p, []),
 }
@@ -346,18 +347,21 @@ def template_autocorr(bank, t, n_j):
     return out
 
 
-def signal_consistency(view, delay_dev, trig, sky, n_slots, autocorr_dev, n_j, out=None):
+def signal_consistency(view, delay_dev, trig, sky, n_slots, autocorr_dev, n_j, out=None,
+                       n_slides=0, step=0, mult=None):
     """spiir_signal_consistency; delay_dev int32 cuda [n_pix][n_det], trig uint8 cuda [n_slots][40],
-    sky uint8 cuda [n_slots][16], autocorr_dev float32 cuda [rows][2 n_j + 1][2]; returns uint8 cuda
-    [n_slots][24] (XI2_DTYPE)."""
+    sky uint8 cuda [n_slots (* n_slides)][16], autocorr_dev float32 cuda [rows][2 n_j + 1][2]; returns uint8
+    cuda [n_slots (* n_slides)][24] (XI2_DTYPE)."""
     import torch
     n_pix, n_det = delay_dev.shape
     assert delay_dev.is_cuda and delay_dev.dtype == torch.int32 and delay_dev.is_contiguous()
     assert autocorr_dev.is_cuda and autocorr_dev.is_contiguous() and autocorr_dev.shape[-2] == 2 * n_j + 1
     if out is None:
-        out = torch.empty(n_slots, 24, dtype=torch.uint8, device="cuda")
+        out = torch.empty(n_slots * max(1, n_slides), 24, dtype=torch.uint8, device="cuda")
+    m = np.ascontiguousarray(mult if mult is not None else np.zeros(n_det), dtype=np.int32)
     _check(lib().spiir_signal_consistency(C.byref(view.c), n_det, n_pix, C.c_void_p(delay_dev.data_ptr()),
                                           C.c_void_p(trig.data_ptr()), C.c_void_p(sky.data_ptr()), n_slots,
+                                          n_slides, int(step), _hp(m),
                                           C.c_void_p(autocorr_dev.data_ptr()), n_j, C.c_void_p(out.data_ptr()),
                                           _stream()))
     return out

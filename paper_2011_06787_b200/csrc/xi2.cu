@@ -21,6 +21,7 @@ struct Xi2Params {
   const spiir_trigger* trig; const spiir_sky_result* sky; int32_t n_slots;
   const int32_t* delay; int32_t n_det, n_pix;
   const float2* acorr; int32_t nj;
+  int32_t n_slides; int64_t step; int32_t mult[SPIIR_MAX_DET];   // n_slides = 0: foreground
   spiir_xi2_result* out;
 };
 
@@ -32,14 +33,16 @@ __device__ __forceinline__ float warp_sum(float v) {
 
 __global__ void __launch_bounds__(kXiThreads) k_xi2(const __grid_constant__ Xi2Params P) {
   const int lane = threadIdx.x & 31;
-  const int i = blockIdx.x * (kXiThreads / 32) + (threadIdx.x >> 5);
-  if (i >= P.n_slots) return;
+  const int S1 = P.n_slides > 0 ? P.n_slides : 1;
+  const long long w = (long long)blockIdx.x * (kXiThreads / 32) + (threadIdx.x >> 5);   // (slot, slide)
+  if (w >= (long long)P.n_slots * S1) return;
+  const int i = (int)(w / S1), sl = (int)(w - (long long)i * S1) + (P.n_slides > 0 ? 1 : 0);
   spiir_xi2_result res;
   res.xi2_c = 0.f; res.used = 0;
 #pragma unroll
   for (int I = 0; I < SPIIR_MAX_DET; ++I) res.xi2[I] = 0.f;
   const spiir_trigger tr = P.trig[i];
-  const int pix = P.sky[i].pix;
+  const int pix = P.sky[w].pix;
   const int D = P.n_det, nj = P.nj, W = 2 * nj + 1;
   bool ok = tr.valid && pix >= 0 && pix < P.n_pix && tr.det >= 0 && tr.det < D;
   int64_t c[SPIIR_MAX_DET];
@@ -48,7 +51,7 @@ __global__ void __launch_bounds__(kXiThreads) k_xi2(const __grid_constant__ Xi2P
     const int32_t* dl = P.delay + (size_t)pix * D;
     const int dT = __ldg(dl + tr.det);
     for (int I = 0; I < D; ++I) {
-      c[I] = tr.k + (int64_t)__ldg(dl + I) - dT;
+      c[I] = tr.k + (int64_t)__ldg(dl + I) - dT - (I != tr.det ? (int64_t)sl * P.step * P.mult[I] : 0);
       ok = ok && c[I] - nj >= kmin && c[I] + nj <= P.k_newest;
     }
   }
@@ -82,7 +85,7 @@ __global__ void __launch_bounds__(kXiThreads) k_xi2(const __grid_constant__ Xi2P
     res.xi2_c = mean / (float)D;
     res.used = 1;
   }
-  if (lane == 0) P.out[i] = res;
+  if (lane == 0) P.out[w] = res;
 }
 
 }  // namespace spiir
@@ -93,12 +96,15 @@ extern "C" {
 
 int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t n_pix, const int32_t* dev_delay,
                              const spiir_trigger* dev_trig, const spiir_sky_result* dev_sky, int32_t n_slots,
+                             int32_t n_slides, int64_t step_samples, const int32_t* host_slide_mult,
                              const spiir_c32* dev_autocorr, int32_t n_j, spiir_xi2_result* dev_out, void* stream) {
   SPIIR_REQUIRE(view && dev_delay && dev_trig && dev_sky && dev_autocorr && dev_out, "a pointer is NULL");
   SPIIR_REQUIRE(view->dev_z && view->ring_len >= 1, "bad SNR view");
   SPIIR_REQUIRE(n_det >= 1 && n_det <= SPIIR_MAX_DET, "n_det %d out of range", n_det);
   SPIIR_REQUIRE(n_pix >= 1 && n_slots >= 0 && n_j >= 1, "bad n_pix / n_slots / n_j");
   SPIIR_REQUIRE(2 * (int64_t)n_j + 1 <= view->ring_len, "window of %d lags longer than the view", 2 * n_j + 1);
+  SPIIR_REQUIRE(n_slides >= 0 && (n_slides == 0 || (host_slide_mult && step_samples >= 0)),
+                "time slides need host_slide_mult and step >= 0");
   if (n_slots == 0) return SPIIR_OK;
   Xi2Params P;
   P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;
@@ -106,8 +112,11 @@ int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t 
   P.trig = dev_trig; P.sky = dev_sky; P.n_slots = n_slots;
   P.delay = dev_delay; P.n_det = n_det; P.n_pix = n_pix;
   P.acorr = (const float2*)dev_autocorr; P.nj = n_j; P.out = dev_out;
+  P.n_slides = n_slides; P.step = step_samples;
+  for (int I = 0; I < SPIIR_MAX_DET; ++I) P.mult[I] = (n_slides > 0 && I < n_det) ? host_slide_mult[I] : 0;
   const int wpb = kXiThreads / 32;
-  k_xi2<<<(n_slots + wpb - 1) / wpb, kXiThreads, 0, (cudaStream_t)stream>>>(P);
+  const long long n_w = (long long)n_slots * (n_slides > 0 ? n_slides : 1);
+  k_xi2<<<(unsigned)((n_w + wpb - 1) / wpb), kXiThreads, 0, (cudaStream_t)stream>>>(P);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());
   return SPIIR_OK;

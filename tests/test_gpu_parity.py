@@ -508,6 +508,20 @@ def test_xi2_signal_consistency(sp, U):
     assert np.all(xi["xi2"][~used] == 0) and np.all(xi["xi2_c"][~used] == 0)
     # noise candidates: a reduced chi^2 of order 1; not exactly 1, the windows are centred on maxima
     assert 0.5 < np.median(xi["xi2_c"][used]) < 1.5
+    # background events: one-second slides of the same candidates (chunk NC-2: slides 1 and 2 exist, 3 does not)
+    S = 3
+    bgs = plan.background(view, trig_dev, D * T, S, 2048, [1, 1, 1])
+    xib = sp.xi2_to_numpy(sp.signal_consistency(view, dl_dev, trig_dev, bgs, D * T, ac_dev, nj,
+                                                n_slides=S, step=2048, mult=[1, 1, 1])).reshape(D * T, S)
+    torch.cuda.synchronize()
+    rb = sp.results_to_numpy(bgs).reshape(D * T, S)
+    refb = oracle.xi2(delay, z, T * ring, ring, ring, k_newest, trig["valid"], trig["tmpl"], trig["det"], trig["k"],
+                      rb["pix"], acorr.astype(np.complex128), nj, n_slides=S, step=2048, slide_mult=[1, 1, 1])
+    assert np.array_equal(xib["used"], refb[:, :, D + 1].astype(np.int32))
+    assert xib["used"][:, 0].sum() >= 20 and xib["used"][:, 2].sum() == 0
+    assert np.all(np.abs(xib["xi2_c"] - refb[:, :, D]) <= 1e-4 * refb[:, :, D] + 1e-5)
+    for I in range(D):
+        assert np.all(np.abs(xib["xi2"][:, :, I] - refb[:, :, I]) <= 1e-4 * refb[:, :, I] + 1e-5)
     # a window that leaves the view (candidates of the newest chunk, k + 175 > k_newest for some) is refused
     tr2, _ = bk.peaks(0.0, 0)
     sky2 = plan.search(view, tr2, D * T)
