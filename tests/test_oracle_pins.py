@@ -594,3 +594,69 @@ def test_p21_xi2_on_time_slides():
     bg6 = oracle.xi2(delay, z, L, L, L, L - 1, pix=np.zeros((1, 6), np.int32), n_slides=6, step=step,
                      slide_mult=[1, 1, 1], **base)
     assert bg6[0, 5, D + 1] == 0 and np.all(bg6[0, 5] == 0) and np.all(bg6[0, :5, D + 1] == 1)
+
+
+# ---- NEXT-2: ranking statistic / FAP from the background (Eq. 13-15) ------------------
+def test_p22_pseudo_log_binning():
+    from oracle import rank
+    x = np.float32(2.0) ** np.arange(-20, 21, dtype=np.float32)
+    assert np.array_equal(rank.pseudo_log2(x), np.arange(-20, 21, dtype=np.float32))      # exact at powers of two
+    xs = np.sort(np.random.default_rng(22).uniform(1e-3, 1e4, 5000).astype(np.float32))
+    u = rank.pseudo_log2(xs)
+    assert np.all(np.diff(u) >= 0)                                                        # monotone
+    err = np.log2(xs.astype(np.float64)) - u
+    assert err.min() > -1e-6 and err.max() < 0.0861                                       # chord under the log, max gap 0.0860
+    assert abs(rank.pseudo_log2(np.float32([3.0]))[0] - 1.5) < 1e-7                       # 3 = 1.5 * 2^1 -> 1 + 0.5
+    # bins: 8 bins over u in [0, 4): x = 1, 2, 3, 4, 15.9, and the clamped outsiders 0.3, 16, 100, 0, -1
+    b = rank.bin_index(np.float32([1, 2, 3, 4, 15.9, 0.3, 16, 100, 0, -1]), 0.0, 4.0, 8)
+    assert b.tolist() == [0, 2, 3, 4, 7, 0, 7, 7, 0, 0]
+
+
+def test_p23_rank_and_fap_by_hand_and_by_counting_events():
+    from oracle import rank
+    # by hand: 2 x 2 bins (rho^2 axis u in [4, 8): edge at 2^6 = 64; xi^2 axis u in [-2, 2): edge at 1).
+    bins = (2, 2, 4.0, 8.0, -2.0, 2.0)
+    coh2 = np.float32([20, 30, 100, 150, 200, 70])          # rho-bins 0 0 1 1 1 1
+    xi2 = np.float32([0.5, 3.0, 0.5, 0.7, 2.0, 0.9])       # xi-bins  0 1 0 0 1 0
+    snr = np.float32([1, 1, 1, 1, 1, 1])
+    H = rank.histogram(bins, snr, coh2, xi2, np.ones(6, np.int32))
+    assert H.tolist() == [[1, 1], [3, 1]]
+    Cc = rank.rank_counts(H)
+    assert Cc.tolist() == [[4, 6], [3, 4]]                  # e.g. R(low rho, high xi) = everything = 6/6
+    F = rank.fap_counts(H, Cc)
+    assert F.tolist() == [[3, 5], [0, 3]]                   # bins with smaller R: (1,0) alone for C = 4; all but itself for C = 6
+    R, fap, far, sel = rank.candidates(bins, H, np.float32([1, 20]), np.float32([120, 120]), np.float32([0.6, 0.6]),
+                                       np.ones(2, np.int32), 50.0)
+    assert sel.tolist() == [1, 0] and R[0] == 3 / 6 and fap[0] == 0.0 and far[0] == 0.0 and R[1] == 0
+    # the cut rho_C >= rho_I + sqrt(2) decided in float32
+    s = np.float32(5.0)
+    edge = np.float32(s + np.float32(1.41421356)) ** 2
+    assert rank.select([s, s], [np.nextafter(edge, np.float32(100)), np.nextafter(edge, np.float32(0)) * np.float32(0.999)],
+                       [1, 1]).tolist() == [True, False]
+    assert rank.select([s], [edge * 2], [0]).tolist() == [False]
+    # by counting events: R and FAP from the event list itself, no histogram arithmetic
+    rng = np.random.default_rng(23)
+    n = 4000
+    coh2 = (rng.chisquare(4, n) + 30).astype(np.float32)
+    xi2 = (rng.chisquare(20, n) / 20).astype(np.float32)
+    snr = rng.uniform(4, 5.5, n).astype(np.float32)
+    used = (rng.random(n) < 0.9).astype(np.int32)
+    bins = (12, 9, 4.5, 7.0, -1.5, 1.5)
+    H = rank.histogram(bins, snr, coh2, xi2, used)
+    sel = rank.select(snr, coh2, used)
+    bi, bj = rank.bin_index(coh2, 4.5, 7.0, 12)[sel], rank.bin_index(xi2, -1.5, 1.5, 9)[sel]
+    assert H.sum() == sel.sum() and 0.1 * n < sel.sum() < n
+    Cc = rank.rank_counts(H)
+    for i in range(12):
+        for j in range(9):
+            assert Cc[i, j] == np.sum((bi >= i) & (bj <= j))
+    assert Cc[0, 8] == sel.sum() and np.all(np.diff(Cc, axis=0) <= 0) and np.all(np.diff(Cc, axis=1) >= 0)
+    F = rank.fap_counts(H, Cc)
+    r_event = Cc[bi, bj]
+    for i in range(12):
+        for j in range(9):
+            assert F[i, j] == np.sum(r_event < Cc[i, j])
+    # Eq. 14 is the cumulative distribution of R under the background: for background events themselves
+    # FAP + P(same R) / 2 is uniform-like, mean 1/2
+    same = np.array([np.sum(r_event == r) for r in r_event])
+    assert abs(np.mean((F[bi, bj] + 0.5 * same) / sel.sum()) - 0.5) < 1e-9
