@@ -406,7 +406,7 @@ def run_ours(args):
 
     # ---- NEXT-1 (outside the timed step): xi^2 of the last step's candidates (Eq. 11, 12), n_j = 175, on a
     #      seeded synthetic autocorrelation table (the arithmetic and the traffic do not depend on its values)
-    xi2_info = None
+    xi2_info = rank_info = None
     if has_sky:
         nj = 175
         g = torch.Generator(device="cpu").manual_seed(cfg["seed"])
@@ -444,6 +444,21 @@ def run_ours(args):
             ms_b = ex[0].elapsed_time(ex[1]) / 2.0
             xi2_info["slides"] = {"ms": ms_b, "events": n_bg,
                                   "algorithmic_GBps": n_bg * (D + 1) * (2 * nj + 1) * 8.0 / (ms_b * 1e-3) / 1e9}
+            # NEXT-2: the chunk's coherent background events into a 256 x 256 histogram, R / FAP tables, ranking
+            rk = sp.Ranker(256, 256, 4.0, 12.0, -3.0, 5.0)
+            rk_out = torch.empty(n_slots, 16, dtype=torch.uint8, device=dev)
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            for rep in range(3):
+                rk.reset()
+                ev[0].record(); rk.accumulate(prev, bg_out, xb_out, n_slots, S)
+                ev[1].record(); rk.finalize()
+                ev[2].record(); rk.candidates(prev, fg_out, xi_out, n_slots, float(S), out=rk_out)
+                ev[3].record()
+            torch.cuda.synchronize()
+            rr = sp.rank_to_numpy(rk_out)
+            rank_info = {"accumulate_ms": ev[0].elapsed_time(ev[1]), "finalize_ms": ev[1].elapsed_time(ev[2]),
+                                "candidates_ms": ev[2].elapsed_time(ev[3]), "bins": [256, 256],
+                                "background_events": rk.tables()[0], "coherent_candidates": int(rr["selected"].sum())}
             del xb_out
 
     # ---- end to end: pinned host strain in, host candidates and results out, every step
@@ -507,7 +522,7 @@ def run_ours(args):
         "per_step": {"updates": upd_chunk, "candidates": n_cand / K if has_sky else None,
                      "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
         "roofline": dominant, "roofline_other": other,
-        "next_rows": {"xi2": xi2_info},
+        "next_rows": {"xi2": xi2_info, "rank": rank_info},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -223,6 +223,36 @@ int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t 
 int spiir_template_autocorr(int64_t n_filters, const spiir_c32* host_a, const spiir_c32* host_b,
                             const int32_t* host_delay, int32_t n_j, spiir_c32* host_out);
 
+/* NEXT-2 — ranking statistic and false-alarm probability from the time-slide background
+ * (Sec. II D 1).  A background event (trigger, slide) or a foreground candidate is a
+ * *coherent event* iff rho_C >= rho_I + sqrt(2) (rho_C = sqrt(coh2), rho_I = trigger snr,
+ * decided in float32) and its xi^2 was evaluated (used = 1).  The probability P(rho_C, xi_C^2 | n) of
+ * Eq. 13 is a 2-D histogram of the coherent background events; the paper gives no binning: here both axes
+ * are uniform in the pseudo-logarithm u(x) = e + (m - 1) of x = m 2^e (m in [1, 2)), x = rho_C^2 on the
+ * first axis and xi_C^2 on the second, values outside [u_min, u_max) going to the edge bins.
+ *   R(bin)   = (1/N_b) sum of the histogram over bins with rho >= and xi^2 <= this bin's     (Eq. 13)
+ *   FAP(bin) = (1/N_b) sum of the histogram over bins whose R is smaller                     (Eq. 14)
+ *   FAR      = FAP N_b / T_b                                                                  (Eq. 15)
+ * Workspace layout (uint64): [0] N_b, [4 ..) histogram [n_rho][n_xi], then R counts, then FAP counts. */
+typedef struct { int32_t n_rho, n_xi; float u_rho_min, u_rho_max, u_xi_min, u_xi_max; } spiir_rank_bins;
+typedef struct { float rank, fap, far; int32_t selected; } spiir_rank_result;          /* 16 bytes */
+int spiir_rank_workspace_bytes(const spiir_rank_bins* bins, size_t* bytes);
+/* Empties the histogram (dev_ws: 16-byte aligned device memory of the queried size). */
+int spiir_rank_reset(void* dev_ws, const spiir_rank_bins* bins, void* stream);
+/* Adds the coherent events among dev_bg [n_slots][n_slides] (timeslide_background) with their
+ * dev_xi [n_slots][n_slides] (spiir_signal_consistency with the same slides) to the histogram. */
+int spiir_rank_accumulate(void* dev_ws, const spiir_rank_bins* bins, const spiir_trigger* dev_trig,
+                          const spiir_sky_result* dev_bg, const spiir_xi2_result* dev_xi, int32_t n_slots,
+                          int32_t n_slides, void* stream);
+/* Forms the R and FAP tables from the histogram as it stands (call after accumulating, before ranking). */
+int spiir_rank_finalize(void* dev_ws, const spiir_rank_bins* bins, void* stream);
+/* Ranks foreground candidates: dev_fg / dev_xi [n_slots] from coherent_sky_search and
+ * spiir_signal_consistency; background_seconds = T_b of Eq. 15 (collection time x number of slides);
+ * dev_out [n_slots]: zeros and selected = 0 for slots that are not coherent events. */
+int spiir_rank_candidates(const void* dev_ws, const spiir_rank_bins* bins, const spiir_trigger* dev_trig,
+                          const spiir_sky_result* dev_fg, const spiir_xi2_result* dev_xi, int32_t n_slots,
+                          double background_seconds, spiir_rank_result* dev_out, void* stream);
+
 /* Introspection: the layout chosen for a band (lanes per unit G, filters per lane
  * F, units, padded slots, shared-memory history depth) and counters for bench. */
 typedef struct {

@@ -54,7 +54,13 @@ TRIGGER_DTYPE = np.dtype([("valid", "<i4"), ("tmpl", "<i4"), ("det", "<i4"), ("_
                           ("z_re", "<f4"), ("z_im", "<f4"), ("snr", "<f4"), ("_pad2", "<f4")])
 RESULT_DTYPE = np.dtype([("coh2", "<f4"), ("null2", "<f4"), ("tot2", "<f4"), ("pix", "<i4")])
 XI2_DTYPE = np.dtype([("xi2_c", "<f4"), ("used", "<i4"), ("xi2", "<f4", (SPIIR_MAX_DET,))])
+RANK_DTYPE = np.dtype([("rank", "<f4"), ("fap", "<f4"), ("far", "<f4"), ("selected", "<i4")])
 assert TRIGGER_DTYPE.itemsize == 40 and RESULT_DTYPE.itemsize == 16 and XI2_DTYPE.itemsize == 24
+
+
+class spiir_rank_bins(C.Structure):
+    _fields_ = [("n_rho", C.c_int32), ("n_xi", C.c_int32), ("u_rho_min", C.c_float), ("u_rho_max", C.c_float),
+                ("u_xi_min", C.c_float), ("u_xi_max", C.c_float)]
 
 _SIGNATURES = {
     "spiir_bank_workspace_bytes": (C.c_int, [C.POINTER(spiir_bank_desc), C.POINTER(C.c_size_t)]),
@@ -85,6 +91,13 @@ _SIGNATURES = {
     "spiir_signal_consistency": (C.c_int, [C.POINTER(spiir_snr_view), C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
                                            C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p,
                                            C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
+    "spiir_rank_workspace_bytes": (C.c_int, [C.c_void_p, C.POINTER(C.c_size_t)]),
+    "spiir_rank_reset": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "spiir_rank_accumulate": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                        C.c_int32, C.c_void_p]),
+    "spiir_rank_finalize": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "spiir_rank_candidates": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                        C.c_double, C.c_void_p, C.c_void_p]),
     "spiir_template_autocorr": (C.c_int, [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]),
     "spiir_last_error": (C.c_char_p, []),
 }
@@ -369,3 +382,49 @@ def signal_consistency(view, delay_dev, trig, sky, n_slots, autocorr_dev, n_j, o
 
 def xi2_to_numpy(out):
     return out.cpu().numpy().view(XI2_DTYPE).reshape(-1)
+
+
+class Ranker:
+    """Owns the workspace of the background histogram (spiir_rank_*): accumulate -> finalize -> candidates."""
+
+    def __init__(self, n_rho, n_xi, u_rho_min, u_rho_max, u_xi_min, u_xi_max):
+        import torch
+        self.bins = spiir_rank_bins(n_rho, n_xi, u_rho_min, u_rho_max, u_xi_min, u_xi_max)
+        n = C.c_size_t(0)
+        _check(lib().spiir_rank_workspace_bytes(C.byref(self.bins), C.byref(n)))
+        self.ws = torch.empty(n.value // 8, dtype=torch.int64, device="cuda")
+        self.reset()
+
+    def _b(self):
+        return C.cast(C.byref(self.bins), C.c_void_p)
+
+    def reset(self):
+        _check(lib().spiir_rank_reset(C.c_void_p(self.ws.data_ptr()), self._b(), _stream()))
+
+    def accumulate(self, trig, bg, xi, n_slots, n_slides):
+        _check(lib().spiir_rank_accumulate(C.c_void_p(self.ws.data_ptr()), self._b(), C.c_void_p(trig.data_ptr()),
+                                           C.c_void_p(bg.data_ptr()), C.c_void_p(xi.data_ptr()), n_slots, n_slides,
+                                           _stream()))
+
+    def finalize(self):
+        _check(lib().spiir_rank_finalize(C.c_void_p(self.ws.data_ptr()), self._b(), _stream()))
+
+    def candidates(self, trig, fg, xi, n_slots, background_seconds, out=None):
+        import torch
+        if out is None:
+            out = torch.empty(n_slots, 16, dtype=torch.uint8, device="cuda")
+        _check(lib().spiir_rank_candidates(C.c_void_p(self.ws.data_ptr()), self._b(), C.c_void_p(trig.data_ptr()),
+                                           C.c_void_p(fg.data_ptr()), C.c_void_p(xi.data_ptr()), n_slots,
+                                           float(background_seconds), C.c_void_p(out.data_ptr()), _stream()))
+        return out
+
+    def tables(self):
+        """(N_b, H, R counts, FAP counts) as numpy int64 arrays [n_rho][n_xi]."""
+        w = self.ws.cpu().numpy()
+        n = self.bins.n_rho * self.bins.n_xi
+        shp = (self.bins.n_rho, self.bins.n_xi)
+        return int(w[0]), w[4:4 + n].reshape(shp), w[4 + n:4 + 2 * n].reshape(shp), w[4 + 2 * n:4 + 3 * n].reshape(shp)
+
+
+def rank_to_numpy(out):
+    return out.cpu().numpy().view(RANK_DTYPE).reshape(-1)

@@ -530,3 +530,74 @@ def test_xi2_signal_consistency(sp, U):
     ref2 = oracle.xi2(delay, z, T * ring, ring, ring, k_newest, t2["valid"], t2["tmpl"], t2["det"], t2["k"],
                       r2["pix"], acorr.astype(np.complex128), nj)
     assert np.array_equal(xi2b["used"], ref2[:, D + 1].astype(np.int32)) and (xi2b["used"] == 0).any()
+
+
+# ------------------------------------------------------------------ NEXT-2: ranking statistic, FAP, FAR (Eq. 13-15)
+def test_rank_statistic_fap_far(sp, U):
+    """spiir_rank_* against oracle/rank.py on seeded event lists shaped like the background of a chunk
+    (rho_C^2 = trigger power + chi^2_4, xi^2 reduced chi^2, 10 % unused, values planted exactly on bin and cut
+    edges).  Histogram, R counts and FAP counts are integers: bit-exact.  R / FAP / FAR of the candidates:
+    one float32 rounding of the same integer ratio."""
+    import torch
+    from oracle import rank
+    rng = np.random.default_rng(31)
+    n_slots, S = 700, 13
+    snr = rng.uniform(4.0, 7.0, n_slots).astype(np.float32)
+    trig = np.zeros(n_slots, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1; trig["snr"] = snr; trig["tmpl"] = np.arange(n_slots)
+    trig["valid"][::11] = 0
+
+    def events(n):
+        base = np.repeat(snr, n // n_slots) ** 2
+        coh2 = (base + rng.chisquare(4, n) * rng.uniform(0.5, 6.0, n)).astype(np.float32)
+        xi2 = (rng.chisquare(30, n) / 30 * rng.choice([1.0, 1.0, 3.0], n)).astype(np.float32)
+        used = (rng.random(n) < 0.9).astype(np.int32)
+        return coh2, xi2, used
+
+    bins = (48, 40, 4.0, 7.5, -1.0, 2.0)
+    coh2, xi2, used = events(n_slots * S)
+    # plant edge cases: exact bin edges (u integer and half-integer), exact cut edge, zeros, huge values
+    coh2[:6] = np.float32([16.0, 2.0 ** 7.5, 64.0, 181.01933, 1e9, 0.0])
+    xi2[:6] = np.float32([0.5, 1.0, 2.0, 4.0, 1e-9, 0.0])
+    edge = (np.float32(snr[1]) + np.float32(1.41421356)) ** 2
+    coh2[S], coh2[S + 1] = edge, np.nextafter(edge, np.float32(0))
+    used[S] = used[S + 1] = 1
+    bg = np.zeros(n_slots * S, sp.RESULT_DTYPE)
+    bg["coh2"] = coh2; bg["tot2"] = coh2; bg["pix"] = np.where(used == 1, 5, -1)
+    xi = np.zeros(n_slots * S, sp.XI2_DTYPE)
+    xi["xi2_c"] = xi2; xi["used"] = used
+    to_dev = lambda a: torch.from_numpy(a.view(np.uint8).reshape(len(a), -1).copy()).cuda()
+    rk = sp.Ranker(*bins)
+    td = to_dev(trig)
+    half = (n_slots // 2) * S                                 # two accumulate calls = one histogram
+    rk.accumulate(td, to_dev(bg[:half]), to_dev(xi[:half]), n_slots // 2, S)
+    rk.accumulate(to_dev(trig[n_slots // 2:]), to_dev(bg[half:]), to_dev(xi[half:]), n_slots - n_slots // 2, S)
+    rk.finalize()
+    torch.cuda.synchronize()
+    nb, H, Cc, F = rk.tables()
+    snr_ev = np.repeat(snr, S)
+    H_ref = rank.histogram(bins, snr_ev, coh2, xi2, used)
+    assert nb == H_ref.sum() and 0.2 * len(coh2) < nb < len(coh2)
+    assert np.array_equal(H, H_ref)
+    C_ref = rank.rank_counts(H_ref)
+    assert np.array_equal(Cc, C_ref)
+    assert np.array_equal(F, rank.fap_counts(H_ref, C_ref))
+    # foreground candidates
+    c2, x2, u2_ = events(n_slots)
+    c2[:40] *= 6.0                                            # some loud ones: R and FAP reach 0
+    fg = np.zeros(n_slots, sp.RESULT_DTYPE); fg["coh2"] = c2; fg["pix"] = np.where(u2_ == 1, 3, -1)
+    xf = np.zeros(n_slots, sp.XI2_DTYPE); xf["xi2_c"] = x2; xf["used"] = u2_
+    T_b = 13.0 * 7.0
+    out = sp.rank_to_numpy(rk.candidates(td, to_dev(fg), to_dev(xf), n_slots, T_b))
+    torch.cuda.synchronize()
+    R, fap, far, sel = rank.candidates(bins, H_ref, snr, c2, x2, u2_ * trig["valid"], T_b)
+    assert np.array_equal(out["selected"], sel) and 0.2 * n_slots < sel.sum() < n_slots
+    np.testing.assert_allclose(out["rank"], R, rtol=1e-6, atol=0)
+    np.testing.assert_allclose(out["fap"], fap, rtol=1e-6, atol=0)
+    np.testing.assert_allclose(out["far"], far, rtol=1e-6, atol=0)
+    assert (out["fap"][sel == 1] == 0).any() and (out["fap"][sel == 1] > 0.5).any()
+    # reset empties everything
+    rk.reset(); rk.finalize()
+    torch.cuda.synchronize()
+    nb0, H0, C0, F0 = rk.tables()
+    assert nb0 == 0 and not H0.any() and not C0.any() and not F0.any()
