@@ -660,3 +660,49 @@ def test_p23_rank_and_fap_by_hand_and_by_counting_events():
     # FAP + P(same R) / 2 is uniform-like, mean 1/2
     same = np.array([np.sum(r_event == r) for r in r_event])
     assert abs(np.mean((F[bi, bj] + 0.5 * same) / sel.sum()) - 0.5) < 1e-9
+
+
+# ---- P14: strain-domain injection through a chirp-matched template (end-to-end sanity, loose by nature) ----
+def test_p14_strain_injection_recovers_its_direction_or_the_mirror_image():
+    """BASELINE.json config 1: the chirp injected into three detectors with the true arrival delays, filtered
+    by the chirp-matched SPIIR template (O2-O3), searched over nside 16 (O5-O6).  With integer delays at
+    2048 Hz (A18) the maximum lands within ~2 pixel widths of the true direction or of its mirror image
+    through the plane of the three detectors; the true pixel is among the best few % and nearly as loud."""
+    cfg = workloads.config(1)
+    bank = workloads.bank_for_config(1, n_templates=1)                       # the chirp-matched template alone
+    st = workloads.strain_for_config(1)
+    inj = st["injections"][0]
+    z = oracle.filter_bank(st["strain"], bank)                               # [3][1][n]
+    k_true = int(round(inj["t_merge"] * 2048))
+    net = np.sum(np.abs(z[:, 0]) ** 2, axis=0)
+    # the loudest single-detector peak near the merger is the trigger
+    lo, hi = k_true - 400, k_true + 400
+    T = int(np.argmax([np.abs(z[I, 0, lo:hi]).max() for I in range(3)]))
+    k = lo + int(np.argmax(np.abs(z[T, 0, lo:hi])))
+    assert abs(k - k_true) < 100 and np.abs(z[T, 0, k]) > 6 and net[lo:hi].max() > 100   # network SNR 15 -> ~225
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    U2, delay = oracle.sky_table(16, pos, resp, cfg["sigma"], st["gmst"], 2048.0)
+    n = z.shape[2]
+    res, pix, mp = oracle.sky_search(U2.astype(np.float32), delay, z, n, n, n, n - 1, [1], [0], [T], [k],
+                                     want_map=True)
+    assert pix[0, 0] >= 0
+    theta, phi = oracle.healpix_ring_centres(16)
+    vec = np.stack([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)], axis=1)
+    tv = np.array([math.sin(inj["theta"]) * math.cos(inj["phi"]), math.sin(inj["theta"]) * math.sin(inj["phi"]),
+                   math.cos(inj["theta"])])
+    # mirror image through the plane of the three detectors (same delays): reflect the source vector, in the
+    # Earth-fixed frame the detector positions live in (longitude = phi - gmst)
+    def earth(v, sign):
+        c, s = math.cos(sign * st["gmst"]), math.sin(sign * st["gmst"])
+        return np.array([c * v[0] + s * v[1], -s * v[0] + c * v[1], v[2]])
+    nrm = np.cross(pos[1] - pos[0], pos[2] - pos[0]); nrm /= np.linalg.norm(nrm)
+    te = earth(tv, +1)
+    mv = earth(te - 2 * np.dot(te, nrm) * nrm, -1)
+    best = vec[pix[0, 0]]
+    ang = np.degrees(np.arccos(np.clip([best @ tv, best @ mv], -1, 1)))
+    assert ang.min() < 7.5, ang
+    p_true = int(np.argmax(vec @ tv))
+    rank_true = int(np.sum(mp[0] > mp[0, p_true]))
+    assert rank_true < 0.03 * len(vec)
+    assert math.sqrt(mp[0, p_true]) >= 0.97 * math.sqrt(res[0, 0, 0])
+    assert 12.0 < math.sqrt(res[0, 0, 0]) < 18.0                             # injected network SNR 15 in unit noise
