@@ -9,17 +9,21 @@
 //   * Eq. 28 writes rho_c^2 as the quadratic form z^H (U I U^T) z.  With
 //     integer delays only ~N_pix/14 distinct delay tuples exist at nside 64, and every
 //     direction of one tuple gathers the SAME samples.  The plan sorts the directions
-//     of each trigger detector T by delay tuple and packs them into a stream of
-//     32-slot chunks: a header slot per tuple (shared-memory rows to gather, number of
-//     directions, which detectors' rows changed since the previous header) followed
-//     by its direction slots (the projector M = U2 U2^T in the order the kernel
-//     consumes it, and the pixel).  Per tuple a thread forms the real products
-//     q_IJ = Re(z_I conj z_J) that changed; each direction then costs one N_q-term dot
-//     product (1 FMUL + 5 FFMA for three detectors) plus the running arg-max.
+//     of each trigger detector T by delay tuple into a stream of 32-slot chunks, one
+//     slot per direction: the projector M = U2 U2^T in the order the kernel consumes
+//     it, the pixel, and a control word (shared-memory rows to gather + which
+//     detectors' rows changed since the previous slot).  On a change a thread
+//     refreshes the real products q_IJ = Re(z_I conj z_J) the changed rows enter; each
+//     direction then costs one N_q-term dot product (1 FMUL + 5 FFMA for three
+//     detectors, issued for two pairs at a time as packed FFMA2 with the weight as a
+//     scalar-broadcast operand) and ONE FMNMX for the running maximum.  Which
+//     direction holds the maximum is recovered afterwards by rescanning the one chunk
+//     that last raised it.
 //   * thread = K (trigger, slide) pairs; a CTA owns 32 K pairs whose delay windows
 //     (the only samples any direction can touch) sit in shared memory, sample-major
-//     so that the per-tuple gather is conflict free; its warps split the chunk
-//     stream and stage each chunk through shared memory for broadcast reads.
+//     so that the per-tuple gather is conflict free (staged with cp.async); its warps
+//     take the stream's chunks round-robin and stage each chunk through shared memory
+//     for broadcast reads.
 //   * valid trigger slots are binned by trigger detector on the device (no host sync);
 //     one launch per trigger detector, persistent CTAs stride over the pair batches.
 #include <algorithm>
