@@ -325,7 +325,7 @@ def run_ours(args):
     cnt_host = torch.empty(1, dtype=torch.int32).pin_memory()
     state = {"i": 0}
 
-    def step(xin, events=None):
+    def step(xin, events=None, fg_out=fg_out, bg_out=bg_out):
         """One pass of the hot path over one chunk (every call goes through the C ABI)."""
         i = state["i"]
         cur, prev = trig[i & 1], trig[(i & 1) ^ 1]
@@ -470,22 +470,46 @@ def run_ours(args):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         if world > 1:
             dist.barrier()
+        # software-pipelined as a streaming caller would run it: the device->host copies of step j (on a copy
+        # stream, into the second of two host/device result sets) overlap the kernels of step j+1; the caller
+        # reads step j's results, complete on the host, while step j+1 runs.  Every step's strain comes from
+        # pinned host memory and every step's candidates and results reach the host inside the timed region.
+        copy_stream = torch.cuda.Stream(device=dev)
+        main = torch.cuda.current_stream()
+        dev_sets = [(fg_out, bg_out), (torch.zeros_like(fg_out), torch.zeros_like(bg_out))]
+        host_sets = [(trig_host, fg_host, bg_host, cnt_host),
+                     tuple(torch.empty_like(t).pin_memory() for t in (trig_host, fg_host, bg_host, cnt_host))]
+        done = [None, None]
+        torch.cuda.synchronize()
         e0.record()
         for j in range(K):
+            b = j & 1
+            if done[b] is not None:
+                main.wait_event(done[b])                             # result set b has been copied out
             x_in.copy_(x_host[(c0 + j) % n_chunks], non_blocking=True)
-            cur = step(x_in)
-            trig_host.copy_(cur, non_blocking=True)
-            cnt_host.copy_(counts[state["i"] - 1:state["i"]], non_blocking=True)
-            if has_sky:
-                fg_host.copy_(fg_out, non_blocking=True)
-                if S:
-                    bg_host.copy_(bg_out, non_blocking=True)
-            torch.cuda.current_stream().synchronize()                # the caller reads this step's results
+            cur = step(x_in, fg_out=dev_sets[b][0], bg_out=dev_sets[b][1])
+            ready = torch.cuda.Event()
+            ready.record(main)
+            th, fh, bh, ch = host_sets[b]
+            with torch.cuda.stream(copy_stream):
+                copy_stream.wait_event(ready)
+                th.copy_(cur, non_blocking=True)
+                ch.copy_(counts[state["i"] - 1:state["i"]], non_blocking=True)
+                if has_sky:
+                    fh.copy_(dev_sets[b][0], non_blocking=True)
+                    if S:
+                        bh.copy_(dev_sets[b][1], non_blocking=True)
+                done[b] = torch.cuda.Event()
+                done[b].record(copy_stream)
+            if j >= 1:
+                done[b ^ 1].synchronize()                            # the caller reads step j-1's results
+        done[(K - 1) & 1].synchronize()
         e1.record()
         torch.cuda.synchronize()
         ms_e2e = shd.max_over_ranks(e0.elapsed_time(e1), dev)
         e2e = {"value": world * upd_chunk * K / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e / K,
-               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "pipelining": "results of step j copied out on a second stream while step j+1 computes"}
         c0 += K
 
     ms_total = shd.max_over_ranks(ms_total, dev)
