@@ -21,9 +21,9 @@
 //     that last raised it.
 //   * thread = K (trigger, slide) pairs; a CTA owns 32 K pairs whose delay windows
 //     (the only samples any direction can touch) sit in shared memory, sample-major
-//     so that the per-tuple gather is conflict free (staged with cp.async); its warps
-//     take the stream's chunks round-robin and stage each chunk through shared memory
-//     for broadcast reads.
+//     so that the per-tuple gather is conflict free (staged with cp.async); each warp
+//     takes a contiguous share of the stream's chunks and stages each chunk through
+//     shared memory for broadcast reads.
 //   * valid trigger slots are binned by trigger detector on the device (no host sync);
 //     one launch per trigger detector, persistent CTAs stride over the pair batches.
 #include <algorithm>
@@ -51,13 +51,13 @@ template <int D> struct SkyFmt {
 //   2 M_To; 2 M_o'o for o' < o, (0,1) (0,2) (1,2).
 //   control = level | row_0 << 2 | row_1 << 12 | row_2 << 22: row_o = shared-memory window row of other
 //   detector o (already offset by its window's first row, < 1024); level = first other detector whose row
-//   differs from the previous slot of the SAME chunk (0 for a chunk's first slot: refresh everything;
-//   NO: same delay tuple, nothing to refresh).
+//   differs from the previous slot (0 for the first slot of a warp's share of the stream: refresh
+//   everything; NO: same delay tuple, nothing to refresh).
 // The last chunk is padded with copies of the last direction (level NO).
 constexpr int kSkyRowBits = 10;
 
 struct SkyParams {
-  const float* stream; int32_t n_chunks;                      // this trigger detector's stream
+  const float* stream; int32_t n_chunks, chunks_per_warp;     // this trigger detector's stream; contiguous share per warp
   int32_t n_pix;
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
   const spiir_trigger* trig;
@@ -107,8 +107,8 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
   const long long n_batches = (n_pairs + NP - 1) / NP;
   const int64_t kmin = (P.k_newest - P.ring_len + 1 > 0) ? P.k_newest - P.ring_len + 1 : 0;
   float* mytile = tiles + warp * kTileWords;
-  // chunks are dealt round-robin to the warps (tuple sizes vary slowly along the stream)
-  const int c_beg = warp, c_end = P.n_chunks;
+  // a contiguous share of chunks per warp: only a share's first slot has to refresh everything
+  const int c_beg = min(P.n_chunks, warp * P.chunks_per_warp), c_end = min(P.n_chunks, c_beg + P.chunks_per_warp);
 
   for (long long batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
     __syncthreads();                                   // previous batch fully consumed
@@ -183,13 +183,13 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
       for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
     }
-    for (int ch = c_beg; ch < c_end; ch += kSkyWarps) {
+    for (int ch = c_beg; ch < c_end; ++ch) {
       __syncwarp();
 #pragma unroll
       for (int c = 0; c < SW / 4; ++c) reinterpret_cast<float4*>(mytile + lane * SW)[c] = pre[c];
       __syncwarp();
-      if (ch + kSkyWarps < c_end) {                           // prefetch the next chunk while this one is consumed
-        const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)(ch + kSkyWarps) * kSkyChunk + lane) * SW);
+      if (ch + 1 < c_end) {                                   // prefetch the next chunk while this one is consumed
+        const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)(ch + 1) * kSkyChunk + lane) * SW);
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
       }
@@ -396,6 +396,7 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
       if (rows[(size_t)x * 3 + o] != rows[(size_t)y * 3 + o]) return rows[(size_t)x * 3 + o] < rows[(size_t)y * 3 + o];
     return x < y;
   });
+  const int cpw = (pl->cap_slots / kSkyChunk + kSkyWarps - 1) / kSkyWarps;   // chunks per warp
   slots.assign((size_t)pl->cap_slots * SW, 0.f);
   S.n_tuples = 0;
   for (int r = 0; r < pl->cap_slots; ++r) {
@@ -417,7 +418,7 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
     } else {
       ++S.n_tuples;
     }
-    if (r % kSkyChunk == 0) level = 0;     // chunks are processed independently of each other
+    if (r % (kSkyChunk * cpw) == 0) level = 0;   // a warp's share of the stream starts from nothing
     const float* u = u2 + (size_t)p * D * 2;
     auto M = [&](int I, int J) { return (double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]; };
     // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order
@@ -558,6 +559,7 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
     SkyParams P;
     memset(&P, 0, sizeof(P));
     P.stream = (const float*)(pl->ws + S.off_slots); P.n_chunks = S.n_chunks;
+    P.chunks_per_warp = (S.n_chunks + kSkyWarps - 1) / kSkyWarps;
     P.n_pix = pl->n_pix;
     P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;
     P.ring_len = view->ring_len; P.k_newest = view->k_newest;
