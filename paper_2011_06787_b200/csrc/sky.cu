@@ -45,12 +45,19 @@ template <int D> struct SkyFmt {
   static constexpr int NO = D - 1;                       // detectors other than the trigger detector
   static constexpr int NQ = D * (D + 1) / 2;             // independent entries of the projector
   static constexpr int SW = (NQ + 2 + 3) / 4 * 4;        // words per slot: NQ weights + pixel + control, padded to 16 B
+  static constexpr int FB = (D <= 3) ? 15 : 10;          // control-word field: element offset (15 bits) or row (10 bits)
 };
+// element offset of other detector o's row in the window region, from the control word
+template <int D> __device__ __forceinline__ int sky_row_elem(int ctrl, int o, int nps) {
+  const int f = (ctrl >> (2 + SkyFmt<D>::FB * o)) & ((1 << SkyFmt<D>::FB) - 1);
+  return (D <= 3) ? f : f * nps;
+}
 // One slot per direction, SW words: words [0,NQ) weights, word NQ = pixel, word NQ+1 = control.
 //   Weight order (T = trigger detector, o = others in increasing detector index): M_TT; M_oo (o = 0..NO-1);
 //   2 M_To; 2 M_o'o for o' < o, (0,1) (0,2) (1,2).
-//   control = level | row_0 << 2 | row_1 << 12 | row_2 << 22: row_o = shared-memory window row of other
-//   detector o (already offset by its window's first row, < 1024); level = first other detector whose row
+//   control = level | f_0 << 2 | f_1 << (2 + FB) | f_2 << (2 + 2 FB): f_o locates the shared-memory window row
+//   of other detector o (row counted from the first window's first row): the row's element offset row * nps
+//   in 15 bits for up to three detectors (no multiply in the kernel), the row itself in 10 bits for four; level = first other detector whose row
 //   differs from the previous slot (0 for the first slot of a warp's share of the stream: refresh
 //   everything; NO: same delay tuple, nothing to refresh).
 // The last chunk is padded with copies of the last direction (level NO).
@@ -67,6 +74,7 @@ struct SkyParams {
   int64_t step; int32_t mult[SPIIR_MAX_DET];
   int32_t lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];   // window of detector I vs T: first delta, width, first row
   int32_t win_elems;                                          // float2 elements of the window region
+  int32_t nps;                                                // float2 stride of a window row (32 k_max + 1)
   spiir_sky_result* out; float* map;
 };
 
@@ -93,7 +101,9 @@ __device__ __forceinline__ float quad_form(const float* __restrict__ w, const fl
 template <int D, int K, bool MAP>
 __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ SkyParams P) {
   constexpr int NO = SkyFmt<D>::NO, NQ = SkyFmt<D>::NQ, SW = SkyFmt<D>::SW;
-  constexpr int NP = 32 * K, NPS = NP + 1;
+  constexpr int NP = 32 * K;
+  constexpr int FB = SkyFmt<D>::FB;                    // bits of a control-word field
+  const int NPS = P.nps;
   constexpr int kTileWords = (kSkyChunk * SW > 2 * NP) ? kSkyChunk * SW : 2 * NP;   // a warp's chunk tile, reused for the reduction
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* win = reinterpret_cast<float2*>(smem_raw);                              // [rows][NPS]
@@ -212,8 +222,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
           for (int o = 0; o < NO; ++o) {
             if (level <= o) {
-              const int row = (ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1);
-              const float2* rp = win + (size_t)row * NPS + lane;
+              const float2* rp = win + sky_row_elem<D>(ctrl, o, NPS) + lane;
 #pragma unroll
               for (int a = 0; a < K; ++a) {
                 const float2 x = rp[32 * a];
@@ -296,8 +305,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         float tot = qq[0];
 #pragma unroll
         for (int o = 0; o < NO; ++o) {
-          const int row = (ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1);
-          const float2 x = win[(size_t)row * NPS + j];
+          const float2 x = win[sky_row_elem<D>(ctrl, o, NPS) + j];
           vv[o] = x;
           qq[1 + o] = re_prod(x, x);
           qq[1 + NO + o] = re_prod(pi.vT, x);
@@ -430,7 +438,8 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
     const int32_t pix = p;
     memcpy(w + NQ, &pix, 4);
     int32_t ctrl = level;
-    for (int o = 0; o < NO; ++o) ctrl |= rw[o] << (2 + kSkyRowBits * o);
+    const int fb = D <= 3 ? 15 : 10, nps = 32 * S.k_max + 1;
+    for (int o = 0; o < NO; ++o) ctrl |= (D <= 3 ? rw[o] * nps : rw[o]) << (2 + fb * o);
     memcpy(w + NQ + 1, &ctrl, 4);
   }
   S.n_chunks = pl->cap_slots / kSkyChunk;
@@ -483,7 +492,10 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
                 sky_smem_bytes(rows, pl->SW, 1), kSkySmemMax);
       delete pl; return SPIIR_EINVAL;
     }
-    if (rows >= (1 << kSkyRowBits)) { set_error("delay span of trigger detector %d: %d window rows (>= %d)", T, rows, 1 << kSkyRowBits); delete pl; return SPIIR_EINVAL; }
+    if (rows >= (1 << kSkyRowBits) || (D <= 3 && (long long)rows * (32 * S.k_max + 1) >= (1 << 15))) {
+      set_error("delay span of trigger detector %d: %d window rows do not fit the control word", T, rows);
+      delete pl; return SPIIR_EINVAL;
+    }
     sky_build_stream(pl, T, u2, delay, slots);
     cudaError_t e = cudaMemcpyAsync(pl->ws + S.off_slots, slots.data(), slots.size() * 4, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);     // the host images are reused for the next detector
@@ -572,9 +584,10 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
     // pairs per thread: as many as shared memory allows, fewer when the launch could not fill the SMs
     int K = S.k_max;
     while (K > 1 && max_pairs / D < (long long)pl->num_sms * 32 * K) --K;
-    P.win_elems = sky_win_elems(S.rows, K);
+    P.win_elems = sky_win_elems(S.rows, S.k_max);            // the plan's row stride whatever K runs
+    P.nps = 32 * S.k_max + 1;
     P.out = out; P.map = map;
-    const size_t smem = sky_smem_bytes(S.rows, pl->SW, K);
+    const size_t smem = sky_smem_bytes(S.rows, pl->SW, S.k_max);   // windows laid out with the plan's stride
     int rc;
     if (D == 2)      rc = map ? sky_launch_k<2, true>(K, P, max_pairs, pl->num_sms, smem, st) : sky_launch_k<2, false>(K, P, max_pairs, pl->num_sms, smem, st);
     else if (D == 3) rc = map ? sky_launch_k<3, true>(K, P, max_pairs, pl->num_sms, smem, st) : sky_launch_k<3, false>(K, P, max_pairs, pl->num_sms, smem, st);
