@@ -317,10 +317,9 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
 
 template <int G, int F>
 static int launch_one(const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det, int smem, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
+  static unsigned long long configured = 0;
+  if (first_use_on_device(configured)) {
     SPIIR_CUDA_OK(cudaFuncSetAttribute(k_bank<G, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    configured = true;
   }
   k_bank<G, F><<<dim3(n_cta, n_det), kBankThreads, smem, st>>>(P, dev_work);
   count_launch();
@@ -480,10 +479,9 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
 }
 
 void launch_combine(const CombineParams& p, int n_det, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
+  static unsigned long long configured = 0;
+  if (first_use_on_device(configured)) {
     cudaFuncSetAttribute(k_combine, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    configured = true;
   }
   const size_t smem = (size_t)(((p.bufA + p.bufB + 1) & ~1) + p.sb_total) * sizeof(float2);
   k_combine<<<dim3(p.T, n_det), kCombineThreads, smem, st>>>(p);

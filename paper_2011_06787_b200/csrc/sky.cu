@@ -523,10 +523,9 @@ int32_t spiir_sky_plan_tuples(const spiir_sky_plan* pl) { return pl ? pl->n_tupl
 
 template <int D, int K, bool MAP>
 static int sky_launch_one(const SkyParams& P, long long max_batches, int num_sms, size_t smem, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
+  static unsigned long long configured = 0;
+  if (first_use_on_device(configured)) {
     SPIIR_CUDA_OK(cudaFuncSetAttribute(k_sky<D, K, MAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSkySmemMax));
-    configured = true;
   }
   const int grid = (int)std::max<long long>(1, std::min<long long>(max_batches, num_sms));
   k_sky<D, K, MAP><<<grid, kSkyThreads, smem, st>>>(P);

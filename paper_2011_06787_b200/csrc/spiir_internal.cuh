@@ -14,6 +14,17 @@ namespace spiir {
 void set_error(const char* fmt, ...);
 void count_launch(int n = 1);
 
+// Function attributes (opt-in shared memory) are per device: true the first time a launch site runs on
+// the current device.
+inline bool first_use_on_device(unsigned long long& mask) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  const unsigned long long bit = 1ull << (dev & 63);
+  if (mask & bit) return false;
+  mask |= bit;
+  return true;
+}
+
 #define SPIIR_CUDA_OK(expr)                                                         \
   do {                                                                              \
     cudaError_t e_ = (expr);                                                        \
