@@ -351,6 +351,15 @@ def test_cfg4_full_size_sampled(sp, U):
     k_iso, v_iso = oracle.peaks_mode0(z_last.reshape(D * T, 2048), THR)
     assert np.array_equal(trig["k"] - (NC - 1) * 2048, k_iso) and np.array_equal(trig["valid"], v_iso)
     assert int(cnt.cpu()[0]) == int(v_iso.sum()) and v_iso.sum() > 0.2 * D * T
+    # the paper's two-step rule (mode 1) on the same chunk, banks of 1000 templates (A10), stage-isolated
+    tr1, cnt1 = bk.peaks(THR, 1)
+    torch.cuda.synchronize()
+    t1 = sp.triggers_to_numpy(tr1)
+    for d in range(D):
+        k1, v1 = oracle.peaks_mode1(z_last[d], THR, 1000)
+        td_ = t1[d * T:(d + 1) * T]
+        assert np.array_equal(td_["valid"], v1) and np.array_equal(td_["k"][v1 == 1] - (NC - 1) * 2048, k1[v1 == 1])
+    assert int(cnt1.cpu()[0]) == int(t1["valid"].sum()) > 100
     # end to end on the sampled templates (near-tie rule A12)
     rows = (np.arange(D)[:, None] * T + sel[None, :]).reshape(-1)
     U.check_peaks_mode0(_subset_trig(trig[rows], sel, D), z_sel[:, :, -2048:], z_ref[:, :, -2048:],
@@ -642,6 +651,14 @@ def test_cfg1_full(sp, U):
         n_near += U.check_peaks_mode0(trig, z[:, :, sl], z_ref[:, :, sl], c * 2048, 4.0)
         prev = (tr.clone(), trig)
     U.check_snr(z, z_ref)
+    tr1, cnt1 = bk.peaks(4.0, 1)                              # mode 1 on the last chunk, one bank of 512 (A10)
+    torch.cuda.synchronize()
+    t1 = sp.triggers_to_numpy(tr1)
+    for d in range(D):
+        k1, v1 = oracle.peaks_mode1(z[d][:, -2048:], 4.0, 512)
+        td_ = t1[d * T:(d + 1) * T]
+        assert np.array_equal(td_["valid"], v1) and np.array_equal(td_["k"][v1 == 1] - (NC - 1) * 2048, k1[v1 == 1])
+    assert int(cnt1.cpu()[0]) == int(t1["valid"].sum()) > 10
     assert n_cand > 3000                                      # ~36 % of the 1536 slots per second once the bank has filled
     print("cfg1 full: %d candidates searched, %d near-tie peak indices (A12), %d set-valued pixels (A19)"
           % (n_cand, n_near, n_pixdiff))
