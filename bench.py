@@ -461,6 +461,25 @@ def run_ours(args):
                                 "background_events": rk.tables()[0], "coherent_candidates": int(rr["selected"].sum())}
             del xb_out
 
+    # ---- the paper's own background grid (768 directions, nside 8) for the same candidates, outside
+    #      the timed step (reading A17 keeps the timed background on the foreground grid)
+    bg8_info = None
+    if has_sky and S:
+        u2b, delayb = sp.sky_table_build(8, pos, resp, cfg["sigma"], st["gmst"], 2048.0)
+        plan8 = sp.SkyPlan(u2b, delayb, max_slots=n_slots)
+        prev = trig[state["i"] & 1]
+        view = bk.snr_view()
+        eb = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        for rep in range(3):
+            if rep == 1: eb[0].record()
+            plan8.background(view, prev, n_slots, S, 2048, mult, out=bg_out)
+        eb[1].record()
+        torch.cuda.synchronize()
+        ms8 = eb[0].elapsed_time(eb[1]) / 2.0
+        n_c = int((sp.triggers_to_numpy(prev)["valid"] == 1).sum())
+        bg8_info = {"ms": ms8, "directions": 768, "evals_per_s": n_c * 768.0 * S / (ms8 * 1e-3),
+                    "note": "not part of the timed step"}
+
     # ---- end to end: pinned host strain in, host candidates and results out, every step
     e2e = None
     if not args.no_e2e:
@@ -547,6 +566,7 @@ def run_ours(args):
                      "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
         "roofline": dominant, "roofline_other": other,
         "next_rows": {"xi2": xi2_info, "rank": rank_info},
+        "background_on_paper_grid_nside8": bg8_info,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:
