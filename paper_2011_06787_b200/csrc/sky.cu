@@ -20,10 +20,11 @@
 //     direction holds the maximum is recovered afterwards by rescanning the one chunk
 //     that last raised it.
 //   * thread = K (trigger, slide) pairs; a CTA owns 32 K pairs whose delay windows
-//     (the only samples any direction can touch) sit in shared memory, sample-major
-//     so that the per-tuple gather is conflict free (staged with cp.async); each warp
-//     takes a contiguous share of the stream's chunks and stages each chunk through
-//     shared memory for broadcast reads.
+//     (the only samples any direction can touch) sit in shared memory, pair-major:
+//     one TMA bulk copy per (pair, detector) window (cp.async.bulk + mbarrier; 8-byte
+//     cp.async when the view is not 16-byte friendly); each warp takes a contiguous
+//     share of the stream's chunks and stages each chunk through shared memory for
+//     broadcast reads.
 //   * valid trigger slots are binned by trigger detector on the device (no host sync);
 //     one launch per trigger detector, persistent CTAs stride over the pair batches.
 #include <algorithm>
@@ -39,25 +40,19 @@ constexpr int kSkyThreads = 512;
 constexpr int kSkyWarps = kSkyThreads / 32;
 constexpr int kSkyChunk = 32;               // slots per stream chunk (one per lane when staging)
 constexpr int kSkyKMax = 4;                 // (trigger, slide) pairs per thread, at most
-constexpr int kSkySmemMax = 227 * 1024;     // opt-in dynamic shared memory per CTA on sm_100
+constexpr int kSkySmemMax = 226 * 1024;     // opt-in dynamic shared memory per CTA on sm_100 (227 KB) less the static part
 
 template <int D> struct SkyFmt {
   static constexpr int NO = D - 1;                       // detectors other than the trigger detector
   static constexpr int NQ = D * (D + 1) / 2;             // independent entries of the projector
   static constexpr int SW = (NQ + 2 + 3) / 4 * 4;        // words per slot: NQ weights + pixel + control, padded to 16 B
-  static constexpr int FB = (D <= 3) ? 15 : 10;          // control-word field: element offset (15 bits) or row (10 bits)
 };
-// element offset of other detector o's row in the window region, from the control word
-template <int D> __device__ __forceinline__ int sky_row_elem(int ctrl, int o, int nps) {
-  const int f = (ctrl >> (2 + SkyFmt<D>::FB * o)) & ((1 << SkyFmt<D>::FB) - 1);
-  return (D <= 3) ? f : f * nps;
-}
 // One slot per direction, SW words: words [0,NQ) weights, word NQ = pixel, word NQ+1 = control.
 //   Weight order (T = trigger detector, o = others in increasing detector index): M_TT; M_oo (o = 0..NO-1);
 //   2 M_To; 2 M_o'o for o' < o, (0,1) (0,2) (1,2).
-//   control = level | f_0 << 2 | f_1 << (2 + FB) | f_2 << (2 + 2 FB): f_o locates the shared-memory window row
-//   of other detector o (row counted from the first window's first row): the row's element offset row * nps
-//   in 15 bits for up to three detectors (no multiply in the kernel), the row itself in 10 bits for four; level = first other detector whose row
+//   control = level | f_0 << 2 | f_1 << 12 | f_2 << 22: f_o = element offset, inside a pair's block of
+//   windows, of the sample of other detector o this direction reads (segment offset + row, < 1024);
+//   level = first other detector whose row
 //   differs from the previous slot (0 for the first slot of a warp's share of the stream: refresh
 //   everything; NO: same delay tuple, nothing to refresh).
 // The last chunk is padded with copies of the last direction (level NO).
@@ -74,11 +69,13 @@ struct SkyParams {
   int64_t step; int32_t mult[SPIIR_MAX_DET];
   int32_t lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];   // window of detector I vs T: first delta, width, first row
   int32_t win_elems;                                          // float2 elements of the window region
-  int32_t nps;                                                // float2 stride of a window row (32 k_max + 1)
+  int32_t ps;                                                 // float2 elements of one pair's block of windows (even)
+  int32_t soff[SPIIR_MAX_DET];                                // offset of detector I's segment in the block (even)
+  int32_t tma;                                                // view is 16-byte friendly: stage with TMA bulk copies
   spiir_sky_result* out; float* map;
 };
 
-struct PairInfo { int32_t slot, slide, valid, row; float2 vT; long long k; };
+struct PairInfo { int32_t slot, slide, valid, row; float2 vT; long long k; unsigned char sh[8]; };   // sh[I]: 0/1 sample shift of detector I's window (TMA copies start 16-byte aligned)
 
 __device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src_gmem) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)),
@@ -102,11 +99,10 @@ template <int D, int K, bool MAP>
 __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ SkyParams P) {
   constexpr int NO = SkyFmt<D>::NO, NQ = SkyFmt<D>::NQ, SW = SkyFmt<D>::SW;
   constexpr int NP = 32 * K;
-  constexpr int FB = SkyFmt<D>::FB;                    // bits of a control-word field
-  const int NPS = P.nps;
+  const int PS = P.ps;                                 // float2 elements of a pair's block of windows
   constexpr int kTileWords = (kSkyChunk * SW > 2 * NP) ? kSkyChunk * SW : 2 * NP;   // a warp's chunk tile, reused for the reduction
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float2* win = reinterpret_cast<float2*>(smem_raw);                              // [rows][NPS]
+  float2* win = reinterpret_cast<float2*>(smem_raw);                              // [pair][PS]: a pair's windows, detector after detector
   float* tiles = reinterpret_cast<float*>(win + P.win_elems);                     // [warps][kTileWords]
   PairInfo* pinfo = reinterpret_cast<PairInfo*>(tiles + kSkyWarps * kTileWords);  // [NP]
 
@@ -119,6 +115,13 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
   float* mytile = tiles + warp * kTileWords;
   // a contiguous share of chunks per warp: only a share's first slot has to refresh everything
   const int c_beg = min(P.n_chunks, warp * P.chunks_per_warp), c_end = min(P.n_chunks, c_beg + P.chunks_per_warp);
+
+  __shared__ uint64_t bar;                             // completion of a batch's TMA window copies
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&bar)), "r"(NP * NO));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  uint32_t bar_phase = 0;
 
   for (long long batch = blockIdx.x; batch < n_batches; batch += gridDim.x) {
     __syncthreads();                                   // previous batch fully consumed
@@ -144,28 +147,72 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       pinfo[tid] = pi;
     }
     __syncthreads();
-    // ---- delay windows -> shared memory [row][pair] with cp.async (all copies of the batch in flight at
-    //      once); a warp copies one (pair, detector) window, its lanes reading consecutive ring samples
-    for (int task = warp; task < NP * NO; task += kSkyWarps) {
-      const int j = task / NO, o = task - j * NO;
-      const int I = o + (o >= T ? 1 : 0);
-      const PairInfo pi = pinfo[j];
-      const int W = P.W[I];
-      float2* dst = win + (size_t)P.woff[I] * NPS + j;
-      if (pi.valid) {
-        const int64_t k0 = pi.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I];
-        const int64_t base = k0 % P.ring_len;
-        const float2* src = P.z + (size_t)I * P.det_stride + (size_t)pi.row * P.row_stride;
-        for (int r = lane; r < W; r += 32) {
-          int64_t idx = base + r;
-          if (idx >= P.ring_len) idx -= P.ring_len;
-          cp_async_8(dst + (size_t)r * NPS, src + idx);
+    // ---- delay windows -> shared memory, pair-major.  With a 16-byte friendly view one thread per (pair,
+    //      detector) issues the window as one TMA bulk copy (two if it wraps the ring), starting at the
+    //      16-byte aligned sample at or before the window (sh = 0/1 samples of shift); completion on an
+    //      mbarrier.  Otherwise warps copy the windows with 8-byte cp.async.
+    if (P.tma) {
+      if (tid < NP * NO) {
+        const int j = tid / NO, o = tid - j * NO;
+        const int I = o + (o >= T ? 1 : 0);
+        const PairInfo pi = pinfo[j];
+        const uint32_t bar_a = (uint32_t)__cvta_generic_to_shared(&bar);
+        float2* dst = win + (size_t)j * PS + P.soff[I];
+        if (pi.valid) {
+          const int64_t k0 = pi.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I];
+          const int64_t base = k0 % P.ring_len;
+          const int sh = (int)(base & 1);
+          const int64_t idx0 = base - sh;
+          const int len = (P.W[I] + sh + 1) & ~1;                    // samples copied: even, covers the window
+          const int n1 = (int)min((int64_t)len, P.ring_len - idx0);  // before the ring's end (even: ring_len is even)
+          const float2* row = P.z + (size_t)I * P.det_stride + (size_t)pi.row * P.row_stride;
+          pinfo[j].sh[I] = (unsigned char)sh;
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a), "r"(len * 8) : "memory");
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                           (uint32_t)__cvta_generic_to_shared(dst)), "l"(row + idx0), "r"(n1 * 8), "r"(bar_a) : "memory");
+          if (n1 < len)
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                             (uint32_t)__cvta_generic_to_shared(dst + n1)), "l"(row), "r"((len - n1) * 8), "r"(bar_a) : "memory");
+        } else {
+          for (int r = 0; r < P.W[I] + 2; ++r) dst[r] = make_float2(0.f, 0.f);
+          pinfo[j].sh[I] = 0;
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar_a) : "memory");
         }
-      } else {
-        for (int r = lane; r < W; r += 32) dst[(size_t)r * NPS] = make_float2(0.f, 0.f);
       }
+      asm volatile(
+          "{\n"
+          ".reg .pred p;\n"
+          "SKY_WAIT:\n"
+          "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+          "@p bra SKY_DONE;\n"
+          "bra SKY_WAIT;\n"
+          "SKY_DONE:\n"
+          "}\n" ::"r"((uint32_t)__cvta_generic_to_shared(&bar)), "r"(bar_phase) : "memory");
+      bar_phase ^= 1u;
+    } else {
+      for (int task = warp; task < NP * NO; task += kSkyWarps) {
+        const int j = task / NO, o = task - j * NO;
+        const int I = o + (o >= T ? 1 : 0);
+        const PairInfo pi = pinfo[j];
+        const int W = P.W[I];
+        float2* dst = win + (size_t)j * PS + P.soff[I];
+        if (lane == 0) pinfo[j].sh[I] = 0;
+        if (pi.valid) {
+          const int64_t k0 = pi.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I];
+          const int64_t base = k0 % P.ring_len;
+          const float2* src = P.z + (size_t)I * P.det_stride + (size_t)pi.row * P.row_stride;
+          for (int r = lane; r < W; r += 32) {
+            int64_t idx = base + r;
+            if (idx >= P.ring_len) idx -= P.ring_len;
+            cp_async_8(dst + r, src + idx);
+          }
+        } else {
+          for (int r = lane; r < W; r += 32) dst[r] = make_float2(0.f, 0.f);
+        }
+      }
+      cp_async_wait_all();
     }
-    cp_async_wait_all();
     __syncthreads();
 
     // ---- the direction stream: this warp's chunks.  Only the running maximum is kept per direction
@@ -175,9 +222,12 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     float2 qp[(K + 1) / 2][NQ];                          // products of pairs (2i, 2i+1) side by side: packed FFMA2 operands
 #define SKY_Q(a, e) (((a) & 1) ? qp[(a) >> 1][e].y : qp[(a) >> 1][e].x)
     long long mrow[K];                                  // sky-map row of each pair, -1 = none
+    int pb[NO][K];                                      // element offset of pair a's block, plus the window's shift
 #pragma unroll
     for (int a = 0; a < K; ++a) {
       const PairInfo pi = pinfo[lane + 32 * a];
+#pragma unroll
+      for (int o = 0; o < NO; ++o) pb[o][a] = (lane + 32 * a) * PS + pi.sh[o + (o >= T ? 1 : 0)];
       vT[a] = pi.vT; best[a] = -1.f; seen[a] = -1.f; bch[a] = c_beg;
       mrow[a] = (MAP && pi.valid) ? (long long)pi.slot * P.n_pix : -1;
 #pragma unroll
@@ -222,10 +272,10 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
           for (int o = 0; o < NO; ++o) {
             if (level <= o) {
-              const float2* rp = win + sky_row_elem<D>(ctrl, o, NPS) + lane;
+              const float2* rp = win + ((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1));
 #pragma unroll
               for (int a = 0; a < K; ++a) {
-                const float2 x = rp[32 * a];
+                const float2 x = rp[pb[o][a]];
                 v[o][a] = x;
                 SKY_Q(a, 1 + o) = re_prod(x, x);
                 SKY_Q(a, 1 + NO + o) = re_prod(vT[a], x);
@@ -305,7 +355,8 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         float tot = qq[0];
 #pragma unroll
         for (int o = 0; o < NO; ++o) {
-          const float2 x = win[sky_row_elem<D>(ctrl, o, NPS) + j];
+          const float2 x = win[(size_t)j * PS + pi.sh[o + (o >= T ? 1 : 0)] +
+                               ((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1))];
           vv[o] = x;
           qq[1 + o] = re_prod(x, x);
           qq[1 + NO + o] = re_prod(pi.vT, x);
@@ -350,7 +401,8 @@ using namespace spiir;
 
 struct spiir_sky_stream {                 // the direction stream of one trigger detector
   int n_chunks = 0, n_tuples = 0, rows = 0, k_max = 0;
-  int lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];
+  int lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];   // woff: offset of the detector's segment in a pair's block
+  int ps = 0;                             // float2 elements of a pair's block (even)
   size_t off_slots = 0;
 };
 
@@ -364,10 +416,10 @@ struct spiir_sky_plan {
 
 static size_t sky_align(size_t x) { return (x + 255) / 256 * 256; }
 static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 2 + 3) / 4 * 4; }
-static int sky_win_elems(int rows, int K) { return (rows * (32 * K + 1) + 1) & ~1; }
-static size_t sky_smem_bytes(int rows, int SW, int K) {
+static int sky_win_elems(int ps, int K) { return ps * 32 * K; }          // ps is even
+static size_t sky_smem_bytes(int ps, int SW, int K) {
   const int NP = 32 * K, tile = std::max(kSkyChunk * SW, 2 * NP);
-  return (size_t)sky_win_elems(rows, K) * 8 + (size_t)kSkyWarps * tile * 4 + (size_t)NP * sizeof(PairInfo);
+  return (size_t)sky_win_elems(ps, K) * 8 + (size_t)kSkyWarps * tile * 4 + (size_t)NP * sizeof(PairInfo);
 }
 
 static void sky_layout(spiir_sky_plan* pl) {
@@ -438,8 +490,7 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
     const int32_t pix = p;
     memcpy(w + NQ, &pix, 4);
     int32_t ctrl = level;
-    const int fb = D <= 3 ? 15 : 10, nps = 32 * S.k_max + 1;
-    for (int o = 0; o < NO; ++o) ctrl |= (D <= 3 ? rw[o] * nps : rw[o]) << (2 + fb * o);
+    for (int o = 0; o < NO; ++o) ctrl |= rw[o] << (2 + kSkyRowBits * o);
     memcpy(w + NQ + 1, &ctrl, 4);
   }
   S.n_chunks = pl->cap_slots / kSkyChunk;
@@ -472,7 +523,7 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
   std::vector<float> slots;
   for (int T = 0; T < D; ++T) {
     spiir_sky_stream& S = pl->st[T];
-    int rows = 0;
+    int ps = 0;
     for (int I = 0; I < D; ++I) {
       int lo = INT_MAX, hi = INT_MIN;
       for (int p = 0; p < n_pix; ++p) {
@@ -480,20 +531,21 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
         if (d < -1000000 || d > 1000000) { set_error("pixel %d: delay difference %lld out of range", p, d); delete pl; return SPIIR_EINVAL; }
         lo = std::min(lo, (int)d); hi = std::max(hi, (int)d);
       }
-      S.lo[I] = lo; S.W[I] = hi - lo + 1; S.woff[I] = rows;
-      if (I != T) rows += S.W[I];
+      // a detector's segment: its window, one sample of alignment shift, rounded up to an even length
+      S.lo[I] = lo; S.W[I] = hi - lo + 1; S.woff[I] = ps;
+      if (I != T) ps += (S.W[I] + 3) & ~1;
     }
-    S.rows = rows;
+    S.rows = ps; S.ps = ps;
     S.k_max = 0;
     for (int K = kSkyKMax; K >= 1; --K)
-      if (sky_smem_bytes(rows, pl->SW, K) <= (size_t)kSkySmemMax) { S.k_max = K; break; }
+      if (sky_smem_bytes(ps, pl->SW, K) <= (size_t)kSkySmemMax) { S.k_max = K; break; }
     if (S.k_max == 0) {
       set_error("delay span of trigger detector %d needs %zu bytes of shared memory (> %d)", T,
-                sky_smem_bytes(rows, pl->SW, 1), kSkySmemMax);
+                sky_smem_bytes(ps, pl->SW, 1), kSkySmemMax);
       delete pl; return SPIIR_EINVAL;
     }
-    if (rows >= (1 << kSkyRowBits) || (D <= 3 && (long long)rows * (32 * S.k_max + 1) >= (1 << 15))) {
-      set_error("delay span of trigger detector %d: %d window rows do not fit the control word", T, rows);
+    if (ps >= (1 << kSkyRowBits)) {
+      set_error("delay span of trigger detector %d: %d window samples do not fit the control word", T, ps);
       delete pl; return SPIIR_EINVAL;
     }
     sky_build_stream(pl, T, u2, delay, slots);
@@ -583,10 +635,14 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
     // pairs per thread: as many as shared memory allows, fewer when the launch could not fill the SMs
     int K = S.k_max;
     while (K > 1 && max_pairs / D < (long long)pl->num_sms * 32 * K) --K;
-    P.win_elems = sky_win_elems(S.rows, S.k_max);            // the plan's row stride whatever K runs
-    P.nps = 32 * S.k_max + 1;
+    P.win_elems = sky_win_elems(S.ps, K);
+    P.ps = S.ps;
+    for (int I = 0; I < D; ++I) P.soff[I] = S.woff[I];
+    // TMA bulk copies need 16-byte aligned sources: an aligned base and even strides (in complex samples)
+    P.tma = (((uintptr_t)view->dev_z & 15) == 0 && view->det_stride % 2 == 0 && view->row_stride % 2 == 0 &&
+             view->ring_len % 2 == 0) ? 1 : 0;
     P.out = out; P.map = map;
-    const size_t smem = sky_smem_bytes(S.rows, pl->SW, S.k_max);   // windows laid out with the plan's stride
+    const size_t smem = sky_smem_bytes(S.ps, pl->SW, K);
     int rc;
     if (D == 2)      rc = map ? sky_launch_k<2, true>(K, P, max_pairs, pl->num_sms, smem, st) : sky_launch_k<2, false>(K, P, max_pairs, pl->num_sms, smem, st);
     else if (D == 3) rc = map ? sky_launch_k<3, true>(K, P, max_pairs, pl->num_sms, smem, st) : sky_launch_k<3, false>(K, P, max_pairs, pl->num_sms, smem, st);
