@@ -105,6 +105,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
   float2* win = reinterpret_cast<float2*>(smem_raw);                              // [pair][PS]: a pair's windows, detector after detector
   float* tiles = reinterpret_cast<float*>(win + P.win_elems);                     // [warps][kTileWords]
   PairInfo* pinfo = reinterpret_cast<PairInfo*>(tiles + kSkyWarps * kTileWords);  // [NP]
+  int* wchunk = reinterpret_cast<int*>(pinfo + NP);                               // [NP] chunk holding each pair's maximum
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int T = P.T;
@@ -321,33 +322,42 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       for (int a = 0; a < K; ++a) { red_c[lane + 32 * a] = best[a]; red_i[lane + 32 * a] = bch[a]; }
     }
     __syncthreads();
-    // ---- across the warps (first in stream order on exact ties); then a warp rescans the winning chunk
-    //      of one pair, lane = slot: every lane forms its own direction's products from scratch, the
-    //      first lane holding the maximum gives the direction, tot2 and null2 there (Eq. 10)
-    for (int j = warp; j < NP; j += kSkyWarps) {
+    // ---- across the warps: thread = pair, the first warp (= earliest chunks of the stream) wins exact ties
+    if (tid < NP) {
+      float bc = tiles[tid]; int bi = reinterpret_cast<const int*>(tiles + NP)[tid];
+#pragma unroll 4
+      for (int wv = 1; wv < kSkyWarps; ++wv) {
+        const float c = tiles[wv * kTileWords + tid];
+        const int i = reinterpret_cast<const int*>(tiles + wv * kTileWords + NP)[tid];
+        if (c > bc) { bc = c; bi = i; }
+      }
+      wchunk[tid] = min(bi, P.n_chunks - 1);
+    }
+    __syncthreads();
+    // ---- then a warp rescans the winning chunk of each of its 2 K pairs, lane = slot (the chunks of four
+    //      pairs are requested before the first is consumed): every lane forms its own direction's products
+    //      from scratch, the first lane holding the maximum gives the direction, tot2 and null2 there (Eq. 10)
+    constexpr int PPW = NP / kSkyWarps, RB = (PPW % 4 == 0) ? 4 : 2;
+    for (int u0 = 0; u0 < PPW; u0 += RB) {
+      float4 wv4[RB][SW / 4];
+#pragma unroll
+      for (int u = 0; u < RB; ++u) {
+        const float4* sp = reinterpret_cast<const float4*>(
+            P.stream + ((size_t)wchunk[warp + (u0 + u) * kSkyWarps] * kSkyChunk + lane) * SW);
+#pragma unroll
+        for (int c = 0; c < SW / 4; ++c) wv4[u][c] = __ldg(sp + c);
+      }
+#pragma unroll
+      for (int u = 0; u < RB; ++u) {
+      const int j = warp + (u0 + u) * kSkyWarps;
       const PairInfo pi = pinfo[j];
       if (pi.slot < 0) continue;
       spiir_sky_result res; res.coh2 = 0.f; res.null2 = 0.f; res.tot2 = 0.f; res.pix = -1;
       if (pi.valid) {
-        float bc = -2.f; int bi = 0;
-        if (lane < kSkyWarps) {
-          bc = tiles[lane * kTileWords + j];
-          bi = reinterpret_cast<const int*>(tiles + lane * kTileWords + NP)[j];
-        }
-        float m = bc;
-#pragma unroll
-        for (int o = 16; o; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-        bi = (bc == m) ? bi : INT_MAX;                       // exact ties: the earliest chunk of the stream
-#pragma unroll
-        for (int o = 16; o; o >>= 1) bi = min(bi, __shfl_xor_sync(0xffffffffu, bi, o));
         float w[SW];
-        {
-          const float4* sp = reinterpret_cast<const float4*>(P.stream + ((size_t)bi * kSkyChunk + lane) * SW);
 #pragma unroll
-          for (int c = 0; c < SW / 4; ++c) {
-            const float4 t = __ldg(sp + c);
-            w[4 * c] = t.x; w[4 * c + 1] = t.y; w[4 * c + 2] = t.z; w[4 * c + 3] = t.w;
-          }
+        for (int c = 0; c < SW / 4; ++c) {
+          w[4 * c] = wv4[u][c].x; w[4 * c + 1] = wv4[u][c].y; w[4 * c + 2] = wv4[u][c].z; w[4 * c + 3] = wv4[u][c].w;
         }
         const int ctrl = __float_as_int(w[NQ + 1]);
         float qq[NQ]; float2 vv[NO];
@@ -375,6 +385,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         res.null2 = fmaxf(res.tot2 - cm, 0.f);
       }
       if (lane == 0) P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
+      }
     }
   }
 }
@@ -419,7 +430,7 @@ static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 2 + 3) / 4 * 4; }
 static int sky_win_elems(int ps, int K) { return ps * 32 * K; }          // ps is even
 static size_t sky_smem_bytes(int ps, int SW, int K) {
   const int NP = 32 * K, tile = std::max(kSkyChunk * SW, 2 * NP);
-  return (size_t)sky_win_elems(ps, K) * 8 + (size_t)kSkyWarps * tile * 4 + (size_t)NP * sizeof(PairInfo);
+  return (size_t)sky_win_elems(ps, K) * 8 + (size_t)kSkyWarps * tile * 4 + (size_t)NP * (sizeof(PairInfo) + 4);
 }
 
 static void sky_layout(spiir_sky_plan* pl) {
