@@ -191,14 +191,29 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
           "SKY_DONE:\n"
           "}\n" ::"r"((uint32_t)__cvta_generic_to_shared(&bar)), "r"(bar_phase) : "memory");
       bar_phase ^= 1u;
+      // the copies landed with sample k0 at offset sh (0/1, from the source's alignment); move each window
+      // so that it starts at the parity its lane wants: lanes l and l+8 of a half-warp then hit distinct banks
+      for (int task = warp; task < NP * NO; task += kSkyWarps) {
+        const int j = task / NO, o = task - j * NO;
+        const int I = o + (o >= T ? 1 : 0);
+        const int sh = pinfo[j].sh[I], par = (j >> 3) & 1;
+        if (sh != par) {
+          float2* seg = win + (size_t)j * PS + P.soff[I];
+          float2 t[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) { const int r = lane + 32 * u; if (r < P.W[I]) t[u] = seg[sh + r]; }
+          __syncwarp();
+#pragma unroll
+          for (int u = 0; u < 4; ++u) { const int r = lane + 32 * u; if (r < P.W[I]) seg[par + r] = t[u]; }
+        }
+      }
     } else {
       for (int task = warp; task < NP * NO; task += kSkyWarps) {
         const int j = task / NO, o = task - j * NO;
         const int I = o + (o >= T ? 1 : 0);
         const PairInfo pi = pinfo[j];
         const int W = P.W[I];
-        float2* dst = win + (size_t)j * PS + P.soff[I];
-        if (lane == 0) pinfo[j].sh[I] = 0;
+        float2* dst = win + (size_t)j * PS + P.soff[I] + ((j >> 3) & 1);
         if (pi.valid) {
           const int64_t k0 = pi.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I];
           const int64_t base = k0 % P.ring_len;
@@ -223,12 +238,11 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     float2 qp[(K + 1) / 2][NQ];                          // products of pairs (2i, 2i+1) side by side: packed FFMA2 operands
 #define SKY_Q(a, e) (((a) & 1) ? qp[(a) >> 1][e].y : qp[(a) >> 1][e].x)
     long long mrow[K];                                  // sky-map row of each pair, -1 = none
-    int pb[NO][K];                                      // element offset of pair a's block, plus the window's shift
+    int pb[K];                                          // element offset of pair a's block, plus its windows' parity
 #pragma unroll
     for (int a = 0; a < K; ++a) {
       const PairInfo pi = pinfo[lane + 32 * a];
-#pragma unroll
-      for (int o = 0; o < NO; ++o) pb[o][a] = (lane + 32 * a) * PS + pi.sh[o + (o >= T ? 1 : 0)];
+      pb[a] = (lane + 32 * a) * PS + ((lane >> 3) & 1);
       vT[a] = pi.vT; best[a] = -1.f; seen[a] = -1.f; bch[a] = c_beg;
       mrow[a] = (MAP && pi.valid) ? (long long)pi.slot * P.n_pix : -1;
 #pragma unroll
@@ -276,7 +290,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
               const float2* rp = win + ((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1));
 #pragma unroll
               for (int a = 0; a < K; ++a) {
-                const float2 x = rp[pb[o][a]];
+                const float2 x = rp[pb[a]];
                 v[o][a] = x;
                 SKY_Q(a, 1 + o) = re_prod(x, x);
                 SKY_Q(a, 1 + NO + o) = re_prod(vT[a], x);
@@ -365,7 +379,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         float tot = qq[0];
 #pragma unroll
         for (int o = 0; o < NO; ++o) {
-          const float2 x = win[(size_t)j * PS + pi.sh[o + (o >= T ? 1 : 0)] +
+          const float2 x = win[(size_t)j * PS + ((j >> 3) & 1) +
                                ((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1))];
           vv[o] = x;
           qq[1 + o] = re_prod(x, x);
@@ -546,6 +560,7 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
       S.lo[I] = lo; S.W[I] = hi - lo + 1; S.woff[I] = ps;
       if (I != T) ps += (S.W[I] + 3) & ~1;
     }
+    if (ps % 4 == 0) ps += 2;               // ps / 2 odd: a half-warp's 16 blocks start on distinct bank pairs
     S.rows = ps; S.ps = ps;
     S.k_max = 0;
     for (int K = kSkyKMax; K >= 1; --K)
@@ -555,6 +570,8 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
                 sky_smem_bytes(ps, pl->SW, 1), kSkySmemMax);
       delete pl; return SPIIR_EINVAL;
     }
+    for (int I = 0; I < D; ++I)
+      if (I != T && S.W[I] > 128) { set_error("delay window of %d samples (detector %d vs %d) exceeds 128", S.W[I], I, T); delete pl; return SPIIR_EINVAL; }
     if (ps >= (1 << kSkyRowBits)) {
       set_error("delay span of trigger detector %d: %d window samples do not fit the control word", T, ps);
       delete pl; return SPIIR_EINVAL;
