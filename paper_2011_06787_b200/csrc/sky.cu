@@ -148,6 +148,14 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       pinfo[tid] = pi;
     }
     __syncthreads();
+    // the warp's first chunk of the direction stream does not depend on the batch: request it now, it arrives
+    // while the windows are staged
+    float4 pre[SW / 4];
+    if (c_beg < c_end) {
+      const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)c_beg * kSkyChunk + lane) * SW);
+#pragma unroll
+      for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
+    }
     // ---- delay windows -> shared memory, pair-major.  With a 16-byte friendly view one thread per (pair,
     //      detector) issues the window as one TMA bulk copy (two if it wraps the ring), starting at the
     //      16-byte aligned sample at or before the window (sh = 0/1 samples of shift); completion on an
@@ -252,12 +260,6 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       for (int o = 0; o < NO; ++o) v[o][a] = make_float2(0.f, 0.f);
     }
 
-    float4 pre[SW / 4];
-    if (c_beg < c_end) {
-      const float4* src = reinterpret_cast<const float4*>(P.stream + ((size_t)c_beg * kSkyChunk + lane) * SW);
-#pragma unroll
-      for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
-    }
     for (int ch = c_beg; ch < c_end; ++ch) {
       __syncwarp();
 #pragma unroll
