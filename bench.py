@@ -43,7 +43,7 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 FP32_LANE_OPS_PER_S = 148 * 128 * 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/); None until a capture exists for the kernel.
-NCU_TRAFFIC_BYTES = {"k_bank": 4.43e9, "k_sky": 2.19e9}   # profiles/r1_ncu_summary.md sections 3 and 2 (mean of the three slide launches)
+NCU_TRAFFIC_BYTES = {"k_bank": 4.43e9, "k_sky": 2.20e9}   # profiles/r1_ncu_summary.md sections 3 and 2 (mean of the three slide launches)
 
 
 def parse_args():
