@@ -379,21 +379,32 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
   float2* sbuf = cbuf + ((p.bufA + p.bufB + 1) & ~1);   // the template's band sums of this chunk, all bands (16-byte aligned)
   const int B = p.B, ob = p.out_band;
 
-  // stage every band's sums at once (one round of HBM latency for the whole template): a template with
-  // one unit in a band is copied asynchronously, more units are added up on the way
+  // stage every band's sums at once (one round of HBM latency for the whole template): a template with one
+  // unit in a band gets that row as ONE TMA bulk copy (thread 0 issues them, completion on an mbarrier: the
+  // LSU path of per-thread cp.async tops out near 14 GB/s per SM here), more units are added up on the way
+  __shared__ uint64_t cbar;
+  if (tid == 0) mbar_init(&cbar, 1);
+  __syncthreads();
+  if (tid == 0) {
+    uint32_t bytes = 0;
+    for (int b = 0; b < B; ++b)
+      if (p.tb_count[t * B + b] == 1) bytes += (uint32_t)p.sb_n[b] * 8u;
+    mbar_expect_tx(&cbar, bytes);
+    for (int b = 0; b < B; ++b)
+      if (p.tb_count[t * B + b] == 1)
+        tma_load_1d(sbuf + p.sb_off[b],
+                    p.S[b] + (size_t)det * p.S_det_stride[b] + (size_t)p.tb_first[t * B + b] * p.nmax[b],
+                    (uint32_t)p.sb_n[b] * 8u, &cbar);
+  }
   for (int b = 0; b < B; ++b) {
     const int ns = p.sb_n[b];                           // samples k_bank stored for this band (n, or n/2 if odd-only)
     const float2* S = p.S[b] + (size_t)det * p.S_det_stride[b];
     const int first = p.tb_first[t * B + b], count = p.tb_count[t * B + b];
     float2* dst = sbuf + p.sb_off[b];
-    if (count == 1) {
-      const float2* row = S + (size_t)first * p.nmax[b];
-      for (int j = tid; j < ns / 2; j += kCombineThreads) cp_async_16(dst + 2 * j, row + 2 * j);
-    } else {
+    if (count != 1)
       for (int m = tid; m < ns; m += kCombineThreads) dst[m] = unit_sum(S, p.nmax[b], first, count, m);
-    }
   }
-  asm volatile("cp.async.wait_all;" ::: "memory");
+  mbar_wait(&cbar, 0);
   __syncthreads();
 
   // acc_{B-1} = s_{B-1}, then acc_b = s_b + up2(acc_{b+1}) down to the output band
