@@ -207,12 +207,17 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         const int sh = pinfo[j].sh[I], par = (j >> 3) & 1;
         if (sh != par) {
           float2* seg = win + (size_t)j * PS + P.soff[I];
-          float2 t[4];
+          const int W = P.W[I], nblk = (W + 127) >> 7;
+          for (int bq = 0; bq < nblk; ++bq) {              // 128 samples at a time, in the direction that never
+            const int r0 = ((par < sh) ? bq : nblk - 1 - bq) << 7;   // overwrites a sample still to be moved
+            float2 t[4];
 #pragma unroll
-          for (int u = 0; u < 4; ++u) { const int r = lane + 32 * u; if (r < P.W[I]) t[u] = seg[sh + r]; }
-          __syncwarp();
+            for (int u = 0; u < 4; ++u) { const int r = r0 + lane + 32 * u; if (r < W) t[u] = seg[sh + r]; }
+            __syncwarp();
 #pragma unroll
-          for (int u = 0; u < 4; ++u) { const int r = lane + 32 * u; if (r < P.W[I]) seg[par + r] = t[u]; }
+            for (int u = 0; u < 4; ++u) { const int r = r0 + lane + 32 * u; if (r < W) seg[par + r] = t[u]; }
+            __syncwarp();
+          }
         }
       }
     } else {
@@ -572,8 +577,6 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
                 sky_smem_bytes(ps, pl->SW, 1), kSkySmemMax);
       delete pl; return SPIIR_EINVAL;
     }
-    for (int I = 0; I < D; ++I)
-      if (I != T && S.W[I] > 128) { set_error("delay window of %d samples (detector %d vs %d) exceeds 128", S.W[I], I, T); delete pl; return SPIIR_EINVAL; }
     if (ps >= (1 << kSkyRowBits)) {
       set_error("delay span of trigger detector %d: %d window samples do not fit the control word", T, ps);
       delete pl; return SPIIR_EINVAL;

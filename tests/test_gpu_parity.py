@@ -702,3 +702,44 @@ def test_cfg2_full(sp, U):
     frac = np.mean([t["valid"].mean() for t in trigs[NC // 2:]])
     assert 0.1 < frac < 0.9
     print("cfg2 full: max |dz| %.2e, %d near-tie peak indices (A12), trigger fraction %.2f" % (worst, n_near, frac))
+
+
+# ------------------------------------------------------------------ four detectors
+def test_sky_four_detectors(sp, U):
+    """N_d = 4 (the library's maximum): H1, L1, V1 and a fourth site built from seeded geometry (a detector's
+    position and arm tensor are inputs of the table, A27).  Foreground with sky map, time slides, ring
+    wrap-around - against the oracle.  With four detectors the null stream has 4 degrees of freedom."""
+    import torch
+    cfg = workloads.config(3)
+    pos3, resp3 = workloads.detector_geometry(cfg["dets"])
+    rng = np.random.default_rng(44)
+    v = rng.standard_normal(3); v *= 6.37e6 / np.linalg.norm(v)              # somewhere on the Earth's surface
+    x = np.cross(v, rng.standard_normal(3)); x /= np.linalg.norm(x)
+    y = np.cross(v, x); y /= np.linalg.norm(y)
+    pos = np.vstack([pos3, v[None]])
+    resp = np.concatenate([resp3, (0.5 * (np.outer(x, x) - np.outer(y, y)))[None]])
+    U2, delay = oracle.sky_table(8, pos, resp, [1.0, 1.0, 0.5, 0.7], 1.1, 2048.0)
+    u2 = U2.astype(np.float32)
+    rows, L, S, step = 150, 1400, 5, 200
+    z = rng.standard_normal((4, rows, L, 2)).astype(np.float32)
+    zc = z.view(np.complex64)[..., 0]
+    k_newest = 2 * L + 77                                                     # the view is a ring that has wrapped twice
+    trig = np.zeros(rows, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1; trig["tmpl"] = np.arange(rows); trig["det"] = rng.integers(0, 4, rows)
+    trig["k"] = rng.integers(k_newest - 200, k_newest - 70, rows)
+    plan = sp.SkyPlan(u2, delay, max_slots=rows)
+    view = sp.SnrView(torch.from_numpy(z).cuda(), k_newest=k_newest)
+    td = sp.triggers_from_numpy(trig)
+    smap = torch.empty(rows, plan.n_pix, dtype=torch.float32, device="cuda")
+    res = sp.results_to_numpy(plan.search(view, td, rows, skymap=smap))
+    bg = sp.results_to_numpy(plan.background(view, td, rows, S, step, [1, 2, 1, 1]))
+    torch.cuda.synchronize()
+    ref = U.oracle_sky_on(zc, L, k_newest, u2, delay, trig, want_map=True)
+    U.check_sky(res, zc, L, k_newest, u2, delay, trig, ref=ref)
+    assert (res["pix"] >= 0).sum() > 100
+    m = smap.cpu().numpy()
+    tot = np.maximum(ref[0][:, 0, 2], 1.0)[:, None]
+    assert np.all(np.abs(m - ref[2]) <= 1e-4 * ref[2] + 2e-6 * tot)
+    U.check_sky(bg, zc, L, k_newest, u2, delay, trig, n_slides=S, step=step, mult=[1, 2, 1, 1])
+    ok = res["pix"] >= 0
+    assert 2.0 < np.mean(res["null2"][ok]) < 6.0 * 1.5                        # ~ (2 N_d - 4) = 4 dof at the arg-max, minus selection
