@@ -541,6 +541,10 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (+ the other one), FP32 probe, CPU baseline
     ffma_rate, _ = sp.fp32_peak_probe(20)
+    probes = {"unit": "fraction of the nominal FP32 lane rate (148 SM x 128 lanes x 1.965 GHz), register-only loops",
+              "recursion_mix_k_bank": sp.pipe_probe(1) / FP32_LANE_OPS_PER_S,
+              "quadratic_form_packed_ffma2": sp.pipe_probe(2) / FP32_LANE_OPS_PER_S,
+              "quadratic_form_scalar_ffma": sp.pipe_probe(3) / FP32_LANE_OPS_PER_S}
     ms_sky = stage[2] + stage[3]
     roof_bank = alu_roofline("k_bank (IIR recursion, H1+H2)", FLOP_PER_UPDATE * upd_chunk * n_rec, ms_rec,
                              n_rec * len_groups(bk), ffma_rate, NCU_TRAFFIC_BYTES["k_bank"],
@@ -564,7 +568,7 @@ def run_ours(args):
                         "sky_evals_per_s": (evals / (ms_sky * 1e-3)) if (has_sky and ms_sky > 0) else None},
         "per_step": {"updates": upd_chunk, "candidates": n_cand / K if has_sky else None,
                      "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
-        "roofline": dominant, "roofline_other": other,
+        "roofline": dominant, "roofline_other": other, "pipe_probes": probes,
         "next_rows": {"xi2": xi2_info, "rank": rank_info},
         "background_on_paper_grid_nside8": bg8_info,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     make_desc, Bank, SkyPlan, SnrView, sky_table_build,
     triggers_to_numpy, triggers_from_numpy, results_to_numpy, fp32_peak_probe,
     XI2_DTYPE, template_autocorr, signal_consistency, xi2_to_numpy,
-    RANK_DTYPE, spiir_rank_bins, Ranker, rank_to_numpy,
+    RANK_DTYPE, spiir_rank_bins, Ranker, rank_to_numpy, pipe_probe,
     SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EOVERFLOW,
 )
 from . import binding as _b

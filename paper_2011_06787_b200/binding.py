@@ -88,6 +88,7 @@ _SIGNATURES = {
     "spiir_bank_timing_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                          C.POINTER(C.c_int32)]),
     "spiir_fp32_peak_probe": (C.c_int, [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
+    "spiir_pipe_probe": (C.c_int, [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
     "spiir_signal_consistency": (C.c_int, [C.POINTER(spiir_snr_view), C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
                                            C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p,
                                            C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
@@ -428,3 +429,10 @@ class Ranker:
 
 def rank_to_numpy(out):
     return out.cpu().numpy().view(RANK_DTYPE).reshape(-1)
+
+
+def pipe_probe(mode, reps=5):
+    """FP32 lane-operations/s of a register-only copy of a hot inner loop (spiir_pipe_probe)."""
+    ms, ops = C.c_double(0), C.c_double(0)
+    _check(lib().spiir_pipe_probe(mode, reps, C.byref(ms), C.byref(ops), _stream()))
+    return ops.value * reps / (ms.value * 1e-3)
