@@ -631,7 +631,7 @@ def test_cfg1_full(sp, U):
     xs = torch.from_numpy(x).cuda()
     z = np.zeros((D, T, NC * 2048), np.complex64)
     out = torch.empty(D, T, 2048, 2, dtype=torch.float32, device="cuda")
-    prev, n_cand, n_near, n_pixdiff = None, 0, 0, 0
+    prev, n_cand, n_near, n_pixdiff, n_e2e = None, 0, 0, 0, 0
     for c in range(NC):
         bk.filter_chunk(xs[:, c * 2048:(c + 1) * 2048].contiguous(), out)
         z[:, :, c * 2048:(c + 1) * 2048] = out.cpu().numpy().view(np.complex64)[..., 0]
@@ -644,6 +644,22 @@ def test_cfg1_full(sp, U):
             zr[:, :, kk % ring] = z[:, :, kk]
             n_pixdiff += U.check_sky(res, zr, ring, k_newest, u2, delay, prev[1])["pix_differs"]
             n_cand += int((res["pix"] >= 0).sum())
+            # end to end with NOTHING from the CUDA path on the oracle's side: float64 SNR -> O4 -> O6, compared
+            # where both sides chose the same sample (they all do unless a near-tie, A12)
+            zr64 = np.zeros((D, T, ring), np.complex128)
+            zr64[:, :, kk % ring] = z_ref[:, :, kk]
+            slp = slice((c - 1) * 2048, c * 2048)
+            k_o, v_o = oracle.peaks_mode0(z_ref[:, :, slp].reshape(D * T, 2048), 4.0)
+            same = (v_o == 1) & (prev[1]["valid"] == 1) & (k_o + (c - 1) * 2048 == prev[1]["k"])
+            ref_e, pix_e, map_e = oracle.sky_search(u2, delay, zr64, T * ring, ring, ring, k_newest, same.astype(np.int32),
+                                                    prev[1]["tmpl"], prev[1]["det"], prev[1]["k"], want_map=True)
+            idx = np.nonzero(same & (pix_e[:, 0] >= 0))[0]
+            assert len(idx) > 0.9 * (prev[1]["valid"] == 1).sum() - 5 and np.all(res["pix"][idx] >= 0)
+            cg, ce = res["coh2"][idx].astype(np.float64), ref_e[idx, 0, 0]
+            assert np.all(np.abs(np.sqrt(cg) - np.sqrt(ce)) <= 1e-3) and np.all(np.abs(cg - ce) <= 1e-4 * ce + 1e-5)
+            at_gpu_pix = map_e[idx, res["pix"][idx]]
+            assert np.all(at_gpu_pix >= ce - np.maximum(1e-4 * ce, 1e-3))                  # A19 with the float64 map
+            n_e2e += len(idx)
         tr, cnt = bk.peaks(4.0, 0)
         torch.cuda.synchronize()
         trig = sp.triggers_to_numpy(tr).copy()
@@ -660,8 +676,9 @@ def test_cfg1_full(sp, U):
         assert np.array_equal(td_["valid"], v1) and np.array_equal(td_["k"][v1 == 1] - (NC - 1) * 2048, k1[v1 == 1])
     assert int(cnt1.cpu()[0]) == int(t1["valid"].sum()) > 10
     assert n_cand > 3000                                      # ~36 % of the 1536 slots per second once the bank has filled
-    print("cfg1 full: %d candidates searched, %d near-tie peak indices (A12), %d set-valued pixels (A19)"
-          % (n_cand, n_near, n_pixdiff))
+    assert n_e2e > 0.95 * n_cand
+    print("cfg1 full: %d candidates searched (%d compared end to end with the float64 chain), %d near-tie peak "
+          "indices (A12), %d set-valued pixels (A19)" % (n_cand, n_e2e, n_near, n_pixdiff))
 
 
 def test_cfg2_full(sp, U):
