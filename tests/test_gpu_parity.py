@@ -381,6 +381,20 @@ def test_cfg4_full_size_sampled(sp, U):
     assert sub["valid"].sum() >= 8
     U.check_sky(fg[rows], zr, ring, k_newest, u2, delay, sub)
     U.check_sky(bg[rows], zr, ring, k_newest, u2, delay, sub, n_slides=1, step=2048, mult=[1, 1, 1])
+    # the same candidates end to end, nothing from the CUDA path on the oracle's side: float64 SNR of the sampled
+    # templates -> O4 -> O6 / O7
+    zr64 = np.zeros((D, len(sel), ring), np.complex128)
+    zr64[:, :, :NC * 2048] = z_ref
+    k_o, v_o = oracle.peaks_mode0(z_ref[:, :, (NC - 2) * 2048:(NC - 1) * 2048].reshape(D * len(sel), 2048), THR)
+    same = (v_o == 1) & (sub["valid"] == 1) & (k_o + (NC - 2) * 2048 == sub["k"])
+    assert same.sum() >= 0.9 * (sub["valid"] == 1).sum()
+    for gres, kw in ((fg[rows], {}), (bg[rows], dict(n_slides=1, step=2048, slide_mult=[1, 1, 1]))):
+        ref_e, pix_e, _ = oracle.sky_search(u2, delay, zr64, len(sel) * ring, ring, ring, k_newest, same.astype(np.int32),
+                                            sub["tmpl"], sub["det"], sub["k"], **kw)
+        idx = np.nonzero(same & (pix_e[:, 0] >= 0))[0]
+        cg, ce = gres["coh2"][idx].astype(np.float64), ref_e[idx, 0, 0]
+        assert len(idx) >= 8 and np.all(gres["pix"][idx] >= 0)
+        assert np.all(np.abs(np.sqrt(cg) - np.sqrt(ce)) <= 1e-3) and np.all(np.abs(cg - ce) <= 1e-4 * ce + 1e-5)
 
 
 def _subset_trig(trig_rows, sel, D):
