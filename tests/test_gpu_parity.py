@@ -529,6 +529,21 @@ def test_xi2_signal_consistency(sp, U):
         assert np.all(np.abs(xi["xi2"][:, I] - ref[:, I]) <= 1e-4 * ref[:, I] + 1e-5)
     assert np.all(np.abs(xi["xi2_c"] - ref[:, D]) <= 1e-4 * ref[:, D] + 1e-5)
     assert np.all(xi["xi2"][~used] == 0) and np.all(xi["xi2_c"][~used] == 0)
+    # end to end, nothing from the CUDA path on the oracle's side: float64 SNR -> O4 -> O6 -> O8 with the oracle's
+    # own float64 autocorrelation; compared where both chains chose the same sample and pixel
+    z64 = oracle.filter_bank(x, bank)
+    sl = slice((NC - 2) * 2048, (NC - 1) * 2048)
+    k_o, v_o = oracle.peaks_mode0(z64[:, :, sl].reshape(D * T, 2048), 2.5)
+    same = (v_o == 1) & (trig["valid"] == 1) & (k_o + (NC - 2) * 2048 == trig["k"])
+    ref_s, pix_s, _ = oracle.sky_search(u2, delay, z64, T * ring, ring, ring, k_newest, same.astype(np.int32),
+                                        trig["tmpl"], trig["det"], trig["k"])
+    A64 = np.stack([oracle.template_autocorr(bank_A, t, nj) for t in range(T)])
+    same &= pix_s[:, 0] == res["pix"]
+    xe = oracle.xi2(delay, z64, T * ring, ring, ring, k_newest, same.astype(np.int32), trig["tmpl"], trig["det"],
+                    trig["k"], pix_s[:, 0], A64, nj)
+    idx = np.nonzero(same & (xe[:, D + 1] == 1))[0]
+    assert len(idx) >= 15
+    assert np.all(np.abs(xi["xi2_c"][idx] - xe[idx, D]) <= 1e-3 * xe[idx, D] + 1e-4)   # float32 table and SNR vs float64
     # noise candidates: a reduced chi^2 of order 1; not exactly 1, the windows are centred on maxima
     assert 0.5 < np.median(xi["xi2_c"][used]) < 1.5
     # background events: one-second slides of the same candidates (chunk NC-2: slides 1 and 2 exist, 3 does not)
