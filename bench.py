@@ -385,9 +385,11 @@ def run_ours(args):
     clk = clocks.stop(wall0, wall1) if clocks else None
     c0 += K
     stage = np.zeros(4)
+    per_step_ms = []
     for e in evs:
         for q in range(4):
             stage[q] += e[q].elapsed_time(e[q + 1])
+        per_step_ms.append(e[0].elapsed_time(e[4]))
     cnt = counts.cpu().numpy()
     # candidates searched in step j are those found in step j-1
     n_cand = int(cnt[i_first - 1:i_first - 1 + K].sum()) if has_sky else 0
@@ -561,6 +563,7 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_dict(args, w),
         "sky_evals_per_s": evals_all / (ms_total * 1e-3) if has_sky else None,
         "chunk_latency_ms": ms_total / K,
+        "chunk_latency_ms_median_max": [float(np.median(per_step_ms)), float(np.max(per_step_ms))],
         "stages_ms_per_step": {"filter_chunk": stage[0] / K, "of_which_k_bank": ms_rec / max(1, n_rec),
                                "peaks": stage[1] / K, "sky_foreground": stage[2] / K, "sky_slides": stage[3] / K},
         "stage_rates": {"bank_updates_per_s": upd_chunk * K / (stage[0] * 1e-3),
