@@ -598,7 +598,7 @@ def len_groups(bk):
     seen = set()
     for b in range(bk.n_bands):
         p = bk.band_plan(b)
-        seen.add((p["lanes_per_unit"], p["filters_per_lane"]))
+        seen.add((p["lanes_per_unit"], p["filters_per_lane"], b == 0 and bk.out_band == 1))
     return len(seen)
 
 

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstring>
 #include <map>
+#include <tuple>
 #include <numeric>
 
 #include "spiir_internal.cuh"
@@ -31,6 +32,7 @@ static inline int round_up(int x, int a) { return (x + a - 1) / a * a; }
 // Host images of the arrays the plan produces (filled only when `fill` is set).
 struct PlanImages {
   std::vector<float4> coef[SPIIR_MAX_BANDS];
+  std::vector<float2> coef2[SPIIR_MAX_BANDS];    // a b of a two-sample (odd-only) band
   std::vector<int32_t> off[SPIIR_MAX_BANDS];
   std::vector<int32_t> tb_first, tb_count;
 };
@@ -95,7 +97,7 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
 
   // per band: filters of each template
   std::vector<std::vector<int64_t>> ids((size_t)T);
-  std::map<std::pair<int, int>, size_t> group_of;
+  std::map<std::tuple<int, int, int>, size_t> group_of;
   for (int b = 0; b < B; ++b) {
     spiir_bank_host_band& hb = bk->band[b];
     hb = spiir_bank_host_band();
@@ -140,16 +142,18 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
     hb.n_wu_long = nul_pad / upw;
     const size_t slots = (size_t)hb.n_units * cap_unit;
     hb.off_coef = take(slots * sizeof(float4));
+    const int odd = (b == 0 && d->out_band == 1) ? 1 : 0;      // the band above the output rate: two samples per step
+    if (odd) hb.off_coef2 = take(slots * sizeof(float2));
     hb.off_off = take(slots * sizeof(int32_t));
     // launch groups, one per (G, F); the long-delay CTAs of a group are listed first (they start first
     // and overlap the rest instead of forming a tail)
     for (int cls = 1; cls >= 0; --cls) {
       const int nwu = cls ? hb.n_wu_long : hb.n_wu_short;
       if (!nwu) continue;
-      auto key = std::make_pair(G, F);
+      auto key = std::make_tuple(G, F, odd);
       if (!group_of.count(key)) {
         group_of[key] = bk->groups.size();
-        spiir_launch_group g; g.G = G; g.F = F;
+        spiir_launch_group g; g.G = G; g.F = F; g.odd = odd;
         bk->groups.push_back(g);
       }
       spiir_launch_group& g = bk->groups[group_of[key]];
@@ -163,6 +167,7 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
     }
     if (img) {
       img->coef[b].assign(slots, make_float4(0.f, 0.f, 0.f, 0.f));
+      if (odd) img->coef2[b].assign(slots, make_float2(0.f, 0.f));
       img->off[b].assign(slots, 0);
       const int prpu = F * (G / 8);                          // phase-rows per unit
       std::vector<std::pair<int, int64_t>> order;
@@ -196,6 +201,12 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
           const int e = (lng ? hb.Hcap : hb.Hs) - dl;
           const int al = e & 3;
           img->coef[b][slot] = make_float4(d->host_a[l].re, d->host_a[l].im, d->host_b[l].re, d->host_b[l].im);
+          if (odd) {                                           // a^2 and a b in float64 from the float32 a, b, rounded once
+            const double ar = d->host_a[l].re, ai = d->host_a[l].im, br = d->host_b[l].re, bi = d->host_b[l].im;
+            img->coef[b][slot].x = (float)(ar * ar - ai * ai);
+            img->coef[b][slot].y = (float)(2.0 * ar * ai);
+            img->coef2[b][slot] = make_float2((float)(ar * br - ai * bi), (float)(ar * bi + ai * br));
+          }
           img->off[b][slot] = al * (lng ? hb.cap : hb.reps) + (e - al);
         }
       }
@@ -281,6 +292,11 @@ int spiir_bank_init(spiir_bank** out, const spiir_bank_desc* desc, void* dev_wor
       e = cudaMemcpyAsync(bk->ws + hb.off_off, img.off[b].data(), img.off[b].size() * sizeof(int32_t),
                           cudaMemcpyHostToDevice, st);
       if (e != cudaSuccess) return fail(e, "copy off");
+      if (!img.coef2[b].empty()) {
+        e = cudaMemcpyAsync(bk->ws + hb.off_coef2, img.coef2[b].data(), img.coef2[b].size() * sizeof(float2),
+                            cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return fail(e, "copy coef2");
+      }
     }
   }
   e = cudaMemcpyAsync(bk->ws + bk->off_tb_first, img.tb_first.data(), img.tb_first.size() * 4, cudaMemcpyHostToDevice, st);
@@ -377,6 +393,7 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     BandDev& bd = P.band[b];
     const size_t slots = (size_t)hb.n_units * hb.G * hb.F;
     bd.coef = (const float4*)(bk->ws + hb.off_coef);
+    bd.coef2 = (const float2*)(bk->ws + hb.off_coef2);
     bd.off = (const int32_t*)(bk->ws + hb.off_off);
     bd.state = (float2*)(bk->ws + hb.off_state);
     bd.S = (float2*)(bk->ws + hb.off_S);
@@ -403,7 +420,7 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
   SPIIR_CUDA_OK(cudaGetLastError());
   if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[1], st));
   for (auto& g : bk->groups) {
-    int rc = launch_bank_group(g.G, g.F, P, (const CtaWork*)(bk->ws + g.off_work), (int)g.work.size(), D,
+    int rc = launch_bank_group(g.G, g.F, g.odd, P, (const CtaWork*)(bk->ws + g.off_work), (int)g.work.size(), D,
                                g.smem_bytes, st);
     if (rc) return rc;
   }

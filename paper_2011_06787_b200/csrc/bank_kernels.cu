@@ -1,7 +1,8 @@
 // Device kernels of the SPIIR filter bank (H0-H3 of DESIGN.md) for sm_100a.
 //
 //   k_prep    H0  history shift + x2 decimator chain + 4 pre-shifted replicas per band
-//   k_bank    H1+H2 delay fetch + IIR recursion + per-unit band sums (THE hot loop)
+//   k_bank    H1+H2 delay fetch + IIR recursion + per-unit band sums (THE hot loop); the band above the
+//             output rate advances two samples per step (a^2, a b precomputed)
 //   k_combine H3  unit sums -> band sums -> interpolating cascade -> SNR ring, fused
 //                 per-template peak tracking (H4 mode 0)
 //
@@ -152,7 +153,8 @@ __device__ __forceinline__ float reduce4(float (&s)[4], int lane) {
 
 template <int F>
 struct FilterRegs {
-  float ar[F], ai[F], br[F], bi[F], yr[F], yi[F];
+  float ar[F], ai[F], br[F], bi[F], yr[F], yi[F];   // in a two-sample (odd-only) band ar/ai hold a^2
+  float abr[F], abi[F];                             // a b, two-sample bands only (dead otherwise)
   int off[F];
 };
 
@@ -227,6 +229,69 @@ __device__ __forceinline__ void step4(FilterRegs<F>& r, const float* __restrict_
   }
 }
 
+// The band above the output rate contributes its odd samples only (reading M5), so its recursion advances TWO
+// samples per step - north_star's "chunked scan using precomputed a1 powers", chunk = 2:
+//   y[2m+1] = a^2 y[2m-1] + (a b) x[2m-d] + b x[2m+1-d]
+// with a^2 and a b formed in float64 at init: 8 multiply-adds + 2 adds per two filter-samples instead of 12 + 2.
+// Four input samples = two steps; s[] = (re1, im1, re3, im3).  Pairs of filters packed as in step4.
+template <int F, bool XG>
+__device__ __forceinline__ void step2x2(FilterRegs<F>& r, const float* __restrict__ x, int i, float (&s)[4]) {
+  float2 sr[2], si[2];
+#pragma unroll
+  for (int f = 0; f + 1 < F; f += 2) {
+    float4 xa, xb;
+    if (XG) {
+      xa = __ldg(reinterpret_cast<const float4*>(x + r.off[f] + i));
+      xb = __ldg(reinterpret_cast<const float4*>(x + r.off[f + 1] + i));
+    } else {
+      xa = *reinterpret_cast<const float4*>(x + r.off[f] + i);
+      xb = *reinterpret_cast<const float4*>(x + r.off[f + 1] + i);
+    }
+    const float xsa[4] = {xa.x, xa.y, xa.z, xa.w}, xsb[4] = {xb.x, xb.y, xb.z, xb.w};
+    const float2 a2r = make_float2(r.ar[f], r.ar[f + 1]), a2i = make_float2(r.ai[f], r.ai[f + 1]);
+    const float2 na2i = make_float2(-r.ai[f], -r.ai[f + 1]);
+    float2 yr = make_float2(r.yr[f], r.yr[f + 1]), yi = make_float2(r.yi[f], r.yi[f + 1]);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const float2 pr = make_float2(fmaf(r.abr[f], xsa[2 * h], r.br[f] * xsa[2 * h + 1]),
+                                    fmaf(r.abr[f + 1], xsb[2 * h], r.br[f + 1] * xsb[2 * h + 1]));
+      const float2 pi = make_float2(fmaf(r.abi[f], xsa[2 * h], r.bi[f] * xsa[2 * h + 1]),
+                                    fmaf(r.abi[f + 1], xsb[2 * h], r.bi[f + 1] * xsb[2 * h + 1]));
+      const float2 tr = __ffma2_rn(na2i, yi, pr);
+      const float2 ti = __ffma2_rn(a2i, yr, pi);
+      const float2 nr = __ffma2_rn(a2r, yr, tr);
+      const float2 ni = __ffma2_rn(a2r, yi, ti);
+      yr = nr; yi = ni;
+      if (f == 0) { sr[h] = yr; si[h] = yi; }
+      else        { sr[h] = __fadd2_rn(sr[h], yr); si[h] = __fadd2_rn(si[h], yi); }
+    }
+    r.yr[f] = yr.x; r.yr[f + 1] = yr.y; r.yi[f] = yi.x; r.yi[f + 1] = yi.y;
+  }
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    s[2 * h] = (F > 1) ? sr[h].x + sr[h].y : 0.f;
+    s[2 * h + 1] = (F > 1) ? si[h].x + si[h].y : 0.f;
+  }
+  if (F & 1) {
+    constexpr int f = F - 1;
+    float4 xv;
+    if (XG) xv = __ldg(reinterpret_cast<const float4*>(x + r.off[f] + i));
+    else    xv = *reinterpret_cast<const float4*>(x + r.off[f] + i);
+    const float xs[4] = {xv.x, xv.y, xv.z, xv.w};
+    float yr = r.yr[f], yi = r.yi[f];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const float pr = fmaf(r.abr[f], xs[2 * h], r.br[f] * xs[2 * h + 1]);
+      const float pi = fmaf(r.abi[f], xs[2 * h], r.bi[f] * xs[2 * h + 1]);
+      const float nr = fmaf(r.ar[f], yr, fmaf(-r.ai[f], yi, pr));
+      const float ni = fmaf(r.ar[f], yi, fmaf(r.ai[f], yr, pi));
+      yr = nr; yi = ni;
+      s[2 * h] += yr; s[2 * h + 1] += yi;
+    }
+    r.yr[f] = yr; r.yi[f] = yi;
+  }
+}
+
 // One sub-chunk of `len` samples for this lane's filters: recursion, unit sums, store.
 template <int G, int F, bool XG, bool ODD>
 __device__ __forceinline__ void run_samples(FilterRegs<F>& r, const float* __restrict__ x, int len, float* __restrict__ So,
@@ -234,7 +299,7 @@ __device__ __forceinline__ void run_samples(FilterRegs<F>& r, const float* __res
   for (int i = 0; i < len; i += 4) {
     if (ODD) {
       float s[4];
-      step4<F, XG, true>(r, x, i, s);
+      step2x2<F, XG>(r, x, i, s);
       const float t = reduce4<G>(s, lane);
       if (g < 8 && !(g & 1)) So[i + (g >> 1)] = t;          // 2 complex samples per 4 inputs
     } else {
@@ -246,7 +311,7 @@ __device__ __forceinline__ void run_samples(FilterRegs<F>& r, const float* __res
   }
 }
 
-template <int G, int F>
+template <int G, int F, bool ODD>
 __global__ void __launch_bounds__(kBankThreads, 2)
 k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
   extern __shared__ __align__(128) float xs[];
@@ -256,7 +321,6 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int wu = w.wu_begin + warp;
   const bool active = wu < w.wu_end;
-  const bool odd = B.odd != 0;                       // CTA-uniform
 
   FilterRegs<F> r;
   const size_t slot0 = ((size_t)wu * F) * 32 + lane;
@@ -267,6 +331,7 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
       const float4 c = __ldg(B.coef + slot0 + f * 32);
       r.ar[f] = c.x; r.ai[f] = c.y; r.br[f] = c.z; r.bi[f] = c.w;
       r.off[f] = __ldg(B.off + slot0 + f * 32);
+      if (ODD) { const float2 ab = __ldg(B.coef2 + slot0 + f * 32); r.abr[f] = ab.x; r.abi[f] = ab.y; }
       const float2 y = st[slot0 + f * 32];
       r.yr[f] = y.x; r.yi[f] = y.y;
     }
@@ -282,8 +347,7 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
     // global memory (L1/L2 resident)
     if (active) {
       const float* x = B.xrep + (size_t)det * B.x_det_stride;
-      if (odd) run_samples<G, F, true, true>(r, x, n, Sout, lane, g);
-      else     run_samples<G, F, true, false>(r, x, n, Sout, lane, g);
+      run_samples<G, F, true, ODD>(r, x, n, Sout, lane, g);
     }
   } else {
     uint64_t* bar = reinterpret_cast<uint64_t*>(xs + kReplicas * B.reps);
@@ -304,8 +368,7 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
       mbar_wait(bar, phase);
       phase ^= 1u;
       if (active) {
-        if (odd) run_samples<G, F, false, true>(r, xs, len, Sout + m0, lane, g);
-        else     run_samples<G, F, false, false>(r, xs, len, Sout + 2 * m0, lane, g);
+        run_samples<G, F, false, ODD>(r, xs, len, Sout + (ODD ? m0 : 2 * m0), lane, g);
       }
     }
   }
@@ -315,13 +378,13 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
   }
 }
 
-template <int G, int F>
+template <int G, int F, bool ODD>
 static int launch_one(const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det, int smem, cudaStream_t st) {
   static unsigned long long configured = 0;
   if (first_use_on_device(configured)) {
-    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_bank<G, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_bank<G, F, ODD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   }
-  k_bank<G, F><<<dim3(n_cta, n_det), kBankThreads, smem, st>>>(P, dev_work);
+  k_bank<G, F, ODD><<<dim3(n_cta, n_det), kBankThreads, smem, st>>>(P, dev_work);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());
   return SPIIR_OK;
@@ -329,19 +392,19 @@ static int launch_one(const BankParams& P, const CtaWork* dev_work, int n_cta, i
 
 #define SPIIR_F_CASES(G)                                                          \
   switch (F) {                                                                    \
-    case 4:  return launch_one<G, 4>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 5:  return launch_one<G, 5>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 6:  return launch_one<G, 6>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 7:  return launch_one<G, 7>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 8:  return launch_one<G, 8>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 9:  return launch_one<G, 9>(P, dev_work, n_cta, n_det, smem, st);        \
-    case 10: return launch_one<G, 10>(P, dev_work, n_cta, n_det, smem, st);       \
-    case 11: return launch_one<G, 11>(P, dev_work, n_cta, n_det, smem, st);       \
-    case 12: return launch_one<G, 12>(P, dev_work, n_cta, n_det, smem, st);       \
+    case 4:  return odd ? launch_one<G, 4, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 4, false>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 5:  return odd ? launch_one<G, 5, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 5, false>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 6:  return odd ? launch_one<G, 6, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 6, false>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 7:  return odd ? launch_one<G, 7, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 7, false>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 8:  return odd ? launch_one<G, 8, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 8, false>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 9:  return odd ? launch_one<G, 9, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 9, false>(P, dev_work, n_cta, n_det, smem, st);        \
+    case 10: return odd ? launch_one<G, 10, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 10, false>(P, dev_work, n_cta, n_det, smem, st);       \
+    case 11: return odd ? launch_one<G, 11, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 11, false>(P, dev_work, n_cta, n_det, smem, st);       \
+    case 12: return odd ? launch_one<G, 12, true>(P, dev_work, n_cta, n_det, smem, st) : launch_one<G, 12, false>(P, dev_work, n_cta, n_det, smem, st);       \
     default: break;                                                               \
   }
 
-int launch_bank_group(int G, int F, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
+int launch_bank_group(int G, int F, int odd, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
                       int smem, cudaStream_t st) {
   if (G == 8) { SPIIR_F_CASES(8) }
   else if (G == 16) { SPIIR_F_CASES(16) }

@@ -52,7 +52,8 @@ constexpr int kSmemFloatsMax = 6400;  // per replica: Hs + sub-chunk <= this (4 
 
 // Device-side description of one rate band, passed by value inside BankParams.
 struct BandDev {
-  const float4* coef;     // [wu][F][32]  (a.re, a.im, b.re, b.im)
+  const float4* coef;     // [wu][F][32]  (a.re, a.im, b.re, b.im); two-sample (odd-only) band: (a^2.re, a^2.im, b.re, b.im)
+  const float2* coef2;    // [wu][F][32]  two-sample band only: a b
   const int32_t* off;     // [wu][F][32]  float offset of the filter's first sample in the replica set
   float2* state;          // [det][wu][F][32]
   float2* S;              // [det][unit][nmax] per-unit partial band sums of the current chunk
@@ -105,7 +106,7 @@ struct CombineParams {
 };
 
 void launch_prep(const PrepParams& p, int n_det, cudaStream_t st);
-int launch_bank_group(int G, int F, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
+int launch_bank_group(int G, int F, int odd, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
                       int smem, cudaStream_t st);
 void launch_combine(const CombineParams& p, int n_det, cudaStream_t st);
 
@@ -130,12 +131,13 @@ struct spiir_bank_host_band {
   int Hcap = 0, Hs = 0, cap = 0, reps = 0, nmax = 0, rate = 0;
   int64_t n_filters = 0;
   // workspace offsets (bytes)
+  size_t off_coef2 = 0;
   size_t off_coef = 0, off_off = 0, off_state = 0, off_S = 0, off_x[2] = {0, 0}, off_uphist = 0;
   int prev_n = 0;
 };
 
 struct spiir_launch_group {
-  int G, F;
+  int G, F, odd;
   std::vector<spiir::CtaWork> work;
   size_t off_work = 0;
   int smem_bytes = 0;
