@@ -9,7 +9,7 @@ import ctypes as C
 import numpy as np
 
 from .build import build as _build
-from .sky import healpix_ring_centres, sky_table, g_sigma  # noqa: F401
+from .sky import healpix_ring_centres, sky_table, g_sigma, table_set, nearest_table  # noqa: F401
 
 _lib = None
 

@@ -74,3 +74,33 @@ def sky_table(nside, pos, resp, sigma, gmst, fs):
     tau = -(n @ np.asarray(pos, float).T) / C_LIGHT
     delay = np.rint(tau * fs).astype(np.int32)
     return U2, delay
+
+
+# ----------------------------------------------------------------------------- O10 (NEXT-3)
+# "we sample U every half hour up to 24 hours and refreshed every day ...  Time offsets of SNRs
+# from different detectors are sampled at the same interval along with U.  The pipeline will
+# calculate the coherent SNR using the U and offset sample that are closest in the time to the
+# triggering candidate".
+SIDEREAL_DAY_S = 86164.0905          # one turn of the Earth against the stars, in seconds
+
+
+def table_set(nside, pos, resp, sigma, gmst0, interval_s, n_sets, fs):
+    """Set i is the table of `sky_table` at time t0 + i interval_s, i.e. at sidereal angle
+    gmst0 + 2 pi i interval_s / SIDEREAL_DAY_S (reading X6).  Returns (U2 [n][P][D][2], delay [n][P][D])."""
+    U, dl = [], []
+    for i in range(int(n_sets)):
+        gm = gmst0 + 2.0 * np.pi * (i * float(interval_s)) / SIDEREAL_DAY_S
+        u, d = sky_table(nside, pos, resp, sigma, gm, fs)
+        U.append(u)
+        dl.append(d)
+    return np.stack(U), np.stack(dl)
+
+
+def nearest_table(t, t0, interval_s, n_sets):
+    """Index of the set closest in time to t, by exhaustive comparison; the earlier one on an exact
+    tie; -1 when t is further than interval_s / 2 from every set (the tables are stale: PAPER.md:173
+    refreshes them every day) — reading X6."""
+    times = t0 + np.arange(int(n_sets)) * float(interval_s)
+    dist = np.abs(float(t) - times)
+    i = int(np.argmin(dist))                                  # first minimum = earlier set
+    return i if dist[i] <= 0.5 * float(interval_s) else -1

@@ -706,3 +706,91 @@ def test_p14_strain_injection_recovers_its_direction_or_the_mirror_image():
     assert rank_true < 0.03 * len(vec)
     assert math.sqrt(mp[0, p_true]) >= 0.97 * math.sqrt(res[0, 0, 0])
     assert 12.0 < math.sqrt(res[0, 0, 0]) < 18.0                             # injected network SNR 15 in unit noise
+
+
+# ----------------------------------------------------------------------------- NEXT-3: table sets
+def _rings(nside):
+    """(start, length) of every HEALPix ring, from the ring structure itself: 4 i pixels in the caps,
+    4 nside in the belt."""
+    out, s = [], 0
+    lens = [4 * i for i in range(1, nside)] + [4 * nside] * (2 * nside + 1) + [4 * i for i in range(nside - 1, 0, -1)]
+    for n in lens:
+        out.append((s, n))
+        s += n
+    assert s == 12 * nside * nside
+    return out
+
+
+def test_p24_table_set_follows_the_earths_rotation():
+    """U and the offsets are sampled every half hour over 24 h 'to accommodate the change
+    of detector locations due to Earth's rotation'.  A quarter turn of the Earth (gmst + pi/2) moves every
+    table entry a quarter of its ring to the east (every ring has a multiple of 4 pixels), a full sidereal
+    day brings the set back, and a solar day leaves the 3 min 56 s that make the daily refresh necessary."""
+    ns = 4
+    pos, resp = workloads.detector_geometry(["H1", "L1", "V1"])
+    sig = [1.0, 0.8, 0.5]
+    U0, d0 = oracle.sky_table(ns, pos, resp, sig, 0.7, 2048.0)
+    U1, d1 = oracle.sky_table(ns, pos, resp, sig, 0.7 + np.pi / 2, 2048.0)
+    P0, P1 = U0 @ U0.transpose(0, 2, 1), U1 @ U1.transpose(0, 2, 1)
+    for s, n in _rings(ns):
+        j = np.arange(n)
+        src = s + (j - n // 4) % n                              # entry now at phi was at phi - pi/2
+        np.testing.assert_allclose(P1[s + j], P0[src], atol=1e-10)
+        assert np.array_equal(d1[s + j], d0[src])
+    assert not np.allclose(P1, P0, atol=1e-3)                   # and it is not the identity
+    # the set: 49 samples a 48th of a sidereal day apart close on themselves, each is sky_table at its angle
+    Us, ds = oracle.table_set(ns, pos, resp, sig, 0.7, oracle.sky.SIDEREAL_DAY_S / 48, 49, 2048.0)
+    Ps = Us @ Us.transpose(0, 1, 3, 2)
+    np.testing.assert_allclose(Ps[48], Ps[0], atol=1e-9)
+    assert np.array_equal(ds[48], ds[0])
+    np.testing.assert_allclose(Ps[12], P1, atol=1e-9)           # 12/48 of a turn = pi/2
+    assert np.array_equal(ds[12], d1)
+    omega = 7.2921150e-5                                        # Earth's rotation rate, rad/s (IERS)
+    Ua, da = oracle.sky_table(ns, pos, resp, sig, 0.7 + omega * 5 * 1800.0, 2048.0)
+    Ub, db = oracle.table_set(ns, pos, resp, sig, 0.7, 1800.0, 6, 2048.0)
+    np.testing.assert_allclose(Ub[5] @ Ub[5].transpose(0, 2, 1), Ua @ Ua.transpose(0, 2, 1), atol=1e-6)
+    assert np.mean(db[5] != da) < 0.01
+    drift = (86400.0 / oracle.sky.SIDEREAL_DAY_S - 1.0) * 86400.0
+    assert abs(drift - 236.6) < 0.5                             # seconds per solar day
+
+
+def test_p25_nearest_table_and_the_east_west_statement():
+    """'closest in the time to the triggering candidate' and 'the maximum coherent SNR value would not be
+    affected but the detected sky direction ... could be off ... up to 15-min in the East-West direction'
+    (PAPER.md:173)."""
+    rng = np.random.default_rng(5)
+    t0, dt, n = 1.0e9, 1800.0, 48
+    for t in np.concatenate([t0 + rng.uniform(-900, 47 * 1800 + 900, 500), [t0, t0 + 47 * 1800.0]]):
+        i = oracle.nearest_table(t, t0, dt, n)
+        assert 0 <= i < n and abs(t - (t0 + i * dt)) <= 900.0   # never further than 15 min
+        assert all(abs(t - (t0 + i * dt)) <= abs(t - (t0 + k * dt)) for k in (i - 1, i + 1))
+    assert oracle.nearest_table(t0 + 2700.0, t0, dt, n) == 1    # exact tie: the earlier set
+    assert oracle.nearest_table(t0 - 900.0, t0, dt, n) == 0
+    assert oracle.nearest_table(t0 - 900.5, t0, dt, n) == -1    # stale on either side
+    assert oracle.nearest_table(t0 + 47 * 1800 + 900.5, t0, dt, n) == -1
+    # a signal built with the table of its own time, searched with a table k belt pixels of rotation
+    # away: same maximum, found k pixels further east in the same ring
+    ns, k = 8, 3
+    pos, resp = workloads.detector_geometry(["H1", "L1", "V1"])
+    sig = [1.0, 1.0, 0.5]
+    Ut, dlt = oracle.sky_table(ns, pos, resp, sig, 1.234, 2048.0)
+    Uo, dlo = oracle.sky_table(ns, pos, resp, sig, 1.234 + k * 2 * np.pi / (4 * ns), 2048.0)
+    rings = _rings(ns)
+    for ring in (ns + 1, 2 * ns, 3 * ns - 2):                   # belt rings
+        s, nr = rings[ring]
+        j0 = int(rng.integers(nr))
+        p0 = s + j0
+        z = np.zeros((3, 1, 800), complex)
+        c = rng.standard_normal(2) + 1j * rng.standard_normal(2)
+        amp = Ut[p0] @ c
+        o = np.arange(-20, 21)
+        env = np.exp(-o ** 2 / (2 * 6.0 ** 2)) * np.exp(0.6j * o)
+        for I in range(3):
+            z[I, 0, 400 + dlt[p0, I] - dlt[p0, 0] + o] = amp[I] * env
+        kw = dict(trig_valid=[1], trig_row=[0], trig_det=[0], trig_k=[400], want_map=True, **_dense_view(z))
+        rt, pt, mt = oracle.sky_search(Ut.astype(np.float32), dlt, z, **kw)
+        ro, po, mo = oracle.sky_search(Uo.astype(np.float32), dlo, z, **kw)
+        assert abs(ro[0, 0, 0] - rt[0, 0, 0]) < 1e-5 * rt[0, 0, 0]          # maximum not affected
+        np.testing.assert_allclose(mo[0, s + (np.arange(nr) + k) % nr], mt[0, s:s + nr], rtol=1e-5, atol=1e-9)
+        same_o = [p for p in range(12 * ns * ns) if np.array_equal(dlo[p] - dlo[p, 0], dlt[p0] - dlt[p0, 0])]
+        assert po[0, 0] in same_o and (s + (j0 + k) % nr) in same_o
