@@ -149,6 +149,26 @@ int spiir_sky_table_build(int32_t nside, int32_t n_det, const double* host_det_p
                           const double* host_det_resp, const double* host_sigma,
                           double gmst_rad, double fs_hz, float* host_u2, int32_t* host_delay);
 
+/* NEXT-3 — "we sample U every half hour up to 24 hours and
+ * refreshed every day ... Time offsets ... are sampled at the same interval
+ * along with U.  The pipeline will calculate the coherent SNR using the U and
+ * offset sample that are closest in the time to the triggering candidate."
+ * Set i (0 <= i < n_sets) is spiir_sky_table_build at sidereal angle
+ * gmst0_rad + 2 pi i interval_s / 86164.0905 (one turn per sidereal day).
+ *   Outputs: host_u2 [n_sets][12 nside^2][n_det][2], host_delay
+ *   [n_sets][12 nside^2][n_det]; other arguments as spiir_sky_table_build. */
+int spiir_sky_table_set_build(int32_t nside, int32_t n_det, const double* host_det_pos_m,
+                              const double* host_det_resp, const double* host_sigma,
+                              double gmst0_rad, double interval_s, int32_t n_sets, double fs_hz,
+                              float* host_u2, int32_t* host_delay);
+
+/* Index of the set closest in time to t_s when set i holds time t0_s +
+ * i interval_s: the earlier set on an exact tie; *index = -1 (and SPIIR_OK)
+ * when t_s is further than interval_s / 2 from every set, i.e. the tables are
+ * stale and must be rebuilt (the paper refreshes them daily).  Host arithmetic
+ * in float64; no device work. */
+int spiir_sky_table_nearest(double t_s, double t0_s, double interval_s, int32_t n_sets, int32_t* index);
+
 /* A look-up table prepared for the device (opaque).  The plan re-orders the
  * directions so that those sharing one tuple of inter-detector delays are
  * adjacent, and stores for each direction the projector U2 U2^T (Eq. 28,

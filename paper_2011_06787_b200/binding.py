@@ -99,6 +99,9 @@ _SIGNATURES = {
     "spiir_rank_finalize": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "spiir_rank_candidates": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                         C.c_double, C.c_void_p, C.c_void_p]),
+    "spiir_sky_table_set_build": (C.c_int, [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                           C.c_double, C.c_int32, C.c_double, C.c_void_p, C.c_void_p]),
+    "spiir_sky_table_nearest": (C.c_int, [C.c_double, C.c_double, C.c_double, C.c_int32, C.c_void_p]),
     "spiir_template_autocorr": (C.c_int, [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]),
     "spiir_last_error": (C.c_char_p, []),
 }
@@ -277,6 +280,48 @@ def sky_table_build(nside, pos, resp, sigma, gmst, fs):
     _check(lib().spiir_sky_table_build(nside, n_det, _hp(pos), _hp(resp), _hp(sigma), float(gmst), float(fs),
                                        _hp(u2), _hp(delay)))
     return u2, delay
+
+
+def sky_table_set_build(nside, pos, resp, sigma, gmst0, interval_s, n_sets, fs):
+    """spiir_sky_table_set_build: (u2 float32 [n_sets][P][D][2], delay int32 [n_sets][P][D])."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    resp = np.ascontiguousarray(resp, dtype=np.float64)
+    sigma = np.ascontiguousarray(sigma, dtype=np.float64)
+    n_det = pos.shape[0]
+    npix = 12 * nside * nside
+    u2 = np.zeros((n_sets, npix, n_det, 2), np.float32)
+    delay = np.zeros((n_sets, npix, n_det), np.int32)
+    _check(lib().spiir_sky_table_set_build(nside, n_det, _hp(pos), _hp(resp), _hp(sigma), float(gmst0),
+                                           float(interval_s), int(n_sets), float(fs), _hp(u2), _hp(delay)))
+    return u2, delay
+
+
+def sky_table_nearest(t, t0, interval_s, n_sets):
+    """spiir_sky_table_nearest: index of the set closest in time, -1 when the tables are stale."""
+    idx = C.c_int32(-2)
+    _check(lib().spiir_sky_table_nearest(float(t), float(t0), float(interval_s), int(n_sets), C.byref(idx)))
+    return int(idx.value)
+
+
+class SkyPlanSet:
+    """One SkyPlan per sampled table; `select(t)` is the plan closest in time to t."""
+
+    def __init__(self, u2_sets, delay_sets, max_slots, t0, interval_s):
+        self.t0, self.interval_s = float(t0), float(interval_s)
+        self.plans = [SkyPlan(u, d, max_slots) for u, d in zip(u2_sets, delay_sets)]
+
+    def index(self, t):
+        i = sky_table_nearest(t, self.t0, self.interval_s, len(self.plans))
+        if i < 0:
+            raise SpiirError(SPIIR_EINVAL, "sky tables are stale at t = %r: rebuild the set" % (t,))
+        return i
+
+    def select(self, t):
+        return self.plans[self.index(t)]
+
+    def close(self):
+        for p in self.plans:
+            p.close()
 
 
 class SkyPlan:

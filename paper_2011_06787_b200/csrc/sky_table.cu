@@ -120,3 +120,37 @@ extern "C" int spiir_sky_table_build(int32_t nside, int32_t n_det, const double*
   }
   return SPIIR_OK;
 }
+
+// NEXT-3: the tables sampled along the Earth's rotation, and the nearest-in-time set.
+extern "C" int spiir_sky_table_set_build(int32_t nside, int32_t n_det, const double* pos, const double* resp,
+                                         const double* sigma, double gmst0, double interval_s, int32_t n_sets,
+                                         double fs, float* u2, int32_t* delay) {
+  SPIIR_REQUIRE(n_sets >= 1 && n_sets <= 4096, "n_sets %d out of range", n_sets);
+  SPIIR_REQUIRE(interval_s > 0.0, "interval_s must be positive");
+  const double kSiderealDay = 86164.0905;
+  const size_t npix = (size_t)12 * nside * nside;
+  for (int i = 0; i < n_sets; ++i) {
+    const double gm = gmst0 + 2.0 * kPi * ((double)i * interval_s) / kSiderealDay;
+    const int rc = spiir_sky_table_build(nside, n_det, pos, resp, sigma, gm, fs, u2 + (size_t)i * npix * n_det * 2,
+                                         delay + (size_t)i * npix * n_det);
+    if (rc) return rc;
+  }
+  return SPIIR_OK;
+}
+
+extern "C" int spiir_sky_table_nearest(double t, double t0, double interval_s, int32_t n_sets, int32_t* index) {
+  SPIIR_REQUIRE(index != nullptr, "index is NULL");
+  SPIIR_REQUIRE(n_sets >= 1 && interval_s > 0.0, "bad n_sets / interval_s");
+  *index = -1;
+  double x = (t - t0) / interval_s;
+  SPIIR_REQUIRE(x == x, "t_s / t0_s is not a number");
+  x = x < -1.0 ? -1.0 : (x > (double)n_sets ? (double)n_sets : x);
+  long i = (long)std::ceil(x - 0.5);                      // nearest; x = i + 1/2 goes to the earlier set i
+  i = i < 0 ? 0 : (i > n_sets - 1 ? n_sets - 1 : i);
+  // settle the last ulp by the distances themselves, as the definition does
+  while (i > 0 && std::fabs(t - (t0 + (double)(i - 1) * interval_s)) <= std::fabs(t - (t0 + (double)i * interval_s))) --i;
+  while (i < n_sets - 1 && std::fabs(t - (t0 + (double)(i + 1) * interval_s)) < std::fabs(t - (t0 + (double)i * interval_s))) ++i;
+  if (std::fabs(t - (t0 + (double)i * interval_s)) > 0.5 * interval_s) return SPIIR_OK;
+  *index = (int32_t)i;
+  return SPIIR_OK;
+}

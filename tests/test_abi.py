@@ -103,6 +103,34 @@ def test_host_table_builder_matches_the_oracle_table(sp):
         assert np.abs(P - Po).max() < 1e-6
 
 
+def test_table_set_and_nearest_selection_match_the_oracle(sp):
+    """spiir_sky_table_set_build / spiir_sky_table_nearest (NEXT-3) vs oracle.table_set /
+    oracle.nearest_table: delays exactly, projectors to float32 rounding, indices exactly."""
+    import oracle
+    pos, resp = workloads.detector_geometry(["H1", "L1", "V1"])
+    sigma = [1.0, 0.9, 0.4]
+    u2, dl = sp.sky_table_set_build(8, pos, resp, sigma, 2.5, 1800.0, 48, 2048.0)
+    U2o, dlo = oracle.table_set(8, pos, resp, sigma, 2.5, 1800.0, 48, 2048.0)
+    assert u2.shape == (48, 768, 3, 2) and np.array_equal(dl, dlo)
+    P = np.einsum("spik,spjk->spij", u2.astype(float), u2.astype(float))
+    Po = np.einsum("spik,spjk->spij", U2o, U2o)
+    assert np.abs(P - Po).max() < 1e-6
+    assert not np.array_equal(dl[0], dl[1])                      # half an hour does move the offsets
+    rng = np.random.default_rng(8)
+    t0 = 1.26e9
+    ts = np.concatenate([t0 + rng.uniform(-2000, 48 * 1800 + 2000, 4000),
+                         t0 + 1800.0 * np.arange(-1, 49) + 900.0,          # every midpoint (ties)
+                         t0 + 1800.0 * np.arange(-1, 49), [t0 - 1e15, t0 + 1e15]])
+    for t in ts:
+        assert sp.sky_table_nearest(t, t0, 1800.0, 48) == oracle.nearest_table(t, t0, 1800.0, 48), t
+    for n, dt in ((1, 10.0), (7, 0.3), (48, 1795.0)):
+        for t in rng.uniform(-3 * dt, (n + 2) * dt, 500):
+            assert sp.sky_table_nearest(t, 0.0, dt, n) == oracle.nearest_table(t, 0.0, dt, n)
+    idx = C.c_int32(0)
+    assert sp.lib().spiir_sky_table_nearest(0.0, 0.0, -1.0, 4, C.byref(idx)) != sp.SPIIR_OK
+    assert sp.lib().spiir_sky_table_nearest(float("nan"), 0.0, 1.0, 4, C.byref(idx)) != sp.SPIIR_OK
+
+
 def test_product_package_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2011_06787_b200")
     for dp, _, fs in os.walk(pkg):

@@ -789,3 +789,47 @@ def test_sky_four_detectors(sp, U):
     U.check_sky(bg, zc, L, k_newest, u2, delay, trig, n_slides=S, step=step, mult=[1, 2, 1, 1])
     ok = res["pix"] >= 0
     assert 2.0 < np.mean(res["null2"][ok]) < 6.0 * 1.5                        # ~ (2 N_d - 4) = 4 dof at the arg-max, minus selection
+
+
+# ------------------------------------------------------------------ NEXT-3: half-hourly table sets
+def test_sky_table_set_nearest_in_time(sp, U):
+    """the search uses the U / offset sample closest in time to the candidate.  The product
+    builds its own 48 tables (spiir_sky_table_set_build) and selects with spiir_sky_table_nearest; the
+    oracle builds its set with numpy's SVD and selects by exhaustive comparison."""
+    import torch
+    cfg = workloads.config(3)
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    nside, n_sets, dt, t0, g0 = 8, 48, 1800.0, 1.2e9, 0.4
+    U2o, dlo = oracle.table_set(nside, pos, resp, cfg["sigma"], g0, dt, n_sets, 2048.0)
+    u2p, dlp = sp.sky_table_set_build(nside, pos, resp, cfg["sigma"], g0, dt, n_sets, 2048.0)
+    n_rows = 64
+    pset = sp.SkyPlanSet(u2p, dlp, max_slots=n_rows, t0=t0, interval_s=dt)
+    rng = np.random.default_rng(31)
+    # signals as they arrive at the time of set 5; candidates stamped around it
+    z, tdet, k, truth = workloads.snr_snippets(rng, U2o[5].astype(np.float32), dlo[5], n_rows, 1, 102, 0.5)
+    zc = np.ascontiguousarray(z).view(np.complex64)[..., 0]
+    L = zc.shape[2]
+    trig = np.zeros(n_rows, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1
+    trig["tmpl"] = np.arange(n_rows)
+    trig["det"] = tdet
+    trig["k"] = k
+    view = sp.SnrView(torch.from_numpy(np.ascontiguousarray(z)).cuda())
+    td = sp.triggers_from_numpy(trig)
+    seen = set()
+    for t in (t0 + 5 * dt, t0 + 5 * dt - 899.0, t0 + 5 * dt + 900.0, t0 + 5 * dt + 901.0, t0 + 3 * dt + 1000.0,
+              t0 + 47 * dt + 900.0, t0 - 900.0):
+        i = oracle.nearest_table(t, t0, dt, n_sets)
+        assert pset.index(t) == i
+        seen.add(i)
+        res = sp.results_to_numpy(pset.select(t).search(view, td, n_rows))
+        torch.cuda.synchronize()
+        U.check_sky(res, zc, L, L - 1, U2o[i].astype(np.float32), dlo[i], trig)
+        if i == 5:
+            sig = truth["is_signal"]
+            assert np.mean(res["coh2"][sig]) > 3 * np.mean(res["coh2"][~sig])
+    assert seen == {0, 4, 5, 6, 47}
+    for t in (t0 - 901.0, t0 + 47 * dt + 901.0):
+        with pytest.raises(sp.SpiirError):
+            pset.select(t)
+    pset.close()
