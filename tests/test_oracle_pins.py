@@ -794,3 +794,82 @@ def test_p25_nearest_table_and_the_east_west_statement():
         np.testing.assert_allclose(mo[0, s + (np.arange(nr) + k) % nr], mt[0, s:s + nr], rtol=1e-5, atol=1e-9)
         same_o = [p for p in range(12 * ns * ns) if np.array_equal(dlo[p] - dlo[p, 0], dlt[p0] - dlt[p0, 0])]
         assert po[0, 0] in same_o and (s + (j0 + k) % nr) in same_o
+
+
+# ----------------------------------------------------------------------------- NEXT-3: sub-sample alignment
+def test_p26_cubic_interpolator():
+    """The 4-tap interpolator: textbook half-sample weights (-1, 9, 9, -1)/16, partition of unity,
+    exact on cubics, sample-preserving, and accurate on a slow complex exponential."""
+    np.testing.assert_allclose(oracle.lagrange4(0.5), np.array([-1, 9, 9, -1]) / 16.0, atol=1e-15)
+    np.testing.assert_allclose(oracle.lagrange4(0.25), np.array([-7, 105, 35, -5]) / 128.0, atol=1e-15)
+    for mu in np.linspace(0, 1, 11)[:-1]:
+        w = oracle.lagrange4(mu)
+        assert abs(w.sum() - 1) < 1e-14
+        for deg in range(4):                                        # reproduces t^deg at t = mu
+            assert abs(np.dot(w, np.array([-1.0, 0.0, 1.0, 2.0]) ** deg) - mu ** deg) < 1e-13
+    # windows: layout, sample preservation, validity at the ring's edges, wrap-around
+    rng = np.random.default_rng(3)
+    D, rows, L, R, H = 2, 3, 64, 4, 5
+    k_newest = 100                                                  # ring holds k = 37 .. 100
+    t = np.arange(k_newest - L + 1, k_newest + 1)
+    poly = lambda x: 0.3 + 0.1 * x - 0.02 * x ** 2 + 0.001j * x ** 3   # noqa: E731
+    z = np.zeros((D, rows, L), complex)
+    z[:, :, t % L] = poly(t - 70.0)
+    trig_k = [70, 43, 42, 94, 95, 60]
+    valid = [1, 1, 1, 1, 1, 0]
+    rows_of = [0, 1, 2, 0, 1, 2]
+    out, ok = oracle.upsample_windows(z, L, k_newest, valid, rows_of, [0, 1, 0, 1, 0, 1], trig_k, R, H)
+    assert out.shape == (D, 6, 2 * R * H + 1)
+    assert list(ok) == [1, 1, 0, 1, 0, 0]                           # k-H-1 >= 37 and k+H+1 <= 100
+    for s in (0, 1, 3):
+        tt = trig_k[s] - H + np.arange(2 * R * H + 1) / R
+        np.testing.assert_allclose(out[0, s], poly(tt - 70.0), atol=1e-12)   # a cubic is reproduced exactly
+        assert np.array_equal(out[1, s, ::R], z[1, rows_of[s], (trig_k[s] - H + np.arange(2 * H + 1)) % L])
+    assert np.all(out[:, [2, 4, 5]] == 0)
+    # a complex exponential at 0.05 cycles per sample (100 Hz at 2048 Hz): error below 1e-3
+    zz = np.exp(2j * np.pi * 0.05 * np.arange(200))[None, None, :]
+    o2, _ = oracle.upsample_windows(zz, 200, 199, [1], [0], [0], [100], 8, 20)
+    tt = 80 + np.arange(321) / 8
+    err = np.abs(o2[0, 0] - np.exp(2j * np.pi * 0.05 * tt)).max()
+    assert 1e-5 < err < 1e-3
+    # textbook remainder of cubic interpolation: |f''''| / 4! * max |(mu+1) mu (mu-1) (mu-2)| = w^4 / 24 * 9/16
+    assert err <= (2 * np.pi * 0.05) ** 4 / 24 * 9 / 16 * 1.01
+
+
+def test_p27_sub_sample_alignment_removes_the_integer_delay_loss():
+    """Reading A18's probe: with delays rounded to the 2048 Hz grid a coherent signal leaks into the null
+    stream; resampling the windows 4 times finer and searching with a table at 4 x 2048 Hz brings the
+    null stream down by an order of magnitude and the coherent SNR back to the total."""
+    rng = np.random.default_rng(41)
+    ns, fs, R, H = 8, 2048.0, 4, 60
+    pos, resp = workloads.detector_geometry(["H1", "L1", "V1"])
+    sig = [1.0, 1.0, 0.5]
+    U1, d1 = oracle.sky_table(ns, pos, resp, sig, 1.234, fs)
+    UR, dR = oracle.sky_table(ns, pos, resp, sig, 1.234, fs * R)
+    assert np.abs(dR - R * d1).max() <= R // 2 + 1                  # the same offsets on a finer grid
+    th, ph = oracle.healpix_ring_centres(ns)
+    lam = ph - 1.234
+    nvec = np.stack([np.sin(th) * np.cos(lam), np.sin(th) * np.sin(lam), np.cos(th)], 1)
+    tau = -(nvec @ pos.T) / workloads.C_LIGHT * fs                  # arrival offsets in samples, not rounded
+    env = lambda x: np.exp(-x ** 2 / (2 * 6.0 ** 2)) * np.exp(0.3j * x)   # noqa: E731  (98 Hz carrier)
+    n, k0 = 400, 200
+    null_int, null_fine, loss_int, loss_fine = [], [], [], []
+    for p0 in rng.choice(768, 12, replace=False):
+        c = rng.standard_normal(2) + 1j * rng.standard_normal(2)
+        amp = U1[p0] @ c
+        tot = np.sum(np.abs(amp) ** 2)
+        z = np.zeros((3, 1, n), complex)
+        for I in range(3):
+            z[I, 0] = amp[I] * env(np.arange(n) - k0 - (tau[p0, I] - tau[p0, 0]))
+        kw = dict(trig_valid=[1], trig_row=[0], trig_det=[0], trig_k=[k0])
+        r1, p1, _ = oracle.sky_search(U1.astype(np.float32), d1, z, **kw, **_dense_view(z))
+        zu, ok = oracle.upsample_windows(z, n, n - 1, [1], [0], [0], [k0], R, H)
+        assert ok[0] == 1
+        r4, p4, _ = oracle.sky_search(UR.astype(np.float32), dR, zu, trig_valid=[1], trig_row=[0], trig_det=[0],
+                                      trig_k=[R * H], **_dense_view(zu))
+        assert p4[0, 0] == p0                                       # the fine search finds the true pixel
+        null_int.append(r1[0, 0, 1] / tot); null_fine.append(r4[0, 0, 1] / tot)
+        loss_int.append(1 - r1[0, 0, 0] / tot); loss_fine.append(1 - r4[0, 0, 0] / tot)
+    assert np.mean(null_fine) < 0.1 * np.mean(null_int)
+    assert np.mean(loss_fine) < 0.25 * np.mean(loss_int) and np.max(loss_fine) < 5e-3
+    assert np.mean(loss_int) > 2e-3                                 # the loss being removed is real
