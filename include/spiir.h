@@ -169,6 +169,30 @@ int spiir_sky_table_set_build(int32_t nside, int32_t n_det, const double* host_d
  * in float64; no device work. */
 int spiir_sky_table_nearest(double t_s, double t0_s, double interval_s, int32_t n_sets, int32_t* index);
 
+/* NEXT-3, second half (reading X7 of DESIGN.md) — sub-sample
+ * alignment.  The paper aligns the detectors' SNR series at integer samples
+ * ("Time offsets of SNRs from different detectors"); this call
+ * resamples, around every candidate, the window z[k - H .. k + H] of each
+ * detector `factor` times finer with the cubic Lagrange interpolator through the
+ * four neighbouring samples, so that coherent_sky_search can run unchanged on the
+ * windows with a table built at factor * fs_hz:
+ *   dev_out[I][s][u] = z_I(row_s, k_s - H + u / factor), u = 0 .. 2 factor H
+ *   (row stride padded to an even number of elements; samples with u a multiple
+ *   of factor are bit copies; the others are w0 z[b-1] + w1 z[b] + w2 z[b+1] +
+ *   w3 z[b+2] in float32: one multiply, then three fused multiply-adds per
+ *   component, weights formed in float64 and rounded once).
+ *   dev_trig_out[s] = the candidate re-addressed to its window: tmpl = s,
+ *   k = factor * H, det / z / snr kept; valid = 0 (and an all-zero window) when
+ *   the slot is empty or k - H - 1 .. k + H + 1 is not inside the view.
+ *   *out_view describes dev_out (rows = slots).  factor 1..16; H must cover the
+ *   largest inter-detector delay in input samples.  dev_out: 16-byte aligned,
+ *   spiir_snr_upsample_elems() complex elements, caller-owned.  Asynchronous on
+ *   `stream`.  Errors: EINVAL, ECUDA. */
+int spiir_snr_upsample_elems(int32_t n_det, int32_t n_slots, int32_t factor, int32_t half_width, size_t* elems);
+int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const spiir_trigger* dev_trig,
+                               int32_t n_slots, int32_t factor, int32_t half_width, spiir_c32* dev_out,
+                               spiir_trigger* dev_trig_out, spiir_snr_view* out_view, void* stream);
+
 /* A look-up table prepared for the device (opaque).  The plan re-orders the
  * directions so that those sharing one tuple of inter-detector delays are
  * adjacent, and stores for each direction the projector U2 U2^T (Eq. 28,

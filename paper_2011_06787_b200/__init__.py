@@ -7,7 +7,7 @@ callers for device memory and streams only.  Nothing here imports ``oracle``.
 from .binding import (  # noqa: F401
     lib, last_error, SpiirError, EXPORTS, LIB_PATH,
     spiir_bank_desc, spiir_snr_view, spiir_band_plan, TRIGGER_DTYPE, RESULT_DTYPE,
-    make_desc, Bank, SkyPlan, SkyPlanSet, SnrView, sky_table_build, sky_table_set_build, sky_table_nearest,
+    make_desc, Bank, SkyPlan, SkyPlanSet, SnrView, sky_table_build, sky_table_set_build, sky_table_nearest, upsample_windows,
     triggers_to_numpy, triggers_from_numpy, results_to_numpy, fp32_peak_probe,
     XI2_DTYPE, template_autocorr, signal_consistency, xi2_to_numpy,
     RANK_DTYPE, spiir_rank_bins, Ranker, rank_to_numpy, pipe_probe,

@@ -833,3 +833,83 @@ def test_sky_table_set_nearest_in_time(sp, U):
         with pytest.raises(sp.SpiirError):
             pset.select(t)
     pset.close()
+
+
+# ------------------------------------------------------------------ NEXT-3: sub-sample alignment
+def test_sub_sample_alignment(sp, U):
+    """spiir_snr_upsample_windows + coherent_sky_search with a table at R x 2048 Hz, against oracle O11
+    (cubic Lagrange in float64) + O6.  Windows: bit copies at the input samples, 1e-6 of the window's
+    largest |z| elsewhere; search: stage-isolated on the GPU's windows and end to end on the oracle's."""
+    import torch
+    rng = np.random.default_rng(77)
+    ns, fs, R, H = 8, 2048.0, 3, 58       # R = 3: the widest windows (trigger in V1) of 32 pairs still fit shared memory
+    cfg = workloads.config(3)
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    U1, d1 = oracle.sky_table(ns, pos, resp, cfg["sigma"], 0.9, fs)
+    UR, dR = oracle.sky_table(ns, pos, resp, cfg["sigma"], 0.9, fs * R)
+    assert np.abs(d1 - d1[:, :1]).max() < H
+    th, ph = oracle.healpix_ring_centres(ns)
+    lam = ph - 0.9
+    nvec = np.stack([np.sin(th) * np.cos(lam), np.sin(th) * np.sin(lam), np.cos(th)], 1)
+    tau = -(nvec @ pos.T) / workloads.C_LIGHT * fs                  # arrival offsets in samples, not rounded
+    D, rows, L, k_newest = 3, 40, 700, 1000                         # ring holds k = 301 .. 1000, wrapped
+    z = (rng.standard_normal((D, rows, L)) + 1j * rng.standard_normal((D, rows, L))) * math.sqrt(0.5)
+    kk = np.arange(k_newest - L + 1, k_newest + 1)
+    trig = np.zeros(rows, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1
+    trig["tmpl"] = rng.permutation(rows)
+    trig["det"] = rng.integers(0, D, rows)
+    trig["k"] = rng.integers(301 + H + 1, 1000 - H - 1, rows)
+    trig["k"][:6] = [301 + H + 1, 301 + H, 1000 - H - 1, 1000 - H, 650, 700]   # both edges, in and out
+    trig["valid"][4] = 0
+    p_true = rng.integers(0, 768, rows)
+    for s in range(6, rows):                                       # loud signals arriving between samples
+        T, r, k0 = int(trig["det"][s]), int(trig["tmpl"][s]), int(trig["k"][s])
+        c = (rng.standard_normal(2) + 1j * rng.standard_normal(2)) * 8.0
+        amp = U1[p_true[s]] @ c
+        for I in range(D):
+            x = kk - k0 - (tau[p_true[s], I] - tau[p_true[s], T])
+            z[I, r, kk % L] += amp[I] * np.exp(-x ** 2 / (2 * 6.0 ** 2)) * np.exp(0.3j * x)
+    z32 = z.astype(np.complex64)
+    trig["z_re"] = z32[trig["det"], trig["tmpl"], trig["k"] % L].real
+    trig["z_im"] = z32[trig["det"], trig["tmpl"], trig["k"] % L].imag
+    trig["snr"] = np.abs(z32[trig["det"], trig["tmpl"], trig["k"] % L])
+    zt = torch.from_numpy(np.ascontiguousarray(z32).view(np.float32).reshape(D, rows, L, 2)).cuda()
+    view = sp.SnrView(zt, k_newest=k_newest)
+    wview, wtrig = sp.upsample_windows(view, D, sp.triggers_from_numpy(trig), rows, R, H)
+    torch.cuda.synchronize()
+    Lw = 2 * R * H + 1
+    Lp = wview.c.row_stride
+    assert Lp == Lw + 1 and wview.c.ring_len == Lp and wview.c.k_newest == Lw - 1 and wview.c.det_stride == rows * Lp
+    g = wview._keep.cpu().numpy().reshape(-1)[:D * rows * Lp * 2].view(np.complex64).reshape(D, rows, Lp)
+    ref, ok = oracle.upsample_windows(z32, L, k_newest, trig["valid"], trig["tmpl"], trig["det"], trig["k"], R, H)
+    assert list(ok[:6]) == [1, 0, 1, 0, 0, 1] and ok[6:].all()
+    t2 = wtrig.cpu().numpy().view(sp.TRIGGER_DTYPE).reshape(-1)
+    assert np.array_equal(t2["valid"], ok) and np.array_equal(t2["tmpl"], np.arange(rows))
+    assert np.all(t2["k"] == R * H)
+    v = ok == 1
+    for f in ("det", "z_re", "z_im", "snr"):
+        assert np.array_equal(t2[f][v], trig[f][v])
+    assert np.all(g[:, :, Lw:] == 0) and np.all(g[:, ~v] == 0)
+    assert np.array_equal(g[:, v, 0:Lw:R], ref[:, v, 0:Lw:R].astype(np.complex64))     # bit copies
+    scale = np.abs(ref).max(axis=2, keepdims=True)
+    assert np.all(np.abs(g[:, :, :Lw] - ref) <= 1e-6 * scale + 1e-30)
+    # search on the windows
+    plan = sp.SkyPlan(UR.astype(np.float32), dR, max_slots=rows)
+    res = sp.results_to_numpy(plan.search(wview, wtrig, rows))
+    torch.cuda.synchronize()
+    U.check_sky(res, np.ascontiguousarray(g), Lp, Lw - 1, UR.astype(np.float32), dR, t2)   # stage-isolated
+    refp = np.zeros((D, rows, Lp), complex)
+    refp[:, :, :Lw] = ref
+    oo, op, _ = oracle.sky_search(UR.astype(np.float32), dR, refp, rows * Lp, Lp, Lp, Lw - 1,
+                                  ok, np.arange(rows), trig["det"], np.full(rows, R * H))      # end to end
+    assert np.all(np.abs(res["coh2"][v] - oo[v, 0, 0]) <= 1e-4 * oo[v, 0, 0])
+    assert np.all(res["pix"][~v] == -1)
+    # against the integer-sample search of the same candidates: less null power, true pixel found
+    plan1 = sp.SkyPlan(U1.astype(np.float32), d1, max_slots=rows)
+    res1 = sp.results_to_numpy(plan1.search(view, sp.triggers_from_numpy(trig), rows))
+    torch.cuda.synchronize()
+    sig = np.arange(rows) >= 6
+    assert np.mean(res["null2"][sig]) < np.mean(res1["null2"][sig])
+    assert np.mean(res["pix"][sig] == p_true[sig]) >= np.mean(res1["pix"][sig] == p_true[sig])
+    assert np.mean(res["pix"][sig] == p_true[sig]) > 0.5
