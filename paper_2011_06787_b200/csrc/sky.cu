@@ -16,9 +16,9 @@
 //     refreshes the real products q_IJ = Re(z_I conj z_J) the changed rows enter; each
 //     direction then costs one N_q-term dot product (1 FMUL + 5 FFMA for three
 //     detectors, issued for two pairs at a time as packed FFMA2 with the weight as a
-//     scalar-broadcast operand) and ONE FMNMX for the running maximum.  Which
-//     direction holds the maximum is recovered afterwards by rescanning the one chunk
-//     that last raised it.
+//     scalar-broadcast operand) and one FMNMX3 per TWO directions for the running
+//     maximum.  Which direction holds the maximum is recovered afterwards by rescanning
+//     the one chunk that last raised it.
 //   * thread = K (trigger, slide) pairs; a CTA owns 32 K pairs whose delay windows
 //     (the only samples any direction can touch) sit in shared memory, pair-major:
 //     one TMA bulk copy per (pair, detector) window (cp.async.bulk + mbarrier; 8-byte
@@ -85,6 +85,12 @@ __device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src_gmem)
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // q_IJ = Re(v_I conj v_J), the same two roundings wherever it is formed (main loop and rescan)
+// max of three (one FMNMX3 on sm_100; the same NaN rule as fmaxf)
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+  float r;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+  return r;
+}
 __device__ __forceinline__ float re_prod(float2 x, float2 y) { return __fmaf_rn(x.x, y.x, __fmul_rn(x.y, y.y)); }
 
 template <int NQ>
@@ -245,7 +251,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     __syncthreads();
 
     // ---- the direction stream: this warp's chunks.  Only the running maximum is kept per direction
-    //      (one FMNMX); which chunk raised it last is noted per chunk, and that chunk is rescanned below.
+    //      (one FMNMX3 per two directions); which chunk raised it last is noted per chunk, and that chunk is rescanned below.
     float2 vT[K], v[NO][K];
     float best[K], seen[K]; int bch[K];
     float2 qp[(K + 1) / 2][NQ];                          // products of pairs (2i, 2i+1) side by side: packed FFMA2 operands
@@ -278,6 +284,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       float4 nxt[SW / 4];
 #pragma unroll
       for (int c = 0; c < SW / 4; ++c) nxt[c] = reinterpret_cast<const float4*>(mytile)[c];
+      float pend[K];
 #pragma unroll 4
       for (int s = 0; s < kSkyChunk; ++s) {
         float w[SW];
@@ -328,7 +335,9 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
           if (MAP) {
             if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = cval[a];
           }
-          best[a] = fmaxf(best[a], cval[a]);
+          // two directions per maximum: the value of an even slot waits for its odd neighbour (one FMNMX3)
+          if (s & 1) best[a] = fmax3(best[a], pend[a], cval[a]);
+          else       pend[a] = cval[a];
         }
       }
 #undef SKY_Q
