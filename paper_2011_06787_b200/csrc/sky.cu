@@ -85,6 +85,11 @@ __device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src_gmem)
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // q_IJ = Re(v_I conj v_J), the same two roundings wherever it is formed (main loop and rescan)
+__device__ __forceinline__ float2 lds64(uint32_t addr) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+  return v;
+}
 // max of three (one FMNMX3 on sm_100; the same NaN rule as fmaxf)
 __device__ __forceinline__ float fmax3(float a, float b, float c) {
   float r;
@@ -257,11 +262,11 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     float2 qp[(K + 1) / 2][NQ];                          // products of pairs (2i, 2i+1) side by side: packed FFMA2 operands
 #define SKY_Q(a, e) (((a) & 1) ? qp[(a) >> 1][e].y : qp[(a) >> 1][e].x)
     long long mrow[K];                                  // sky-map row of each pair, -1 = none
-    int pb[K];                                          // element offset of pair a's block, plus its windows' parity
+    uint32_t pb[K];                                     // shared-space byte address of pair a's block, plus its windows' parity
 #pragma unroll
     for (int a = 0; a < K; ++a) {
       const PairInfo pi = pinfo[lane + 32 * a];
-      pb[a] = (lane + 32 * a) * PS + ((lane >> 3) & 1);
+      pb[a] = (uint32_t)__cvta_generic_to_shared(win + (lane + 32 * a) * PS + ((lane >> 3) & 1));
       vT[a] = pi.vT; best[a] = -1.f; seen[a] = -1.f; bch[a] = c_beg;
       mrow[a] = (MAP && pi.valid) ? (long long)pi.slot * P.n_pix : -1;
 #pragma unroll
@@ -301,10 +306,11 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
           for (int o = 0; o < NO; ++o) {
             if (level <= o) {
-              const float2* rp = win + ((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1));
+              // 32-bit shared-space addresses: one IADD per gather instead of a 64-bit generic address
+              const uint32_t ro = (uint32_t)((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1)) * 8u;
 #pragma unroll
               for (int a = 0; a < K; ++a) {
-                const float2 x = rp[pb[a]];
+                const float2 x = lds64(pb[a] + ro);
                 v[o][a] = x;
                 SKY_Q(a, 1 + o) = re_prod(x, x);
                 SKY_Q(a, 1 + NO + o) = re_prod(vT[a], x);
