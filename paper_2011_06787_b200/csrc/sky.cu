@@ -50,12 +50,12 @@ template <int D> struct SkyFmt {
 // One slot per direction, SW words: words [0,NQ) weights, word NQ = pixel, word NQ+1 = control.
 //   Weight order (T = trigger detector, o = others in increasing detector index): M_TT; M_oo (o = 0..NO-1);
 //   2 M_To; 2 M_o'o for o' < o, (0,1) (0,2) (1,2).
-//   control = level | f_0 << 2 | f_1 << 12 | f_2 << 22: f_o = element offset, inside a pair's block of
+//   control = nref | f_0 << 2 | f_1 << 12 | f_2 << 22: f_o = element offset, inside a pair's block of
 //   windows, of the sample of other detector o this direction reads (segment offset + row, < 1024);
-//   level = first other detector whose row
-//   differs from the previous slot (0 for the first slot of a warp's share of the stream: refresh
-//   everything; NO: same delay tuple, nothing to refresh).
-// The last chunk is padded with copies of the last direction (level NO).
+//   nref = NO - (first other detector whose row differs from the previous slot): the last nref
+//   detectors are refreshed (NO for the first slot of a warp's share of the stream: refresh
+//   everything; 0: same delay tuple, nothing to refresh — one bit test on the common path).
+// The last chunk is padded with copies of the last direction (nref 0).
 constexpr int kSkyRowBits = 10;
 
 struct SkyParams {
@@ -300,12 +300,12 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         for (int c = 0; c < SW / 4; ++c)
           nxt[c] = reinterpret_cast<const float4*>(mytile + ((s + 1) & (kSkyChunk - 1)) * SW)[c];
         const int ctrl = __float_as_int(w[NQ + 1]);
-        const int level = ctrl & 3;
-        if (level < NO) {
+        const int nref = ctrl & 3;
+        if (nref) {
           // new delay tuple: gather the rows that changed, refresh the products they enter
 #pragma unroll
           for (int o = 0; o < NO; ++o) {
-            if (level <= o) {
+            if (o >= NO - nref) {
               // 32-bit shared-space addresses: one IADD per gather instead of a 64-bit generic address
               const uint32_t ro = (uint32_t)((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1)) * 8u;
 #pragma unroll
@@ -511,7 +511,7 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
     if (r >= n_pix) {                      // padding: the last direction again, nothing to refresh
       memcpy(w, w - SW, (size_t)SW * 4);
       int32_t ctrl; memcpy(&ctrl, w + NQ + 1, 4);
-      ctrl = (ctrl & ~3) | NO;
+      ctrl &= ~3;
       memcpy(w + NQ + 1, &ctrl, 4);
       continue;
     }
@@ -536,7 +536,7 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
       for (int o2 = 0; o2 < o; ++o2) w[1 + 2 * NO + o * (o - 1) / 2 + o2] = (float)(2.0 * M(oth[o2], oth[o]));
     const int32_t pix = p;
     memcpy(w + NQ, &pix, 4);
-    int32_t ctrl = level;
+    int32_t ctrl = NO - level;             // how many of the other detectors' rows to refresh, the last ones
     for (int o = 0; o < NO; ++o) ctrl |= rw[o] << (2 + kSkyRowBits * o);
     memcpy(w + NQ + 1, &ctrl, 4);
   }
