@@ -58,12 +58,22 @@ template <int D> struct SkyFmt {
 // The last chunk is padded with copies of the last direction (nref 0).
 constexpr int kSkyRowBits = 10;
 
+// One candidate as k_sky_bin leaves it for k_sky: everything a (candidate, slide) pair needs from the
+// trigger and the trigger detector's SNR in ONE 32-byte read (the chain list -> trigger -> z would be
+// three dependent HBM latencies at the head of every batch, and z_T the same for all slides).
+struct __align__(16) SkyRec {
+  int32_t slot, row;
+  int64_t k;
+  float2 vT;                  // z_T(row, k); zero when k is outside the view
+  int32_t k_ok, _pad;
+};
+
 struct SkyParams {
   const float* stream; int32_t n_chunks, chunks_per_warp;     // this trigger detector's stream; contiguous share per warp
   int32_t n_pix;
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
   const spiir_trigger* trig;
-  const int32_t* list; const int32_t* counts;                 // slots of trigger detector T
+  const SkyRec* list; const int32_t* counts;                  // candidates of trigger detector T
   int32_t T;
   int32_t n_slides;                                           // 0 = foreground
   int64_t step; int32_t mult[SPIIR_MAX_DET];
@@ -142,19 +152,19 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
       PairInfo pi; pi.slot = -1; pi.slide = 0; pi.valid = 0; pi.row = 0; pi.vT = make_float2(0.f, 0.f); pi.k = 0;
       const long long q = batch * NP + tid;
       if (q < n_pairs) {
-        pi.slot = P.list[q / S1];
+        const SkyRec rc = P.list[q / S1];
+        pi.slot = rc.slot;
         pi.slide = (int)(q % S1) + (P.n_slides > 0 ? 1 : 0);
-        const spiir_trigger tr = P.trig[pi.slot];
-        pi.row = tr.tmpl; pi.k = tr.k;
-        bool ok = tr.k >= kmin && tr.k <= P.k_newest;
+        pi.row = rc.row; pi.k = rc.k;
+        bool ok = rc.k_ok != 0;
 #pragma unroll
         for (int I = 0; I < D; ++I) {
           if (I == T) continue;
-          const int64_t k0 = tr.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I];
+          const int64_t k0 = rc.k - (int64_t)pi.slide * P.step * P.mult[I] + P.lo[I];
           ok = ok && k0 >= kmin && k0 + P.W[I] - 1 <= P.k_newest;
         }
         pi.valid = ok ? 1 : 0;
-        if (ok) pi.vT = P.z[(size_t)T * P.det_stride + (size_t)tr.tmpl * P.row_stride + (size_t)(tr.k % P.ring_len)];
+        if (ok) pi.vT = rc.vT;
       }
       pinfo[tid] = pi;
     }
@@ -428,14 +438,22 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 
 // valid slots -> per-detector lists; invalid slots get their "no result" rows here
 __global__ void __launch_bounds__(256) k_sky_bin(const spiir_trigger* trig, int n_slots, int n_det, int S1,
-                                                 int32_t* lists, int32_t* counts, int max_slots,
+                                                 const float2* z, int64_t det_stride, int64_t row_stride,
+                                                 int64_t ring_len, int64_t k_newest,
+                                                 SkyRec* lists, int32_t* counts, int max_slots,
                                                  spiir_sky_result* out) {
   const int i = blockIdx.x * 256 + threadIdx.x;
   if (i >= n_slots) return;
   const spiir_trigger t = trig[i];
   if (t.valid && t.det >= 0 && t.det < n_det) {
+    const int64_t kmin = (k_newest - ring_len + 1 > 0) ? k_newest - ring_len + 1 : 0;
+    SkyRec rc;
+    rc.slot = i; rc.row = t.tmpl; rc.k = t.k; rc._pad = 0;
+    rc.k_ok = (t.k >= kmin && t.k <= k_newest) ? 1 : 0;
+    rc.vT = rc.k_ok ? z[(size_t)t.det * det_stride + (size_t)t.tmpl * row_stride + (size_t)(t.k % ring_len)]
+                    : make_float2(0.f, 0.f);
     const int pos = atomicAdd(counts + t.det, 1);
-    lists[(size_t)t.det * max_slots + pos] = i;
+    lists[(size_t)t.det * max_slots + pos] = rc;
   } else {
     spiir_sky_result r; r.coh2 = 0.f; r.null2 = 0.f; r.tot2 = 0.f; r.pix = -1;
     for (int s = 0; s < S1; ++s) out[(size_t)i * S1 + s] = r;
@@ -477,7 +495,7 @@ static void sky_layout(spiir_sky_plan* pl) {
   for (int T = 0; T < D; ++T) {
     pl->st[T].off_slots = cur; cur = sky_align(cur + (size_t)pl->cap_slots * pl->SW * 4);
   }
-  pl->off_lists = cur;  cur = sky_align(cur + (size_t)D * pl->max_slots * 4);
+  pl->off_lists = cur;  cur = sky_align(cur + (size_t)D * pl->max_slots * sizeof(SkyRec));
   pl->off_counts = cur; cur = sky_align(cur + SPIIR_MAX_DET * 4);
   pl->bytes = cur;
 }
@@ -657,10 +675,12 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
   if (n_slots == 0) return SPIIR_OK;
   const int D = pl->n_det, S1 = n_slides > 0 ? n_slides : 1;
   int32_t* counts = (int32_t*)(pl->ws + pl->off_counts);
-  int32_t* lists = (int32_t*)(pl->ws + pl->off_lists);
+  SkyRec* lists = (SkyRec*)(pl->ws + pl->off_lists);
   SPIIR_CUDA_OK(cudaMemsetAsync(counts, 0, SPIIR_MAX_DET * 4, st));
   if (map) SPIIR_CUDA_OK(cudaMemsetAsync(map, 0, (size_t)n_slots * pl->n_pix * sizeof(float), st));
-  k_sky_bin<<<(n_slots + 255) / 256, 256, 0, st>>>(trig, n_slots, D, S1, lists, counts, pl->max_slots, out);
+  k_sky_bin<<<(n_slots + 255) / 256, 256, 0, st>>>(trig, n_slots, D, S1, (const float2*)view->dev_z, view->det_stride,
+                                                   view->row_stride, view->ring_len, view->k_newest, lists, counts,
+                                                   pl->max_slots, out);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());
   // pairs one launch can see at most (the real count is on the device): all slots of one detector
