@@ -582,7 +582,7 @@ def run_ours(args):
     if has_sky and evals:
         roof_sky = alu_roofline("k_sky (coherent search + slides, H5+H6)", FLOP_PER_EVAL * evals, ms_sky,
                                 2 * D * K if S else D * K, ffma_rate, NCU_TRAFFIC_BYTES["k_sky"],
-                                issue_ops=7.0 * evals)
+                                issue_ops=6.5 * evals)
     dominant, other = (roof_bank, roof_sky) if (roof_sky is None or ms_rec >= ms_sky) else (roof_sky, roof_bank)
     line = {
         "metric": METRIC, "value": upd_all / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
