@@ -131,6 +131,20 @@ def test_table_set_and_nearest_selection_match_the_oracle(sp):
     assert sp.lib().spiir_sky_table_nearest(float("nan"), 0.0, 1.0, 4, C.byref(idx)) != sp.SPIIR_OK
 
 
+def test_upsample_window_sizing_and_argument_checks(sp):
+    """spiir_snr_upsample_elems (host only): [n_det][n_slots][2 R H + 1 padded to even] complex elements."""
+    n = C.c_size_t(0)
+    for D, S, R, H in ((3, 10, 4, 58), (2, 0, 1, 1), (4, 7, 16, 5), (1, 3, 3, 2)):
+        assert sp.lib().spiir_snr_upsample_elems(D, S, R, H, C.byref(n)) == sp.SPIIR_OK
+        Lw = 2 * R * H + 1
+        assert n.value == D * S * (Lw + (Lw & 1))
+    for D, S, R, H in ((0, 1, 2, 2), (5, 1, 2, 2), (3, -1, 2, 2), (3, 1, 0, 2), (3, 1, 17, 2), (3, 1, 2, 0)):
+        assert sp.lib().spiir_snr_upsample_elems(D, S, R, H, C.byref(n)) == sp.SPIIR_EINVAL
+    assert sp.lib().spiir_snr_upsample_elems(3, 1, 2, 2, None) == sp.SPIIR_EINVAL
+    # NULL view / buffers are refused before any device work
+    assert sp.lib().spiir_snr_upsample_windows(None, 3, None, 1, 2, 2, None, None, None, None) == sp.SPIIR_EINVAL
+
+
 def test_product_package_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2011_06787_b200")
     for dp, _, fs in os.walk(pkg):
