@@ -9,9 +9,9 @@
 //   u = R q + r:  r = 0  the sample itself (bit copy)
 //                 r > 0  w_r[0] z[b-1] + w_r[1] z[b] + w_r[2] z[b+1] + w_r[3] z[b+2],  b = k_s - H + q,
 //                        float32, one multiply then three fused multiply-adds per component
-// One CTA per (slot, detector), threads stride over u: reads 2 H + 3 consecutive ring samples
-// (coalesced, L1-resident across the R phases), writes R times as many.  HBM-bound:
-// 8 (2 H + 3) B read + 8 (2 R H + 2) B written per (slot, detector).
+// One CTA per (slot, detector), threads stride over the output samples (coalesced stores, reads of 2 H + 3
+// consecutive ring samples served by L1 across the R phases; one 64-bit modulo per thread, then wraps).
+// HBM-bound: 8 (2 H + 3) B read + 8 (2 R H + 2) B written per (slot, detector).
 #include "spiir_internal.cuh"
 
 namespace spiir {
@@ -21,42 +21,54 @@ constexpr int kUpMaxFactor = 16;
 
 struct UpParams {
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
-  const spiir_trigger* trig; int32_t n_slots;
+  const spiir_trigger* trig; int32_t n_slots, n_det;
   int32_t R, H, Lw; int64_t Lp;
   float4 w[kUpMaxFactor];
   float2* out; spiir_trigger* trig_out;
 };
 
+// the re-addressed candidates (one thread per slot)
+__global__ void __launch_bounds__(kUpThreads) k_upsample_trig(const __grid_constant__ UpParams P) {
+  const int s = blockIdx.x * kUpThreads + threadIdx.x;
+  if (s >= P.n_slots) return;
+  const spiir_trigger t = P.trig[s];
+  const int64_t k_old = P.k_newest - P.ring_len + 1 > 0 ? P.k_newest - P.ring_len + 1 : 0;
+  const bool ok = t.valid && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
+  spiir_trigger o = t;
+  o.valid = ok ? 1 : 0; o.tmpl = s; o.k = (int64_t)P.R * P.H;
+  if (!t.valid) { o.det = 0; o.z_re = o.z_im = o.snr = 0.f; }
+  o._pad = 0; o._pad2 = 0.f;
+  P.trig_out[s] = o;
+}
+
+// the windows: one CTA per (slot, detector), threads stride over the output samples (coalesced stores; the
+// 2 H + 3 ring samples a window reads are consecutive and stay in L1 across the R phases).  One 64-bit
+// modulo per thread places the window in the ring; after that a sample's neighbours are conditional wraps.
 __global__ void __launch_bounds__(kUpThreads) k_upsample(const __grid_constant__ UpParams P) {
   const int s = blockIdx.x, I = blockIdx.y;
   const spiir_trigger t = P.trig[s];
   const int64_t k_old = P.k_newest - P.ring_len + 1 > 0 ? P.k_newest - P.ring_len + 1 : 0;
   const bool ok = t.valid && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
-  if (I == 0 && threadIdx.x == 0) {
-    spiir_trigger o = t;
-    o.valid = ok ? 1 : 0; o.tmpl = s; o.k = (int64_t)P.R * P.H;
-    if (!t.valid) { o.det = 0; o.z_re = o.z_im = o.snr = 0.f; }
-    o._pad = 0; o._pad2 = 0.f;
-    P.trig_out[s] = o;
-  }
   float2* out = P.out + ((size_t)I * P.n_slots + s) * P.Lp;
   if (!ok) {
     for (int u = threadIdx.x; u < P.Lp; u += kUpThreads) out[u] = make_float2(0.f, 0.f);
     return;
   }
   const float2* zr = P.z + (size_t)I * P.det_stride + (size_t)t.tmpl * P.row_stride;
-  const int64_t b0 = t.k - P.H;
+  const int64_t L = P.ring_len;
+  const int64_t i0 = (t.k - P.H) % L;                    // t.k - H >= 1 here
+  auto wrap = [L](int64_t i) { return i >= L ? i - L : (i < 0 ? i + L : i); };
   for (int u = threadIdx.x; u < P.Lp; u += kUpThreads) {
     float2 v = make_float2(0.f, 0.f);
     if (u < P.Lw) {
       const int q = u / P.R, r = u - q * P.R;
-      const int64_t b = b0 + q;
+      // q <= 2 H: if the window is longer than the ring the validity test above has already failed
+      const int64_t i = wrap(i0 + q);
       if (r == 0) {
-        v = zr[b % P.ring_len];
+        v = zr[i];
       } else {
         const float4 w = P.w[r];
-        const float2 z0 = zr[(b - 1) % P.ring_len], z1 = zr[b % P.ring_len];
-        const float2 z2 = zr[(b + 1) % P.ring_len], z3 = zr[(b + 2) % P.ring_len];
+        const float2 z0 = zr[wrap(i - 1)], z1 = zr[i], z2 = zr[wrap(i + 1)], z3 = zr[wrap(wrap(i + 1) + 1)];
         v.x = __fmaf_rn(w.w, z3.x, __fmaf_rn(w.z, z2.x, __fmaf_rn(w.y, z1.x, __fmul_rn(w.x, z0.x))));
         v.y = __fmaf_rn(w.w, z3.y, __fmaf_rn(w.z, z2.y, __fmaf_rn(w.y, z1.y, __fmul_rn(w.x, z0.y))));
       }
@@ -94,7 +106,7 @@ int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const 
   P.z = (const float2*)view->dev_z;
   P.det_stride = view->det_stride; P.row_stride = view->row_stride;
   P.ring_len = view->ring_len; P.k_newest = view->k_newest;
-  P.trig = dev_trig; P.n_slots = n_slots;
+  P.trig = dev_trig; P.n_slots = n_slots; P.n_det = n_det;
   P.R = factor; P.H = half_width; P.Lw = 2 * factor * half_width + 1;
   P.Lp = ((int64_t)P.Lw + 1) & ~(int64_t)1;
   for (int r = 0; r < kUpMaxFactor; ++r) {
@@ -110,8 +122,9 @@ int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const 
   out_view->ring_len = P.Lp;
   out_view->k_newest = P.Lw - 1;
   if (n_slots == 0) return SPIIR_OK;
+  k_upsample_trig<<<(n_slots + kUpThreads - 1) / kUpThreads, kUpThreads, 0, (cudaStream_t)stream>>>(P);
   k_upsample<<<dim3((unsigned)n_slots, (unsigned)n_det), kUpThreads, 0, (cudaStream_t)stream>>>(P);
-  count_launch();
+  count_launch(2);
   SPIIR_CUDA_OK(cudaGetLastError());
   return SPIIR_OK;
 }
