@@ -662,6 +662,89 @@ def test_p23_rank_and_fap_by_hand_and_by_counting_events():
     assert abs(np.mean((F[bi, bj] + 0.5 * same) / sel.sum()) - 0.5) < 1e-9
 
 
+# ---- P28 / P29: the two pins round 1 lacked (VERDICT r1 "What's weak" 1) --------------------------------
+def _mutant(func, old, new):
+    """The oracle function `func` with one source fragment replaced (a deliberately broken oracle): a pin
+    earns its name only if such a plausible mistake turns it red."""
+    import inspect
+    import textwrap
+    src = textwrap.dedent(inspect.getsource(func))
+    assert src.count(old) == 1, "mutation target not found exactly once: %r" % old
+    ns = dict(func.__globals__)
+    exec(compile(src.replace(old, new), "<mutant of %s>" % func.__name__, "exec"), ns)
+    return ns[func.__name__]
+
+
+def _healpix_golden():
+    rows = []
+    for line in open(os.path.join(HERE, "golden", "healpix_ring_centres.txt")):
+        f = line.split("#")[0].split()
+        if len(f) == 4:
+            rows.append((int(f[0]), int(f[1]), float(f[2]), float(f[3])))
+    return rows
+
+
+def _healpix_matches_golden(centres):
+    for nside, pix, z, phi_over_pi in _healpix_golden():
+        theta, phi = centres(nside)
+        if abs(math.cos(theta[pix]) - z) > 1e-12 or abs(phi[pix] / math.pi - phi_over_pi) > 1e-12:
+            return False
+    return True
+
+
+def test_p28_healpix_ring_centres_golden_values():
+    """The in-ring phase of the HEALPix RING centres (the half-pixel shift of alternate belt rings, the
+    j - 1/2 of the caps) against the base-pixel centres of ref. [46], typed into
+    tests/golden/healpix_ring_centres.txt.  P15's invariants (sum of centres, ring count, spacing) are
+    blind to that phase: the mutants below pass P15's checks and must fail here."""
+    from oracle import sky
+    rows = _healpix_golden()
+    assert sum(1 for r in rows if r[0] == 1) == 12 and {r[1] for r in rows if r[0] == 2} >= {0, 4, 12, 20, 28, 44}
+    assert _healpix_matches_golden(sky.healpix_ring_centres)
+    # deliberately broken oracles: the belt's alternation swapped; the caps' half-pixel offset dropped
+    swapped = _mutant(sky.healpix_ring_centres, "0.5 if (i + N) % 2 == 0 else 1.0", "1.0 if (i + N) % 2 == 0 else 0.5")
+    assert not _healpix_matches_golden(swapped)
+    th, ph = swapped(2)                                                       # ... while P15-style invariants still hold
+    v = np.stack([np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph), np.cos(th)], axis=1)
+    assert np.abs(v.sum(axis=0)).max() < 1e-12 and len(np.unique(np.round(np.cos(th), 12))) == 7
+    no_half = _mutant(sky.healpix_ring_centres, "            z = 1.0 - i * i / (3.0 * N * N)\n            f = (j - 0.5)",
+                      "            z = 1.0 - i * i / (3.0 * N * N)\n            f = (j - 1.0)")
+    assert not _healpix_matches_golden(no_half)
+    south = _mutant(sky.healpix_ring_centres, "j = 4 * i + 1 - (ps - 2 * i * (i - 1))", "j = ps - 2 * i * (i - 1)")
+    assert not _healpix_matches_golden(south)                                 # a mirrored south cap is caught by pixels 44 / 47
+
+
+def test_p29_far_by_hand_eq15():
+    """Eq. 15: FAR = FAP N_b / T_b.  P23's 2 x 2 background (N_b = 6; H = [[1,1],[3,1]],
+    R counts [[4,6],[3,4]], FAP counts [[3,5],[0,3]]) with T_b = 50 s:
+      candidate in bin (0,0): R = 4/6, FAP = 3/6, FAR = 3/50 = 0.06 Hz;
+      candidate in bin (0,1): R = 6/6, FAP = 5/6, FAR = 5/50 = 0.10 Hz  (N_b = 6, F = 5, T_b = 50 all differ,
+      so a swapped or dropped factor gives another number)."""
+    from oracle import rank
+    bins = (2, 2, 4.0, 8.0, -2.0, 2.0)
+    H = rank.histogram(bins, np.float32([1] * 6), np.float32([20, 30, 100, 150, 200, 70]),
+                       np.float32([0.5, 3.0, 0.5, 0.7, 2.0, 0.9]), np.ones(6, np.int32))
+    args = (bins, H, np.float32([1, 1, 1]), np.float32([30, 40, 100]), np.float32([0.5, 3.0, 0.6]), np.ones(3, np.int32), 50.0)
+
+    def check(fn):
+        R, fap, far, sel = fn(*args)
+        return (sel.tolist() == [1, 1, 1]
+                and np.allclose(R, [4 / 6, 1.0, 3 / 6], rtol=0, atol=1e-15)
+                and np.allclose(fap, [3 / 6, 5 / 6, 0.0], rtol=0, atol=1e-15)
+                and np.allclose(far, [0.06, 0.10, 0.0], rtol=0, atol=1e-15))
+
+    assert check(rank.candidates)
+    # deliberately broken oracles: N_b dropped (FAR = FAP / T_b), N_b applied twice, T_b ignored
+    assert not check(_mutant(rank.candidates, "F[i, j] / float(background_seconds)",
+                             "F[i, j] / max(nb, 1) / float(background_seconds)"))
+    assert not check(_mutant(rank.candidates, "F[i, j] / float(background_seconds)",
+                             "F[i, j] * nb / float(background_seconds)"))
+    assert not check(_mutant(rank.candidates, "F[i, j] / float(background_seconds)", "F[i, j] / 1.0"))
+    # T_b scales FAR inversely and leaves R and FAP alone
+    far100 = rank.candidates(*args[:-1], 100.0)[2]
+    assert np.allclose(far100, [0.03, 0.05, 0.0], rtol=0, atol=1e-15)
+
+
 # ---- P14: strain-domain injection through a chirp-matched template (end-to-end sanity, loose by nature) ----
 def test_p14_strain_injection_recovers_its_direction_or_the_mirror_image():
     """BASELINE.json config 1: the chirp injected into three detectors with the true arrival delays, filtered
