@@ -126,11 +126,13 @@ int spiir_peaks(spiir_bank* bank, float snr_threshold, int32_t mode,
 
 /* A window onto complex SNR series: z(det,row,k) = dev_z[det*det_stride +
  * row*row_stride + (k mod ring_len)] (strides in complex elements), defined for
- * max(0, k_newest - ring_len + 1) <= k <= k_newest. */
+ * 0 <= row < n_rows and max(0, k_newest - ring_len + 1) <= k <= k_newest.  A trigger
+ * slot whose tmpl is not a row of the view is treated as an empty slot.  48 bytes. */
 typedef struct {
   const spiir_c32* dev_z;
   int64_t det_stride, row_stride;
   int64_t ring_len, k_newest;
+  int64_t n_rows;
 } spiir_snr_view;
 
 /* The bank's own SNR ring as a view (rows = templates). */

@@ -40,7 +40,7 @@ class spiir_bank_desc(C.Structure):
 
 class spiir_snr_view(C.Structure):
     _fields_ = [("dev_z", C.c_void_p), ("det_stride", C.c_int64), ("row_stride", C.c_int64),
-                ("ring_len", C.c_int64), ("k_newest", C.c_int64)]
+                ("ring_len", C.c_int64), ("k_newest", C.c_int64), ("n_rows", C.c_int64)]
 
 
 class spiir_band_plan(C.Structure):
@@ -192,7 +192,7 @@ class SnrView:
         n_det, rows, ring_len, _ = z.shape
         self._keep = z
         self.c = spiir_snr_view(z.data_ptr(), rows * ring_len, ring_len, ring_len,
-                                ring_len - 1 if k_newest is None else int(k_newest))
+                                ring_len - 1 if k_newest is None else int(k_newest), rows)
 
 
 def upsample_windows(view, n_det, trig, n_slots, factor, half_width):

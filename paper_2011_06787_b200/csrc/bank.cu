@@ -522,6 +522,7 @@ int spiir_bank_snr_view(const spiir_bank* bk, spiir_snr_view* view) {
   view->det_stride = (int64_t)bk->desc.n_templates * bk->desc.ring_len;
   view->ring_len = bk->desc.ring_len;
   view->k_newest = bk->k_next - 1;
+  view->n_rows = bk->desc.n_templates;
   return SPIIR_OK;
 }
 

@@ -29,18 +29,15 @@
 //     one launch per trigger detector, persistent CTAs stride over the pair batches.
 #include <algorithm>
 #include <climits>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
-#include "spiir_internal.cuh"
+#include "sky_internal.cuh"
 
 namespace spiir {
 
-constexpr int kSkyThreads = 512;
-constexpr int kSkyWarps = kSkyThreads / 32;
-constexpr int kSkyChunk = 32;               // slots per stream chunk (one per lane when staging)
 constexpr int kSkyKMax = 4;                 // (trigger, slide) pairs per thread, at most
-constexpr int kSkySmemMax = 226 * 1024;     // opt-in dynamic shared memory per CTA on sm_100 (227 KB) less the static part
 
 template <int D> struct SkyFmt {
   static constexpr int NO = D - 1;                       // detectors other than the trigger detector
@@ -56,18 +53,6 @@ template <int D> struct SkyFmt {
 //   detectors are refreshed (NO for the first slot of a warp's share of the stream: refresh
 //   everything; 0: same delay tuple, nothing to refresh — one bit test on the common path).
 // The last chunk is padded with copies of the last direction (nref 0).
-constexpr int kSkyRowBits = 10;
-
-// One candidate as k_sky_bin leaves it for k_sky: everything a (candidate, slide) pair needs from the
-// trigger and the trigger detector's SNR in ONE 32-byte read (the chain list -> trigger -> z would be
-// three dependent HBM latencies at the head of every batch, and z_T the same for all slides).
-struct __align__(16) SkyRec {
-  int32_t slot, row;
-  int64_t k;
-  float2 vT;                  // z_T(row, k); zero when k is outside the view
-  int32_t k_ok, _pad;
-};
-
 struct SkyParams {
   const float* stream; int32_t n_chunks, chunks_per_warp;     // this trigger detector's stream; contiguous share per warp
   int32_t n_pix;
@@ -87,32 +72,11 @@ struct SkyParams {
 
 struct PairInfo { int32_t slot, slide, valid, row; float2 vT; long long k; unsigned char sh[8]; };   // sh[I]: 0/1 sample shift of detector I's window (TMA copies start 16-byte aligned)
 
-__device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src_gmem) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)),
-               "l"(src_gmem)
-               : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-// q_IJ = Re(v_I conj v_J), the same two roundings wherever it is formed (main loop and rescan)
-__device__ __forceinline__ float2 lds64(uint32_t addr) {
-  float2 v;
-  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
-  return v;
-}
-// max of three (one FMNMX3 on sm_100; the same NaN rule as fmaxf)
-__device__ __forceinline__ float fmax3(float a, float b, float c) {
-  float r;
-  asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
-  return r;
-}
-__device__ __forceinline__ float re_prod(float2 x, float2 y) { return __fmaf_rn(x.x, y.x, __fmul_rn(x.y, y.y)); }
-
 template <int NQ>
 __device__ __forceinline__ float quad_form(const float* __restrict__ w, const float (&q)[NQ]) {
-  float c = __fmul_rn(w[0], q[0]);
+  float c = __fmul_rn(w[1], q[1]);                     // the term of q[0] = |z_T|^2 is the constant 2 q[0] (trace of the projector)
 #pragma unroll
-  for (int e = 1; e < NQ; ++e) c = __fmaf_rn(w[e], q[e], c);
+  for (int e = 2; e < NQ; ++e) c = __fmaf_rn(w[e], q[e], c);
   return c;
 }
 
@@ -182,6 +146,9 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     //      16-byte aligned sample at or before the window (sh = 0/1 samples of shift); completion on an
     //      mbarrier.  Otherwise warps copy the windows with 8-byte cp.async.
     if (P.tma) {
+      // the windows were last written through the generic proxy (zero fill, in-place shift); the bulk copies below
+      // write them through the async proxy
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       if (tid < NP * NO) {
         const int j = tid / NO, o = tid - j * NO;
         const int I = o + (o >= T ? 1 : 0);
@@ -210,15 +177,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
           asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar_a) : "memory");
         }
       }
-      asm volatile(
-          "{\n"
-          ".reg .pred p;\n"
-          "SKY_WAIT:\n"
-          "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-          "@p bra SKY_DONE;\n"
-          "bra SKY_WAIT;\n"
-          "SKY_DONE:\n"
-          "}\n" ::"r"((uint32_t)__cvta_generic_to_shared(&bar)), "r"(bar_phase) : "memory");
+      mbar_wait_bounded((uint32_t)__cvta_generic_to_shared(&bar), bar_phase);
       bar_phase ^= 1u;
       // the copies landed with sample k0 at offset sh (0/1, from the source's alignment); move each window
       // so that it starts at the parity its lane wants: lanes l and l+8 of a half-warp then hit distinct banks
@@ -277,7 +236,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     for (int a = 0; a < K; ++a) {
       const PairInfo pi = pinfo[lane + 32 * a];
       pb[a] = (uint32_t)__cvta_generic_to_shared(win + (lane + 32 * a) * PS + ((lane >> 3) & 1));
-      vT[a] = pi.vT; best[a] = -1.f; seen[a] = -1.f; bch[a] = c_beg;
+      vT[a] = pi.vT; best[a] = -3.0e38f; seen[a] = -3.0e38f; bch[a] = c_beg;
       mrow[a] = (MAP && pi.valid) ? (long long)pi.slot * P.n_pix : -1;
 #pragma unroll
       for (int e = 0; e < NQ; ++e) SKY_Q(a, e) = 0.f;
@@ -322,7 +281,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
               for (int a = 0; a < K; ++a) {
                 const float2 x = lds64(pb[a] + ro);
                 v[o][a] = x;
-                SKY_Q(a, 1 + o) = re_prod(x, x);
+                SKY_Q(a, 1 + o) = __fsub_rn(re_prod(x, x), SKY_Q(a, 0));
                 SKY_Q(a, 1 + NO + o) = re_prod(vT[a], x);
 #pragma unroll
                 for (int o2 = 0; o2 < o; ++o2) SKY_Q(a, 1 + 2 * NO + o * (o - 1) / 2 + o2) = re_prod(v[o2][a], x);
@@ -335,21 +294,21 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         float cval[K];
 #pragma unroll
         for (int i = 0; i < K / 2; ++i) {
-          float2 c2 = __fmul2_rn(make_float2(w[0], w[0]), qp[i][0]);
+          float2 c2 = __fmul2_rn(make_float2(w[1], w[1]), qp[i][1]);
 #pragma unroll
-          for (int e = 1; e < NQ; ++e) c2 = __ffma2_rn(make_float2(w[e], w[e]), qp[i][e], c2);
+          for (int e = 2; e < NQ; ++e) c2 = __ffma2_rn(make_float2(w[e], w[e]), qp[i][e], c2);
           cval[2 * i] = c2.x; cval[2 * i + 1] = c2.y;
         }
         if (K & 1) {
-          float c = __fmul_rn(w[0], qp[K / 2][0].x);
+          float c = __fmul_rn(w[1], qp[K / 2][1].x);
 #pragma unroll
-          for (int e = 1; e < NQ; ++e) c = __fmaf_rn(w[e], qp[K / 2][e].x, c);
+          for (int e = 2; e < NQ; ++e) c = __fmaf_rn(w[e], qp[K / 2][e].x, c);
           cval[K - 1] = c;
         }
 #pragma unroll
         for (int a = 0; a < K; ++a) {
           if (MAP) {
-            if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = cval[a];
+            if (mrow[a] >= 0) P.map[mrow[a] + __float_as_int(w[NQ])] = __fmaf_rn(2.f, SKY_Q(a, 0), cval[a]);
           }
           // two directions per maximum: the value of an even slot waits for its odd neighbour (one FMNMX3)
           if (s & 1) best[a] = fmax3(best[a], pend[a], cval[a]);
@@ -414,21 +373,22 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
           const float2 x = win[(size_t)j * PS + ((j >> 3) & 1) +
                                ((ctrl >> (2 + kSkyRowBits * o)) & ((1 << kSkyRowBits) - 1))];
           vv[o] = x;
-          qq[1 + o] = re_prod(x, x);
+          const float xx = re_prod(x, x);
+          qq[1 + o] = __fsub_rn(xx, qq[0]);
           qq[1 + NO + o] = re_prod(pi.vT, x);
 #pragma unroll
           for (int o2 = 0; o2 < o; ++o2) qq[1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(vv[o2], x);
-          tot += qq[1 + o];
+          tot += xx;
         }
         const float c = quad_form<NQ>(w, qq);
         float cm = c;
 #pragma unroll
         for (int o = 16; o; o >>= 1) cm = fmaxf(cm, __shfl_xor_sync(0xffffffffu, cm, o));
         const int src = __ffs(__ballot_sync(0xffffffffu, c == cm)) - 1;
-        res.coh2 = cm;
+        res.coh2 = __fmaf_rn(2.f, qq[0], cm);
         res.tot2 = __shfl_sync(0xffffffffu, tot, src);
         res.pix = __shfl_sync(0xffffffffu, __float_as_int(w[NQ]), src);
-        res.null2 = fmaxf(res.tot2 - cm, 0.f);
+        res.null2 = fmaxf(res.tot2 - res.coh2, 0.f);
       }
       if (lane == 0) P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
       }
@@ -439,13 +399,13 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 // valid slots -> per-detector lists; invalid slots get their "no result" rows here
 __global__ void __launch_bounds__(256) k_sky_bin(const spiir_trigger* trig, int n_slots, int n_det, int S1,
                                                  const float2* z, int64_t det_stride, int64_t row_stride,
-                                                 int64_t ring_len, int64_t k_newest,
+                                                 int64_t ring_len, int64_t k_newest, int64_t n_rows,
                                                  SkyRec* lists, int32_t* counts, int max_slots,
                                                  spiir_sky_result* out) {
   const int i = blockIdx.x * 256 + threadIdx.x;
   if (i >= n_slots) return;
   const spiir_trigger t = trig[i];
-  if (t.valid && t.det >= 0 && t.det < n_det) {
+  if (t.valid && t.det >= 0 && t.det < n_det && t.tmpl >= 0 && t.tmpl < n_rows) {   // a stale or garbage slot never indexes the view
     const int64_t kmin = (k_newest - ring_len + 1 > 0) ? k_newest - ring_len + 1 : 0;
     SkyRec rc;
     rc.slot = i; rc.row = t.tmpl; rc.k = t.k; rc._pad = 0;
@@ -463,21 +423,6 @@ __global__ void __launch_bounds__(256) k_sky_bin(const spiir_trigger* trig, int 
 }  // namespace spiir
 
 using namespace spiir;
-
-struct spiir_sky_stream {                 // the direction stream of one trigger detector
-  int n_chunks = 0, n_tuples = 0, rows = 0, k_max = 0;
-  int lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];   // woff: offset of the detector's segment in a pair's block
-  int ps = 0;                             // float2 elements of a pair's block (even)
-  size_t off_slots = 0;
-};
-
-struct spiir_sky_plan {
-  int n_det = 0, n_pix = 0, max_slots = 0, n_tuples = 0, SW = 0, cap_slots = 0;
-  char* ws = nullptr;
-  size_t off_lists = 0, off_counts = 0, bytes = 0;
-  spiir_sky_stream st[SPIIR_MAX_DET];
-  int num_sms = 148;
-};
 
 static size_t sky_align(size_t x) { return (x + 255) / 256 * 256; }
 static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 2 + 3) / 4 * 4; }
@@ -547,7 +492,15 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
     const float* u = u2 + (size_t)p * D * 2;
     auto M = [&](int I, int J) { return (double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]; };
     // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order
-    w[0] = (float)M(T, T);
+    // U2 has orthonormal columns (Eq. 27: the left singular vectors), so the projector has trace 2 and
+    // M_TT = 2 - sum_o M_oo: the kernel evaluates rho_c^2 - 2 |z_T|^2 = sum_o M_oo (|z_o|^2 - |z_T|^2) + cross terms,
+    // one multiply-add fewer per direction, and adds the constant back at the end
+    w[0] = 0.f;
+    {
+      double tr = M(T, T);
+      for (int o = 0; o < NO; ++o) tr += M(oth[o], oth[o]);
+      if (!(tr > 2.0 - 1e-4 && tr < 2.0 + 1e-4)) S.bad_trace = 1;
+    }
     for (int o = 0; o < NO; ++o) w[1 + o] = (float)M(oth[o], oth[o]);
     for (int o = 0; o < NO; ++o) w[1 + NO + o] = (float)(2.0 * M(T, oth[o]));
     for (int o = 1; o < NO; ++o)
@@ -586,6 +539,9 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
   pl->ws = (char*)dev_workspace;
   cudaStream_t st = (cudaStream_t)stream;
   std::vector<float> slots;
+  // debugging knob: SPIIR_SKY_KERNEL=general makes three-detector plans run the general kernel (A/B comparisons)
+  const char* knob = getenv("SPIIR_SKY_KERNEL");
+  const bool force_general = knob && strcmp(knob, "general") == 0;
   for (int T = 0; T < D; ++T) {
     spiir_sky_stream& S = pl->st[T];
     int ps = 0;
@@ -602,19 +558,40 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
     }
     if (ps % 4 == 0) ps += 2;               // ps / 2 odd: a half-warp's 16 blocks start on distinct bank pairs
     S.rows = ps; S.ps = ps;
-    S.k_max = 0;
-    for (int K = kSkyKMax; K >= 1; --K)
-      if (sky_smem_bytes(ps, pl->SW, K) <= (size_t)kSkySmemMax) { S.k_max = K; break; }
-    if (S.k_max == 0) {
-      set_error("delay span of trigger detector %d needs %zu bytes of shared memory (> %d)", T,
-                sky_smem_bytes(ps, pl->SW, 1), kSkySmemMax);
+    S.k_max = 0; S.fmt3 = 0; S.k3 = 0;
+    if (D == 3 && !force_general) {
+      // three detectors: the stream walks the other detector with the narrower window fast (its windows are the
+      // ones kept in shared memory; on equal widths the higher index, as the general kernel does)
+      const int o0 = (T == 0) ? 1 : 0, o1 = (T == 2) ? 1 : 2;
+      const int If = (S.W[o0] < S.W[o1]) ? o0 : o1, Is = (If == o0) ? o1 : o0;
+      // four pairs per thread must fit: with two, the broadcast reads of the weights (per slot and warp, whatever the
+      // number of pairs) make the kernel shared-memory bound and the general kernel is faster (V1 as the trigger
+      // detector: 9.1 against 7.2 ms, profiles/r2_ncu_summary.md)
+      if (sky3_smem_bytes(S.W[If], 4) <= (size_t)kSkySmemMax) S.k3 = 4;
+      if (S.k3 && S.W[Is] < (1 << kSkyRowBits) && S.W[If] < (1 << kSkyRowBits) && pl->cap_slots / kSkyChunk < 32767) {
+        S.fmt3 = 1; S.I_s = Is; S.I_f = If;
+      }
+    }
+    if (!S.fmt3) {
+      for (int K = kSkyKMax; K >= 1; --K)
+        if (sky_smem_bytes(ps, pl->SW, K) <= (size_t)kSkySmemMax) { S.k_max = K; break; }
+      if (S.k_max == 0) {
+        set_error("delay span of trigger detector %d needs %zu bytes of shared memory (> %d)", T,
+                  sky_smem_bytes(ps, pl->SW, 1), kSkySmemMax);
+        delete pl; return SPIIR_EINVAL;
+      }
+      if (ps >= (1 << kSkyRowBits)) {
+        set_error("delay span of trigger detector %d: %d window samples do not fit the control word", T, ps);
+        delete pl; return SPIIR_EINVAL;
+      }
+    }
+    S.bad_trace = 0;
+    if (S.fmt3) sky3_build_stream(pl, T, u2, delay, slots);
+    else        sky_build_stream(pl, T, u2, delay, slots);
+    if (S.bad_trace) {
+      set_error("host_u2: the two columns of U2 must be orthonormal at every pixel (Eq. 27: left singular vectors)");
       delete pl; return SPIIR_EINVAL;
     }
-    if (ps >= (1 << kSkyRowBits)) {
-      set_error("delay span of trigger detector %d: %d window samples do not fit the control word", T, ps);
-      delete pl; return SPIIR_EINVAL;
-    }
-    sky_build_stream(pl, T, u2, delay, slots);
     cudaError_t e = cudaMemcpyAsync(pl->ws + S.off_slots, slots.data(), slots.size() * 4, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);     // the host images are reused for the next detector
     if (e != cudaSuccess) { set_error("sky plan upload failed: %s", cudaGetErrorString(e)); delete pl; return SPIIR_ECUDA; }
@@ -667,7 +644,7 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
                    int32_t n_slides, int64_t step, const int32_t* mult, spiir_sky_result* out, float* map,
                    cudaStream_t st) {
   SPIIR_REQUIRE(pl && view && trig && out, "a pointer is NULL");
-  SPIIR_REQUIRE(view->dev_z && view->ring_len >= 1, "bad SNR view");
+  SPIIR_REQUIRE(view->dev_z && view->ring_len >= 1 && view->n_rows >= 1, "bad SNR view");
   SPIIR_REQUIRE(n_slots >= 0 && n_slots <= pl->max_slots, "n_slots %d exceeds the plan's max_slots %d", n_slots,
                 pl->max_slots);
   SPIIR_REQUIRE(n_slides >= 0, "n_slides < 0");
@@ -679,7 +656,7 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
   SPIIR_CUDA_OK(cudaMemsetAsync(counts, 0, SPIIR_MAX_DET * 4, st));
   if (map) SPIIR_CUDA_OK(cudaMemsetAsync(map, 0, (size_t)n_slots * pl->n_pix * sizeof(float), st));
   k_sky_bin<<<(n_slots + 255) / 256, 256, 0, st>>>(trig, n_slots, D, S1, (const float2*)view->dev_z, view->det_stride,
-                                                   view->row_stride, view->ring_len, view->k_newest, lists, counts,
+                                                   view->row_stride, view->ring_len, view->k_newest, view->n_rows, lists, counts,
                                                    pl->max_slots, out);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());
@@ -687,6 +664,13 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
   const long long max_pairs = (long long)n_slots * S1;
   for (int T = 0; T < D; ++T) {
     const spiir_sky_stream& S = pl->st[T];
+    if (S.fmt3) {
+      SPIIR_REQUIRE(view->ring_len < (1ll << 31), "ring_len must be below 2^31 samples");
+      int rc3 = sky3_launch(pl, T, view, lists + (size_t)T * pl->max_slots, counts, max_pairs, n_slides, step, mult, out,
+                            map, st);
+      if (rc3) return rc3;
+      continue;
+    }
     SkyParams P;
     memset(&P, 0, sizeof(P));
     P.stream = (const float*)(pl->ws + S.off_slots); P.n_chunks = S.n_chunks;

@@ -20,7 +20,7 @@ constexpr int kUpThreads = 128;
 constexpr int kUpMaxFactor = 16;
 
 struct UpParams {
-  const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
+  const float2* z; int64_t det_stride, row_stride, ring_len, k_newest, n_rows;
   const spiir_trigger* trig; int32_t n_slots, n_det;
   int32_t R, H, Lw; int64_t Lp;
   float4 w[kUpMaxFactor];
@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(kUpThreads) k_upsample_trig(const __grid_const
   if (s >= P.n_slots) return;
   const spiir_trigger t = P.trig[s];
   const int64_t k_old = P.k_newest - P.ring_len + 1 > 0 ? P.k_newest - P.ring_len + 1 : 0;
-  const bool ok = t.valid && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
+  const bool ok = t.valid && t.tmpl >= 0 && t.tmpl < P.n_rows && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
   spiir_trigger o = t;
   o.valid = ok ? 1 : 0; o.tmpl = s; o.k = (int64_t)P.R * P.H;
   if (!t.valid) { o.det = 0; o.z_re = o.z_im = o.snr = 0.f; }
@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(kUpThreads) k_upsample(const __grid_constant__
   const int s = blockIdx.x, I = blockIdx.y;
   const spiir_trigger t = P.trig[s];
   const int64_t k_old = P.k_newest - P.ring_len + 1 > 0 ? P.k_newest - P.ring_len + 1 : 0;
-  const bool ok = t.valid && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
+  const bool ok = t.valid && t.tmpl >= 0 && t.tmpl < P.n_rows && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
   float2* out = P.out + ((size_t)I * P.n_slots + s) * P.Lp;
   if (!ok) {
     for (int u = threadIdx.x; u < P.Lp; u += kUpThreads) out[u] = make_float2(0.f, 0.f);
@@ -100,12 +100,12 @@ int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const 
   int rc = spiir_snr_upsample_elems(n_det, n_slots, factor, half_width, &elems);
   if (rc) return rc;
   SPIIR_REQUIRE(view && view->dev_z && dev_trig && dev_out && dev_trig_out && out_view, "a pointer is NULL");
-  SPIIR_REQUIRE(view->ring_len >= 1 && view->k_newest >= 0, "bad view");
+  SPIIR_REQUIRE(view->ring_len >= 1 && view->k_newest >= 0 && view->n_rows >= 1, "bad view");
   SPIIR_REQUIRE(((uintptr_t)dev_out & 15) == 0, "dev_out must be 16-byte aligned");
   UpParams P;
   P.z = (const float2*)view->dev_z;
   P.det_stride = view->det_stride; P.row_stride = view->row_stride;
-  P.ring_len = view->ring_len; P.k_newest = view->k_newest;
+  P.ring_len = view->ring_len; P.k_newest = view->k_newest; P.n_rows = view->n_rows;
   P.trig = dev_trig; P.n_slots = n_slots; P.n_det = n_det;
   P.R = factor; P.H = half_width; P.Lw = 2 * factor * half_width + 1;
   P.Lp = ((int64_t)P.Lw + 1) & ~(int64_t)1;
@@ -121,6 +121,7 @@ int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const 
   out_view->row_stride = P.Lp;
   out_view->ring_len = P.Lp;
   out_view->k_newest = P.Lw - 1;
+  out_view->n_rows = n_slots;
   if (n_slots == 0) return SPIIR_OK;
   k_upsample_trig<<<(n_slots + kUpThreads - 1) / kUpThreads, kUpThreads, 0, (cudaStream_t)stream>>>(P);
   k_upsample<<<dim3((unsigned)n_slots, (unsigned)n_det), kUpThreads, 0, (cudaStream_t)stream>>>(P);

@@ -17,7 +17,7 @@ namespace spiir {
 constexpr int kXiThreads = 128;
 
 struct Xi2Params {
-  const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
+  const float2* z; int64_t det_stride, row_stride, ring_len, k_newest, n_rows;
   const spiir_trigger* trig; const spiir_sky_result* sky; int32_t n_slots;
   const int32_t* delay; int32_t n_det, n_pix;
   const float2* acorr; int32_t nj;
@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(kXiThreads) k_xi2(const __grid_constant__ Xi2P
   const spiir_trigger tr = P.trig[i];
   const int pix = P.sky[w].pix;
   const int D = P.n_det, nj = P.nj, W = 2 * nj + 1;
-  bool ok = tr.valid && pix >= 0 && pix < P.n_pix && tr.det >= 0 && tr.det < D;
+  bool ok = tr.valid && pix >= 0 && pix < P.n_pix && tr.det >= 0 && tr.det < D && tr.tmpl >= 0 && tr.tmpl < P.n_rows;
   int64_t c[SPIIR_MAX_DET];
   if (ok) {
     const int64_t kmin = (P.k_newest - P.ring_len + 1 > 0) ? P.k_newest - P.ring_len + 1 : 0;
@@ -99,7 +99,7 @@ int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t 
                              int32_t n_slides, int64_t step_samples, const int32_t* host_slide_mult,
                              const spiir_c32* dev_autocorr, int32_t n_j, spiir_xi2_result* dev_out, void* stream) {
   SPIIR_REQUIRE(view && dev_delay && dev_trig && dev_sky && dev_autocorr && dev_out, "a pointer is NULL");
-  SPIIR_REQUIRE(view->dev_z && view->ring_len >= 1, "bad SNR view");
+  SPIIR_REQUIRE(view->dev_z && view->ring_len >= 1 && view->n_rows >= 1, "bad SNR view");
   SPIIR_REQUIRE(n_det >= 1 && n_det <= SPIIR_MAX_DET, "n_det %d out of range", n_det);
   SPIIR_REQUIRE(n_pix >= 1 && n_slots >= 0 && n_j >= 1, "bad n_pix / n_slots / n_j");
   SPIIR_REQUIRE(2 * (int64_t)n_j + 1 <= view->ring_len, "window of %d lags longer than the view", 2 * n_j + 1);
@@ -108,7 +108,7 @@ int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t 
   if (n_slots == 0) return SPIIR_OK;
   Xi2Params P;
   P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;
-  P.ring_len = view->ring_len; P.k_newest = view->k_newest;
+  P.ring_len = view->ring_len; P.k_newest = view->k_newest; P.n_rows = view->n_rows;
   P.trig = dev_trig; P.sky = dev_sky; P.n_slots = n_slots;
   P.delay = dev_delay; P.n_det = n_det; P.n_pix = n_pix;
   P.acorr = (const float2*)dev_autocorr; P.nj = n_j; P.out = dev_out;

@@ -40,7 +40,7 @@ def test_every_declared_symbol_is_exported(sp):
 
 
 def test_struct_sizes_match_the_header(sp):
-    assert C.sizeof(sp.spiir_snr_view) == 40
+    assert C.sizeof(sp.spiir_snr_view) == 48
     assert C.sizeof(sp.spiir_bank_desc) == 16 + 32 + 32 + 8 + 7 * 8 + 8 + 8
     assert sp.TRIGGER_DTYPE.itemsize == 40 and sp.RESULT_DTYPE.itemsize == 16 and sp.XI2_DTYPE.itemsize == 24
     assert sp.RANK_DTYPE.itemsize == 16 and C.sizeof(sp.spiir_rank_bins) == 24
