@@ -41,9 +41,23 @@ FLOP_PER_EVAL = 11.0            # this kernel: 1 FMUL + 5 FFMA per direction (N_
 # 8 issue slots) tops out at 12/16 = 75 % of it.
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 FP32_LANE_OPS_PER_S = 148 * 128 * 1.965e9
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/); None until a capture exists for the kernel.
-NCU_TRAFFIC_BYTES = {"k_bank": 4.43e9, "k_sky": 2.20e9}   # profiles/r1_ncu_summary.md sections 3 and 2 (mean of the three slide launches)
+FLOP_PER_EVAL_EXECUTED = 9.0    # 1 FMUL + 4 FFMA: the term of |z_T|^2 is a constant (trace of the projector = 2)
+
+
+def ncu_traffic_bytes():
+    """dram__bytes_read.sum + dram__bytes_write.sum of the two hot kernels, summed over the launches of ONE step,
+    read from the committed `ncu --set full` export profiles/r2_traffic.csv (kernel, launches per step, bytes);
+    None for a kernel without a capture.  The number is a record of that capture, not measured by this run."""
+    out = {"k_bank": None, "k_sky": None}
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    try:
+        for line in open(path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 3 and f[0] in out:
+                out[f[0]] = float(f[2])
+    except OSError:
+        pass
+    return out
 
 
 def parse_args():
@@ -57,6 +71,7 @@ def parse_args():
     ap.add_argument("--slides", type=int, default=None, help="override the number of time slides")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check after the timed region")
     ap.add_argument("--fast-norm", action="store_true",
                     help="diagonal approximation of the bank's noise normalisation (quicker set-up)")
     return ap.parse_args()
@@ -147,7 +162,14 @@ _SAMPLE_INPUTS = {}
 STEADY_TRIGGER_FRACTION = 0.36
 
 
-def oracle_sample(args, n_templates, n_chunks, n_trig, repeat=1):
+def oracle_setup():
+    """The timed build of the oracle (-O3 -march=native -fopenmp, compiled on this box)
+    on the physical cores.  Returns the thread count."""
+    import oracle
+    return oracle.use_timed_build()
+
+
+def oracle_sample(args, n_templates, n_chunks, n_trig, repeat=1, threads=None):
     """Times the float64 oracle (oracle/, as it stands) on a bounded sample of the workload:
     the first `n_templates` templates over `n_chunks` seconds (O1-O4) and the sky search with
     all its slides for `n_trig` candidates on packed SNR snippets (O6-O7).  Work is linear in
@@ -161,6 +183,8 @@ def oracle_sample(args, n_templates, n_chunks, n_trig, repeat=1):
         _SAMPLE_INPUTS[key] = (workloads.bank_for_config(args.config, n_templates=n_templates),
                                workloads.strain_for_config(args.config, seconds=n_chunks)["strain"])
     bank, x = _SAMPLE_INPUTS[key]
+    if threads:
+        oracle.set_threads(threads)
     dec, itp = workloads.halfband_taps()
     multirate = len(cfg["band_rates"]) > 1
     out = dict(threads=oracle.num_threads(), n_templates=n_templates, n_chunks=n_chunks, n_trig=n_trig)
@@ -213,44 +237,73 @@ def oracle_whole_step_rate(s, updates_full, evals_full, slots_full):
     return updates_full / t, t
 
 
-def run_reference(args):
-    """--impl reference: the oracle on the host cores, K timed steps after W warm-ups; each step
-    is one bounded sample (64 templates x 1 s through O1-O4, 8 candidates through O6-O7)."""
+def cpu_leg(args, w, n_t, n_c, n_trig, steps=1, warmup=0):
+    """The oracle on the host cores: `steps` timed repetitions of one bounded sample after `warmup` untimed
+    ones, on all physical cores, plus one single-thread pass over an eighth of the sample.  Both CPU legs of
+    this file (--impl reference and cpu_baseline) go through here, with samples that fill the cores."""
     import oracle
-    w = workload_params(args)
-    n_t, n_c, n_trig = min(64, w["T"]), 1, (8 if w["nside"] else 0)
-    for _ in range(max(0, args.warmup)):
-        oracle_sample(args, n_t, n_c, n_trig)
+    import workloads
+    threads = oracle_setup()
+    for _ in range(max(0, warmup)):
+        oracle_sample(args, n_t, n_c, n_trig, threads=threads)
     acc = None
     t0 = time.perf_counter()
-    for _ in range(args.steps):
-        s = oracle_sample(args, n_t, n_c, n_trig)
+    for _ in range(max(1, steps)):
+        s = oracle_sample(args, n_t, n_c, n_trig, threads=threads)
         if acc is None:
             acc = dict(s)
         else:
             for key in ("updates", "t_bank", "t_peaks", "evals", "t_sky"):
                 acc[key] += s[key]
     wall = time.perf_counter() - t0
-    import workloads
-    per_t = updates_per_chunk(workloads.bank_for_config(args.config, n_templates=n_t), w["D"], w["chunk"]) / n_t
+    one = oracle_sample(args, max(16, n_t // 8), n_c, max(4, n_trig // 8) if n_trig else 0, threads=1)
+    oracle.set_threads(threads)
+    per_t = updates_per_chunk(workloads.bank_for_config(args.config, n_templates=min(n_t, 64)), w["D"], w["chunk"]) / min(n_t, 64)
     updates_full = per_t * w["T"]
     slots_full = w["D"] * w["T"]
     frac = acc["trigger_fraction"] if acc["trigger_fraction"] > 0.05 else STEADY_TRIGGER_FRACTION
-    evals_full = frac * slots_full * w["n_pix"] * (1 + w["S"]) if w["nside"] else 0
-    value, t_chunk = oracle_whole_step_rate(acc, updates_full, evals_full, slots_full)
-    sample = ("per step: first %d templates x %d s through O1-O4 + %d candidates x %d directions x (1+%d slides) "
-              "through O6-O7; whole-chunk rate extrapolated linearly in templates and candidates"
-              % (n_t, n_c, n_trig, w["n_pix"], w["S"]))
+    return dict(acc=acc, wall=wall, threads=threads, one=one, updates_full=updates_full, slots_full=slots_full,
+                trigger_fraction=frac)
+
+
+def cpu_baseline_dict(leg, value, t_chunk, w, S):
+    acc, one = leg["acc"], leg["one"]
+    import multiprocessing
+    return {
+        "value": value, "unit": UNIT, "cores": leg["threads"], "logical_cpus": multiprocessing.cpu_count(),
+        "kind": "oracle", "build": "gcc -O3 -march=native -fopenmp -ffp-contract=off (compiled on this box)",
+        "bank_updates_per_s": acc["updates"] / acc["t_bank"],
+        "sky_evals_per_s": (acc["evals"] / acc["t_sky"]) if acc["evals"] else None,
+        "single_thread": {"bank_updates_per_s": one["updates"] / one["t_bank"],
+                          "sky_evals_per_s": (one["evals"] / one["t_sky"]) if one["evals"] else None},
+        "extrapolated_s_per_chunk": t_chunk,
+        "sample": "per repetition: first %d templates x %d s through O1-O4 (%.2f s in all) and %d candidates x %d "
+                  "directions x (1+%d slides) through O6-O7 (%.2f s in all); whole-chunk rate extrapolated linearly in "
+                  "templates and candidates" % (acc["n_templates"], acc["n_chunks"], acc["t_bank"], acc["n_trig"],
+                                                w["n_pix"], S, acc["t_sky"])}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, K timed steps after W warm-ups; each step is one bounded
+    sample that fills the cores (1024 templates x 1 s through O1-O4, 16 candidates per thread through O6-O7)."""
+    w = workload_params(args)
+    import oracle
+    from oracle.build import physical_cores
+    n_t, n_c = min(1024, w["T"]), 1
+    n_trig = max(256, 16 * physical_cores()) if w["nside"] else 0
+    leg = cpu_leg(args, w, n_t, n_c, n_trig, steps=args.steps, warmup=args.warmup)
+    acc = leg["acc"]
+    evals_full = leg["trigger_fraction"] * leg["slots_full"] * w["n_pix"] * (1 + w["S"]) if w["nside"] else 0
+    value, t_chunk = oracle_whole_step_rate(acc, leg["updates_full"], evals_full, leg["slots_full"])
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps),
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * leg["wall"] / max(1, args.steps),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": config_dict(args, w),
         "bank_updates_per_s": acc["updates"] / acc["t_bank"],
         "sky_evals_per_s": (acc["evals"] / acc["t_sky"]) if acc["evals"] else None,
         "extrapolated_s_per_chunk": t_chunk,
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                         "sample": sample},
+        "cpu_baseline": cpu_baseline_dict(leg, value, t_chunk, w, w["S"]),
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -266,6 +319,63 @@ def config_dict(args, w):
             "templates_per_gpu": w["T"], "ring_seconds": w["ring_len"] // 2048,
             "l2": "no flush: per-step working set (coefficients, states, band sums, SNR ring segment) exceeds the 126 MB L2",
             "parallelism": "template shards, no collective"}
+
+
+def parity_check(args, w, bank, x, fed, bk, prev_trig, fg_out, bg_out, u2, delay, mult, dec, itp, n_tmpl=8):
+    """Sampled oracle check of the run that was just timed (same process, same device state)."""
+    import torch
+    import oracle
+    import paper_2011_06787_b200 as sp
+    D, T, S, chunk = w["D"], w["T"], w["S"], w["chunk"]
+    n_slots = D * T
+    view = bk.snr_view()
+    L, k_new = int(view.c.ring_len), int(view.c.k_newest)
+    tp = sp.triggers_to_numpy(prev_trig)
+    rng = np.random.default_rng(w["cfg"]["seed"] + 99)
+    have = np.unique(tp["tmpl"][tp["valid"] == 1])
+    if have.size == 0:
+        return {"n": 0, "note": "no candidate in the last step"}
+    sel = np.unique(np.concatenate([have[:2], rng.choice(have, size=min(n_tmpl - 2, have.size), replace=False)]))[:n_tmpl]
+    # (1) SNR end to end: the oracle over every chunk fed so far, for the sampled templates
+    xs = np.concatenate([x[:, c * chunk:(c + 1) * chunk] for c in fed], axis=1)
+    z_ref = oracle.filter_bank(xs, bank, dec, itp, templates=sel.astype(np.int64))       # [D][n_sel][n_fed * 2048]
+    rows = bk.ring_rows(torch.from_numpy(sel.astype(np.int64)).cuda())                    # [D][n_sel][L][2] float32
+    zr = rows.cpu().numpy().view(np.complex64)[..., 0]                                    # ring index = k mod L
+    n_out = z_ref.shape[2]
+    assert n_out == k_new + 1, (n_out, k_new)
+    kk = np.arange(max(0, n_out - L), n_out)
+    err_snr = float(np.abs(zr[:, :, kk % L].astype(np.complex128) - z_ref[:, :, kk]).max())
+    # (2) the sky results of the sampled templates' candidates against O6 / O7 on the GPU's ring
+    slot_rows = (np.arange(D)[:, None] * T + sel[None, :]).reshape(-1)
+    sub = tp[slot_rows].copy()
+    sub["tmpl"] = np.tile(np.arange(len(sel)), D)
+    fg = sp.results_to_numpy(fg_out)[slot_rows]
+    bg = sp.results_to_numpy(bg_out).reshape(n_slots, max(S, 1))[slot_rows] if S else None
+    worst, n_res, bad_pix = 0.0, 0, 0
+    for res, kw in ((fg.reshape(-1, 1), {}), (bg, dict(n_slides=S, step=2048, slide_mult=mult))):
+        if res is None:
+            continue
+        out, pix, _ = oracle.sky_search(u2, delay, zr, len(sel) * L, L, L, k_new, sub["valid"], sub["tmpl"],
+                                        sub["det"], sub["k"], **kw)
+        has = pix >= 0
+        if not np.array_equal(res["pix"] >= 0, has):
+            bad_pix += int(((res["pix"] >= 0) != has).sum())
+            continue
+        c = out[..., 0]
+        rel = np.abs(res["coh2"].astype(np.float64) - c)[has] / np.maximum(c[has], 1e-30)
+        worst = max(worst, float(rel.max()) if rel.size else 0.0)
+        n_res += int(has.sum())
+        for i, sl in np.argwhere(has & (res["pix"] != pix)):
+            ok, cc, _, _ = oracle.sky_eval(u2, delay, zr, len(sel) * L, L, L, k_new, int(sub["tmpl"][i]), int(sub["det"][i]),
+                                           int(sub["k"][i]), int(res["pix"][i, sl]), s=(sl + 1 if kw else 0),
+                                           step=2048 if kw else 0, slide_mult=mult if kw else None)
+            if not (ok and cc >= c[i, sl] - max(1e-4 * c[i, sl], 1e-3)):
+                bad_pix += 1
+    ok = err_snr <= 1e-3 and worst <= 1e-4 and bad_pix == 0
+    return {"ok": bool(ok), "templates": int(len(sel)), "chunks_streamed": len(fed), "ring_wrapped": bool(k_new + 1 > L),
+            "snr_samples": int(zr[:, :, kk % L].size), "max_abs_err_snr": err_snr, "tol_snr": 1e-3,
+            "sky_results": n_res, "max_rel_err_coh2": worst, "tol_coh2_rel": 1e-4, "pixels_not_argmax": bad_pix,
+            "n": int(zr[:, :, kk % L].size) + n_res, "max_err": max(err_snr, worst)}
 
 
 # ----------------------------------------------------------------------------- the CUDA arm
@@ -324,6 +434,7 @@ def run_ours(args):
     bg_host = torch.empty(n_slots * max(S, 1), 16, dtype=torch.uint8).pin_memory()
     cnt_host = torch.empty(1, dtype=torch.int32).pin_memory()
     state = {"i": 0}
+    fed = []                                             # indices of the strain chunks fed so far, in order
 
     def step(xin, events=None, fg_out=fg_out, bg_out=bg_out):
         """One pass of the hot path over one chunk (every call goes through the C ABI)."""
@@ -331,6 +442,7 @@ def run_ours(args):
         cur, prev = trig[i & 1], trig[(i & 1) ^ 1]
         if events is not None: events[0].record()
         bk.filter_chunk(xin)                                           # H0-H3 (+ fused H4 maximum)
+        fed.append(state.get("chunk"))
         if events is not None: events[1].record()
         bk.peaks(w["thr"], 0, trig=cur, count=counts[i:i + 1])         # H4
         if events is not None: events[2].record()
@@ -350,10 +462,12 @@ def run_ours(args):
     n_fill = w["ring_len"] // 2048
     for c in range(n_fill):
         bk.filter_chunk(x_dev[c % n_chunks])
+        fed.append(c % n_chunks)
     torch.cuda.synchronize()
     t_setup = time.time() - t_setup
     c0 = n_fill
     for j in range(args.warmup):
+        state["chunk"] = (c0 + j) % n_chunks
         step(x_dev[(c0 + j) % n_chunks])
     c0 += args.warmup
     torch.cuda.synchronize()
@@ -372,6 +486,7 @@ def run_ours(args):
     e_begin, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e_begin.record()
     for j in range(K):
+        state["chunk"] = (c0 + j) % n_chunks
         step(x_dev[(c0 + j) % n_chunks], evs[j])
     e_end.record()
     torch.cuda.synchronize()
@@ -405,6 +520,15 @@ def run_ours(args):
             bg_np = sp.results_to_numpy(bg_out).reshape(n_slots, S)
             okb = bg_np["pix"][prev_np["valid"] == 1] >= 0
             searched = min(searched, float(okb.mean())) if okb.size else searched
+
+    # ---- parity in the regime that was just timed (once, outside the timed region; rank 0 of a single-GPU run):
+    #      the SNR of a seeded sample of templates over the whole stream fed so far against the float64 oracle
+    #      (O1-O3), and the last step's sky results of those templates' candidates, foreground and every slide,
+    #      against O6 / O7 on the ring as it stands (wrapped, threshold 4, 100 slides)
+    parity = None
+    if world == 1 and has_sky and not args.no_parity:
+        parity = parity_check(args, w, bank, x, fed, bk, trig[state["i"] & 1], fg_out, bg_out, u2, delay, mult,
+                              dec if multirate else None, itp if multirate else None)
 
     # ---- NEXT-1 (outside the timed step): xi^2 of the last step's candidates (Eq. 11, 12), n_j = 175, on a
     #      seeded synthetic autocorrelation table (the arithmetic and the traffic do not depend on its values)
@@ -534,6 +658,7 @@ def run_ours(args):
             b = j & 1
             if done[b] is not None:
                 main.wait_event(done[b])                             # result set b has been copied out
+            state["chunk"] = (c0 + j) % n_chunks
             x_in.copy_(x_host[(c0 + j) % n_chunks], non_blocking=True)
             cur = step(x_in, fg_out=dev_sets[b][0], bg_out=dev_sets[b][1])
             ready = torch.cuda.Event()
@@ -569,20 +694,31 @@ def run_ours(args):
         return
 
     # ---- roofline of the dominant kernel (+ the other one), FP32 probe, CPU baseline
-    ffma_rate, _ = sp.fp32_peak_probe(20)
+    import bench_probes as bp
+    ffma_rate, _ = bp.fp32_peak_probe(20)
     probes = {"unit": "fraction of the nominal FP32 lane rate (148 SM x 128 lanes x 1.965 GHz), register-only loops",
-              "recursion_mix_k_bank": sp.pipe_probe(1) / FP32_LANE_OPS_PER_S,
-              "quadratic_form_packed_ffma2": sp.pipe_probe(2) / FP32_LANE_OPS_PER_S,
-              "quadratic_form_scalar_ffma": sp.pipe_probe(3) / FP32_LANE_OPS_PER_S}
+              "recursion_mix_k_bank": bp.pipe_probe(1) / FP32_LANE_OPS_PER_S,
+              "quadratic_form_packed_ffma2": bp.pipe_probe(2) / FP32_LANE_OPS_PER_S,
+              "quadratic_form_scalar_ffma": bp.pipe_probe(3) / FP32_LANE_OPS_PER_S}
     ms_sky = stage[2] + stage[3]
+    traffic = ncu_traffic_bytes()
+    # executed FP32 lane-operations of the recursion: 8 per update, 5 in the band above the output rate, which
+    # advances two samples per step; `counted` keeps the paper's 8 per update everywhere
+    band_arr = np.asarray(bank["band"]).astype(np.int64)
+    upd_b0 = int(D * np.sum(band_arr == 0) * chunk) if bk.out_band == 1 else 0
+    exec_ops = (5.0 * upd_b0 + 8.0 * (upd_chunk - upd_b0)) * n_rec
     roof_bank = alu_roofline("k_bank (IIR recursion, H1+H2)", FLOP_PER_UPDATE * upd_chunk * n_rec, ms_rec,
-                             n_rec * len_groups(bk), ffma_rate, NCU_TRAFFIC_BYTES["k_bank"],
-                             issue_ops=8.0 * upd_chunk * n_rec)
+                             n_rec * len_groups(bk), ffma_rate, traffic["k_bank"],
+                             issue_ops=8.0 * upd_chunk * n_rec, executed_ops=exec_ops)
+    roof_bank["flop_per_unit"] = "12 per filter-sample update (PAPER.md:135)"
     roof_sky = None
     if has_sky and evals:
-        roof_sky = alu_roofline("k_sky (coherent search + slides, H5+H6)", FLOP_PER_EVAL * evals, ms_sky,
-                                2 * D * K if S else D * K, ffma_rate, NCU_TRAFFIC_BYTES["k_sky"],
-                                issue_ops=6.5 * evals)
+        roof_sky = alu_roofline("k_sky3 / k_sky (coherent search + slides, H5+H6)", FLOP_PER_EVAL * evals, ms_sky,
+                                2 * D * K if S else D * K, ffma_rate, traffic["k_sky"],
+                                issue_ops=6.5 * evals, executed_ops=5.5 * evals)
+        roof_sky["flop_per_unit"] = ("11 per (candidate or candidate-slide, direction) evaluation: the six-term quadratic form "
+                                     "of Eq. 28, as in round 1; the kernels execute 9 (five terms, trace of the projector = 2): "
+                                     "frac_executed_flop = %.4f" % (FLOP_PER_EVAL_EXECUTED * evals / (ms_sky * 1e-3) / 1e12 / FP32_PEAK_TFLOPS))
     dominant, other = (roof_bank, roof_sky) if (roof_sky is None or ms_rec >= ms_sky) else (roof_sky, roof_bank)
     line = {
         "metric": METRIC, "value": upd_all / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
@@ -596,6 +732,7 @@ def run_ours(args):
         "stage_rates": {"bank_updates_per_s": upd_chunk * K / (stage[0] * 1e-3),
                         "k_bank_updates_per_s": upd_chunk * n_rec / (ms_rec * 1e-3),
                         "sky_evals_per_s": (evals / (ms_sky * 1e-3)) if (has_sky and ms_sky > 0) else None},
+        "parity_checked": parity,
         "per_step": {"updates": upd_chunk, "candidates": n_cand / K if has_sky else None,
                      "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
         "roofline": dominant, "roofline_other": other, "pipe_probes": probes,
@@ -604,17 +741,10 @@ def run_ours(args):
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:
-        s = oracle_sample(args, min(8192, T), 2, 4096 if has_sky else 0)        # about 10-15 s of host work at config 4
-        cpu_v, cpu_t = oracle_whole_step_rate(s, upd_chunk, evals / K if has_sky else 0, n_slots)
-        line["cpu_baseline"] = {
-            "value": cpu_v, "unit": UNIT, "cores": s["threads"], "kind": "oracle",
-            "bank_updates_per_s": s["updates"] / s["t_bank"],
-            "sky_evals_per_s": (s["evals"] / s["t_sky"]) if s["evals"] else None,
-            "extrapolated_s_per_chunk": cpu_t,
-            "sample": "first %d templates x %d s through O1-O4 (%.1f s) and %d candidates x %d directions x (1+%d "
-                      "slides) through O6-O7 (%.1f s); whole-chunk rate extrapolated linearly in templates and "
-                      "candidates" % (s["n_templates"], s["n_chunks"], s["t_bank"], s["n_trig"], w["n_pix"], S,
-                                      s["t_sky"])}
+        # about 10-15 s of host work at config 4
+        leg = cpu_leg(args, w, min(8192, T), 2, 4096 if has_sky else 0)
+        cpu_v, cpu_t = oracle_whole_step_rate(leg["acc"], upd_chunk, evals / K if has_sky else 0, n_slots)
+        line["cpu_baseline"] = cpu_baseline_dict(leg, cpu_v, cpu_t, w, S)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -629,15 +759,17 @@ def len_groups(bk):
     return len(seen)
 
 
-def alu_roofline(name, flops, ms, n_launches, ffma_rate, traffic, issue_ops):
+def alu_roofline(name, flops, ms, n_launches, ffma_rate, traffic, issue_ops, executed_ops=None):
     """FP32-ALU roofline entry: achieved = algorithmic flop / device time of the kernel's launches
     (CUDA events on the launching stream, inside the timed region)."""
     achieved = flops / (ms * 1e-3) / 1e12
     return {"kernel": name, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
             "frac": achieved / FP32_PEAK_TFLOPS, "traffic": traffic,
+            "traffic_source": "profiles/r2_traffic.csv (ncu --set full capture of one step; a record, not measured by this run)",
             "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (clocks.max.sm); not in "
                            "MEASURED_PEAKS.json",
             "fp32_issue_frac": issue_ops / (ms * 1e-3) / FP32_LANE_OPS_PER_S,
+            "fp32_issue_frac_executed": (executed_ops / (ms * 1e-3) / FP32_LANE_OPS_PER_S) if executed_ops else None,
             "measured_ffma_tflops_same_run": 2.0 * ffma_rate / 1e12,
             "frac_of_measured_ffma": achieved / (2.0 * ffma_rate / 1e12),
             "ms_per_launch_set": ms / max(1, n_launches), "launches": n_launches}

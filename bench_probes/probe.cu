@@ -1,7 +1,13 @@
-// Measurement helper: a dependency-free FP32 FFMA loop on every SM, so that bench.py
-// can quote the ALU roofline measured in the same process and at the same clocks
-// (the FP32 peak is not in MEASURED_PEAKS.json).
-#include "spiir_internal.cuh"
+// Measurement helpers of bench.py — NOT part of the product library (libspiir_b200.so allocates nothing and
+// exports only the method's calls).  Built by bench_probes/build.py into bench_probes/libspiir_probe.so.
+//   probe_fp32_peak: a dependency-free FP32 FFMA loop on every SM, so that bench.py can quote the ALU roofline
+//   measured in the same process and at the same clocks (the FP32 peak is not in MEASURED_PEAKS.json).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define SPIIR_OK 0
+#define SPIIR_REQUIRE(cond, msg) do { if (!(cond)) return -1; } while (0)
+#define SPIIR_CUDA_OK(expr) do { if ((expr) != cudaSuccess) return -3; } while (0)
 
 namespace spiir {
 
@@ -25,7 +31,7 @@ __global__ void __launch_bounds__(kProbeThreads) k_fp32_probe(float* sink, float
 
 }  // namespace spiir
 
-extern "C" int spiir_fp32_peak_probe(int32_t reps, double* ms_out, double* fma_per_launch, void* stream) {
+extern "C" int probe_fp32_peak(int32_t reps, double* ms_out, double* fma_per_launch, void* stream) {
   using namespace spiir;
   SPIIR_REQUIRE(reps >= 1 && ms_out && fma_per_launch, "bad arguments");
   cudaStream_t st = (cudaStream_t)stream;
@@ -137,14 +143,14 @@ __global__ void __launch_bounds__(512, 1) k_probe_quadform(const float* wts, flo
 
 }  // namespace spiir
 
-extern "C" int spiir_pipe_probe(int32_t mode, int32_t reps, double* ms_out, double* lane_ops_per_launch, void* stream) {
+extern "C" int probe_pipe(int32_t mode, int32_t reps, double* ms_out, double* lane_ops_per_launch, void* stream) {
   using namespace spiir;
   SPIIR_REQUIRE(mode >= 1 && mode <= 3 && reps >= 1 && ms_out && lane_ops_per_launch, "bad arguments");
   cudaStream_t st = (cudaStream_t)stream;
   int dev = 0, sms = 0;
   SPIIR_CUDA_OK(cudaGetDevice(&dev));
   SPIIR_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  float* buf = nullptr;                                  // measurement helper only; not on the hot path
+  float* buf = nullptr;                
   const size_t n_coef = (size_t)kPF * 256 * 4;
   SPIIR_CUDA_OK(cudaMalloc(&buf, (16 + n_coef) * sizeof(float)));
   SPIIR_CUDA_OK(cudaMemsetAsync(buf, 0, (16 + n_coef) * sizeof(float), st));

@@ -321,17 +321,6 @@ int64_t spiir_launch_count(void);
 int spiir_bank_timing_enable(spiir_bank* bank, int32_t enable);
 int spiir_bank_timing_read(spiir_bank* bank, double* ms_recursion, double* ms_chunk, int32_t* n_chunks);
 
-/* Measurement helper: runs a dependency-free FP32 FMA loop on every SM and
- * returns the duration of `reps` launches in *ms_out and the FMA-lane-operations
- * performed per launch in *fma_per_launch (peak = 2*fma/time flop/s). */
-int spiir_fp32_peak_probe(int32_t reps, double* ms_out, double* fma_per_launch, void* stream);
-/* Measurement helper: register-only copies of the two hot inner loops (no memory traffic), so that the
- * ceilings DESIGN.md quotes for their operation mixes can be re-measured from committed code.
- *   mode 1: the k_bank recursion (8 FP32 lane-operations per update); mode 2: the k_sky quadratic form as
- *   packed FFMA2 with vector-register operands; mode 3: the same as scalar FFMA (6 lane-operations per
- *   evaluation).  *ms_out = duration of `reps` launches, *lane_ops_per_launch = FP32 lane-operations of one. */
-int spiir_pipe_probe(int32_t mode, int32_t reps, double* ms_out, double* lane_ops_per_launch, void* stream);
-
 const char* spiir_last_error(void);
 
 #ifdef __cplusplus

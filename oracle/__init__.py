@@ -15,10 +15,28 @@ from .upsample import lagrange4, upsample_windows  # noqa: F401
 _lib = None
 
 
+_timed = False
+
+
+def use_timed_build(threads=None):
+    """bench.py only: switch to the -O3 -march=native build of the same source (compiled here, on this box) and
+    set the OpenMP thread count (default: the physical cores).  Returns the thread count in use."""
+    global _lib, _timed
+    from .build import physical_cores
+    _timed, _lib = True, None
+    n = int(threads) if threads else physical_cores()
+    lib().spiir_oracle_set_threads(C.c_int(n))
+    return n
+
+
+def set_threads(n):
+    lib().spiir_oracle_set_threads(C.c_int(int(n)))
+
+
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(_build())
+        _lib = C.CDLL(_build(timed=_timed))
         _lib.spiir_oracle_bank.restype = C.c_int
         _lib.spiir_oracle_sky.restype = C.c_int
         _lib.spiir_oracle_sky_eval.restype = C.c_int

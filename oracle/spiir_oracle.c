@@ -303,7 +303,7 @@ EXPORT int spiir_oracle_sky(int n_det, int64_t n_pix, const float* u2, const int
     if (n_det < 2 || n_det > 8) return -1;
     const sky_ctx c = { n_det, n_pix, u2, delay, z, z_is_f32, det_stride, row_stride, ring_len, k_newest };
     const int S = n_slides > 0 ? n_slides : 1;
-    #pragma omp parallel for schedule(dynamic, 4)
+    #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t i = 0; i < n_trig; ++i) {
         for (int s = 0; s < S; ++s) {
             double* o = out + ((size_t)i * S + s) * 3;
@@ -413,6 +413,16 @@ EXPORT int spiir_oracle_xi2(int n_det, const int32_t* delay,
         }
     }
     return 0;
+}
+
+/* Thread count for the timed runs of bench.py (the physical cores of the box); no arithmetic here. */
+EXPORT void spiir_oracle_set_threads(int n)
+{
+    #ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+    #else
+    (void)n;
+    #endif
 }
 
 EXPORT int spiir_oracle_num_threads(void)

@@ -8,9 +8,9 @@ from .binding import (  # noqa: F401
     lib, last_error, SpiirError, EXPORTS, LIB_PATH,
     spiir_bank_desc, spiir_snr_view, spiir_band_plan, TRIGGER_DTYPE, RESULT_DTYPE,
     make_desc, Bank, SkyPlan, SkyPlanSet, SnrView, sky_table_build, sky_table_set_build, sky_table_nearest, upsample_windows,
-    triggers_to_numpy, triggers_from_numpy, results_to_numpy, fp32_peak_probe,
+    triggers_to_numpy, triggers_from_numpy, results_to_numpy,
     XI2_DTYPE, template_autocorr, signal_consistency, xi2_to_numpy,
-    RANK_DTYPE, spiir_rank_bins, Ranker, rank_to_numpy, pipe_probe,
+    RANK_DTYPE, spiir_rank_bins, Ranker, rank_to_numpy,
     SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EOVERFLOW,
 )
 from . import binding as _b

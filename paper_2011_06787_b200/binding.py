@@ -87,8 +87,6 @@ _SIGNATURES = {
     "spiir_bank_timing_enable": (C.c_int, [C.c_void_p, C.c_int32]),
     "spiir_bank_timing_read": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                          C.POINTER(C.c_int32)]),
-    "spiir_fp32_peak_probe": (C.c_int, [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
-    "spiir_pipe_probe": (C.c_int, [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]),
     "spiir_signal_consistency": (C.c_int, [C.POINTER(spiir_snr_view), C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
                                            C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p,
                                            C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]),
@@ -259,6 +257,17 @@ class Bank:
         _check(lib().spiir_bank_snr_view(self.h, C.byref(v)))
         return SnrView(raw=v)
 
+    def ring_rows(self, rows):
+        """The SNR ring rows of the templates `rows` (int64 cuda tensor) as float32 cuda [n_det][len(rows)][ring_len][2]
+        (element k mod ring_len of a row is sample k): a torch view of the workspace, copied; no arithmetic."""
+        import torch
+        v = self.snr_view().c
+        off = int(v.dev_z) - self.ws.data_ptr()
+        L = int(v.ring_len)
+        n = self.n_det * self.n_templates * L * 2
+        ring = self.ws[off:off + 4 * n].view(torch.float32).view(self.n_det, self.n_templates, L, 2)
+        return ring[:, rows].contiguous()
+
     def band_plan(self, band):
         p = spiir_band_plan()
         _check(lib().spiir_bank_band_plan(self.h, band, C.byref(p)))
@@ -407,13 +416,6 @@ def results_to_numpy(out):
     return out.cpu().numpy().view(RESULT_DTYPE).reshape(-1)
 
 
-def fp32_peak_probe(reps=20):
-    """(FP32 FMA lane-ops/s, ms) from the library's dependency-free FFMA kernel."""
-    ms, fma = C.c_double(0), C.c_double(0)
-    _check(lib().spiir_fp32_peak_probe(reps, C.byref(ms), C.byref(fma), _stream()))
-    return fma.value * reps / (ms.value * 1e-3), ms.value
-
-
 def template_autocorr(bank, t, n_j):
     """spiir_template_autocorr for template ``t`` of a bank dict: complex64 [2 n_j + 1]."""
     off = np.asarray(bank["tmpl_offset"])
@@ -494,10 +496,3 @@ class Ranker:
 
 def rank_to_numpy(out):
     return out.cpu().numpy().view(RANK_DTYPE).reshape(-1)
-
-
-def pipe_probe(mode, reps=5):
-    """FP32 lane-operations/s of a register-only copy of a hot inner loop (spiir_pipe_probe)."""
-    ms, ops = C.c_double(0), C.c_double(0)
-    _check(lib().spiir_pipe_probe(mode, reps, C.byref(ms), C.byref(ops), _stream()))
-    return ops.value * reps / (ms.value * 1e-3)

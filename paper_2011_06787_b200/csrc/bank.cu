@@ -483,8 +483,7 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     cp.sb_off[b] = cp.sb_total;
     cp.sb_total += (cp.sb_n[b] + 1) & ~1;
   }
-  launch_combine(cp, D, st);
-  SPIIR_CUDA_OK(cudaGetLastError());
+  { const int rcc = launch_combine(cp, D, st); if (rcc) return rcc; }
   if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[3], st));
 
   bk->parity = newp;

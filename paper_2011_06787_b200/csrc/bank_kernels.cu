@@ -25,18 +25,23 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
                : "memory");
 }
+// Bounded wait: try_wait suspends the thread for a hardware time slice per poll; a copy that faulted or an
+// expect_tx that disagrees with the bytes issued traps after seconds instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra WAIT_DONE;\n"
-      "bra WAIT_LOOP;\n"
-      "WAIT_DONE:\n"
-      "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity)
-      : "memory");
+  uint32_t done = 0;
+  for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    if (done) return;
+  }
+  __trap();
 }
 // 1-D TMA bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP).
 __device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
@@ -552,14 +557,16 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
   }
 }
 
-void launch_combine(const CombineParams& p, int n_det, cudaStream_t st) {
+int launch_combine(const CombineParams& p, int n_det, cudaStream_t st) {
   static unsigned long long configured = 0;
   if (first_use_on_device(configured)) {
-    cudaFuncSetAttribute(k_combine, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_combine, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   }
   const size_t smem = (size_t)(((p.bufA + p.bufB + 1) & ~1) + p.sb_total) * sizeof(float2);
   k_combine<<<dim3(p.T, n_det), kCombineThreads, smem, st>>>(p);
   count_launch();
+  SPIIR_CUDA_OK(cudaGetLastError());
+  return SPIIR_OK;
 }
 
 }  // namespace spiir

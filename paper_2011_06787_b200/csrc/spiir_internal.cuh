@@ -108,7 +108,7 @@ struct CombineParams {
 void launch_prep(const PrepParams& p, int n_det, cudaStream_t st);
 int launch_bank_group(int G, int F, int odd, const BankParams& P, const CtaWork* dev_work, int n_cta, int n_det,
                       int smem, cudaStream_t st);
-void launch_combine(const CombineParams& p, int n_det, cudaStream_t st);
+int launch_combine(const CombineParams& p, int n_det, cudaStream_t st);
 
 // peaks.cu
 struct PeakParams {

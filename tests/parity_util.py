@@ -94,27 +94,30 @@ def check_sky(res_gpu, view_z, ring_len, k_newest, u2, delay, trig, n_slides=0, 
     out, pix, _ = ref
     g = res_gpu.reshape(n_trig, S)
     D, rows, L = view_z.shape
-    n_pixdiff = 0
-    for i in range(n_trig):
-        for s in range(S):
-            gp = int(g["pix"][i, s])
-            if pix[i, s] < 0:
-                assert gp == -1 and g["coh2"][i, s] == 0 and g["tot2"][i, s] == 0 and g["null2"][i, s] == 0
-                continue
-            assert gp >= 0, "GPU reports no result where the oracle has one (trigger %d slide %d)" % (i, s)
-            cmax = out[i, s, 0]
-            tol = max(TOL_COH2_REL * cmax, 1e-6)
-            assert abs(g["coh2"][i, s] - cmax) <= tol, (i, s, g["coh2"][i, s], cmax)
-            assert abs(np.sqrt(g["coh2"][i, s]) - np.sqrt(cmax)) <= 1e-3
-            if gp != pix[i, s]:
-                n_pixdiff += 1
-                ok, c, nul, tot = oracle.sky_eval(u2, delay, view_z, rows * L, L, ring_len, k_newest,
-                                                  int(trig["tmpl"][i]), int(trig["det"][i]), int(trig["k"][i]), gp,
-                                                  s=(s + 1 if n_slides else 0), step=step, slide_mult=mult)
-                assert ok
-                assert c >= cmax - max(1e-4 * cmax, 1e-3), "GPU pixel is not a valid arg-max (A19)"
-            else:
-                c, tot = cmax, out[i, s, 2]
-            assert abs(g["tot2"][i, s] - tot) <= 1e-5 * tot + 1e-6
-            assert abs(g["null2"][i, s] - max(tot - c, 0.0)) <= 1e-4 * tot + 1e-5
-    return dict(pix_differs=n_pixdiff)
+    gp = g["pix"].astype(np.int64)
+    gc, gt, gn = g["coh2"].astype(np.float64), g["tot2"].astype(np.float64), g["null2"].astype(np.float64)
+    none = pix < 0
+    assert np.all(gp[none] == -1) and np.all(gc[none] == 0) and np.all(gt[none] == 0) and np.all(gn[none] == 0)
+    has = ~none
+    bad = has & (gp < 0)
+    assert not bad.any(), "GPU reports no result where the oracle has one (trigger, slide) %s" % (np.argwhere(bad)[:4].tolist(),)
+    cmax = out[..., 0]
+    tol = np.maximum(TOL_COH2_REL * cmax, 1e-6)
+    err = np.abs(gc - cmax)
+    assert np.all(err[has] <= tol[has]), "coh2 differs: worst %s" % (np.argwhere(has & (err > tol))[:4].tolist(),)
+    assert np.all(np.abs(np.sqrt(gc[has]) - np.sqrt(cmax[has])) <= 1e-3)
+    # at the oracle's own pixel the three values compare directly; elsewhere the GPU's pixel must be a valid
+    # arg-max (A19) and the values are compared with the oracle evaluated AT THAT PIXEL
+    c_at, tot_at = cmax.copy(), out[..., 2].copy()
+    differs = np.argwhere(has & (gp != pix))
+    for i, s in differs:
+        ok, c, nul, tot = oracle.sky_eval(u2, delay, view_z, rows * L, L, ring_len, k_newest,
+                                          int(trig["tmpl"][i]), int(trig["det"][i]), int(trig["k"][i]), int(gp[i, s]),
+                                          s=(s + 1 if n_slides else 0), step=step, slide_mult=mult)
+        assert ok
+        assert c >= cmax[i, s] - max(1e-4 * cmax[i, s], 1e-3), "GPU pixel is not a valid arg-max (A19)"
+        c_at[i, s], tot_at[i, s] = c, tot
+    assert np.all(np.abs(gt - tot_at)[has] <= (1e-5 * tot_at + 1e-6)[has])
+    assert np.all(np.abs(gn - np.maximum(tot_at - c_at, 0.0))[has] <= (1e-4 * tot_at + 1e-5)[has])
+    rel = np.where(has, err / np.maximum(cmax, 1e-30), 0.0)
+    return dict(pix_differs=int(len(differs)), n=int(has.sum()), max_rel_err_coh2=float(rel.max()) if has.any() else 0.0)

@@ -438,12 +438,13 @@ def test_sky_degenerate_inputs(sp, U):
     U.check_sky(res, zc, L, L - 1, u2, delay, trig)
 
 
-# ------------------------------------------------------------------ config 3 at FULL size, sampled outputs
-def test_cfg3_full_size_sampled(sp, U):
-    """BASELINE.json config 3: 4096 triggers, HEALPix nside 64 (49 152 directions), 100 time slides,
-    packed +-50 ms snippets.  The whole search runs on the GPU; the oracle checks a
-    seeded sample of 12 triggers (signals and noise) on the foreground and on all 100 slides, and the
-    strong injected signals must come back at (or tied with) their pixel."""
+# ------------------------------------------------------------------ config 3 in FULL
+def test_cfg3_full(sp, U):
+    """BASELINE.json config 3 in full ("configs 0-3: the oracle runs in full"): 4096 triggers,
+    HEALPix nside 64 (49 152 directions), 100 time slides on packed +-50 ms snippets
+    (DESIGN.md §8).  The oracle evaluates every (trigger, slide, direction) — 2.03e10 evaluations of O6 / O7
+    in float64 — and every one of the 4096 x 101 GPU results is compared with it (coh2 1e-4 relative, pixel by
+    the set-valued rule A19, tot2 / null2 at the GPU's pixel)."""
     import torch
     cfg = workloads.config(3)
     n_rows, S, half = cfg["n_triggers"], cfg["n_slides"], cfg["snippet_half"]
@@ -463,24 +464,24 @@ def test_cfg3_full_size_sampled(sp, U):
     fg = sp.results_to_numpy(plan.search(view, td, n_rows))
     bg = sp.results_to_numpy(plan.background(view, td, n_rows, S, W, [1, 1, 1])).reshape(n_rows, S)
     torch.cuda.synchronize()
+    del zd
     assert np.all(fg["pix"] >= 0) and np.all(bg["pix"] >= 0)
     # invariants that hold at any size: coh2 <= tot2, null2 = max(tot2 - coh2, 0)
     for r in (fg, bg.reshape(-1)):
         assert np.all(r["coh2"] <= r["tot2"] * (1 + 1e-5) + 1e-6)
         assert np.all(np.abs(r["null2"] - np.maximum(r["tot2"] - r["coh2"], 0)) <= 1e-6 * r["tot2"] + 1e-6)
-    # sampled triggers against the oracle, foreground and every slide
+    # every trigger against the oracle: foreground and all 100 slides
+    zc = np.ascontiguousarray(z).view(np.complex64)[..., 0]
+    st_f = U.check_sky(fg, zc, L, L - 1, u2, delay, trig)
+    st_b = U.check_sky(bg.reshape(-1), zc, L, L - 1, u2, delay, trig, n_slides=S, step=W, mult=[1, 1, 1])
+    assert st_f["n"] == n_rows and st_b["n"] == n_rows * S
+    print("cfg3 full: foreground %s, slides %s" % (st_f, st_b))
+    # injected signals in the plane of their pixel: the foreground is far above the time-slid background of the
+    # same trigger (the slid background keeps |z_T|^2)
     sig = np.nonzero(truth["is_signal"])[0]
-    noi = np.nonzero(~truth["is_signal"])[0]
-    pick = np.concatenate([sig[:6], noi[:6]])
-    zc = np.ascontiguousarray(z[:, pick]).view(np.complex64)[..., 0]
-    sub = trig[pick].copy(); sub["tmpl"] = np.arange(len(pick))
-    U.check_sky(fg[pick], zc, L, L - 1, u2, delay, sub)
-    U.check_sky(bg[pick].reshape(-1), zc, L, L - 1, u2, delay, sub, n_slides=S, step=W, mult=[1, 1, 1])
-    # injected signals in the plane of their pixel: null2 at the maximum is small against coh2, and the
-    # foreground is far above the time-slid background of the same trigger
     strong = sig[truth["rho"][sig] > 12]
     assert len(strong) > 50
-    assert np.median(fg["coh2"][strong] / np.median(bg["coh2"][strong], axis=1)) > 2   # (the slid background keeps |z_T|^2)
+    assert np.median(fg["coh2"][strong] / np.median(bg["coh2"][strong], axis=1)) > 2
 
 
 # ------------------------------------------------------------------ NEXT-1: signal-consistency statistic (Eq. 11, 12)
