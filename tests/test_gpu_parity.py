@@ -397,11 +397,153 @@ def test_cfg4_full_size_sampled(sp, U):
         assert np.all(np.abs(np.sqrt(cg) - np.sqrt(ce)) <= 1e-3) and np.all(np.abs(cg - ce) <= 1e-4 * ce + 1e-5)
 
 
+def test_cfg4_steady_state(sp, U):
+    """BASELINE.json config 4 in the regime bench.py times: all 128 one-second chunks streamed through the full
+    bank (20 000 templates x 700 filters, 8 bands, 3 detectors), threshold 4, SNR ring of 103 s
+    so that it WRAPS, 100 one-second time slides on the foreground grid (nside 32).
+    Sampled outputs (the oracle cannot run 14 M filters): 16 seeded templates (3 chirp-matched long-delay ones)
+      * their SNR over the whole 128 s against the float64 oracle of exactly those templates (O1-O3);
+      * their peaks in EVERY chunk, stage-isolated and end to end (A12); all 60 000 peaks of eight chunks around
+        the start, the ring wrap and the end, stage-isolated;
+      * for the last two searched chunks (ring wrapped, low-rate bands full): their candidates through O6 on the
+        foreground and O7 on all 100 slides, and xi^2 (O8) on foreground and slides."""
+    import torch
+    cfg = workloads.config(4)
+    T, D, NC, S, THR, nj = cfg["n_templates"], 3, 128, 100, 4.0, 175
+    bank = workloads.bank_for_config(4)
+    st = workloads.strain_for_config(4)
+    x = st["strain"]
+    assert x.shape[1] == NC * 4096
+    dec, itp = workloads.halfband_taps()
+    rng = np.random.default_rng(44)
+    sel = np.unique(np.concatenate([[0, 7, 19, 20, T - 1], rng.integers(21, T - 1, 11)])).astype(np.int64)
+    ns = len(sel)
+    z_ref = oracle.filter_bank(x, bank, dec, itp, templates=sel)             # [D][ns][NC*2048]
+    L = (S + 3) * 2048
+    bk = sp.Bank(bank, D, 4096, ring_len=L, bank_size=1000, dec_taps=dec, int_taps=itp)
+    u2, delay = _table(cfg, gmst=st["gmst"])
+    plan = sp.SkyPlan(u2, delay, max_slots=D * T)
+    dl_dev = torch.from_numpy(np.ascontiguousarray(delay, dtype=np.int32)).cuda()
+    # a seeded synthetic autocorrelation table (an INPUT of Eq. 11 like the sky table; multirate templates have no
+    # host helper): A[j] = exp(-|j| / tau + i w j)
+    g = np.random.default_rng(45)
+    tau, om = 5.0 + 40.0 * g.random(T), 0.1 + 1.2 * g.random(T)
+    lag = np.arange(-nj, nj + 1)
+    acorr = (np.exp(-np.abs(lag)[None, :] / tau[:, None]) * np.exp(1j * om[:, None] * lag[None, :])).astype(np.complex64)
+    ac_dev = torch.from_numpy(acorr.view(np.float32).reshape(T, 2 * nj + 1, 2)).cuda()
+    xs = torch.from_numpy(x).cuda()
+    out = torch.empty(D, T, 2048, 2, dtype=torch.float32, device="cuda")
+    z_sel = np.zeros((D, ns, NC * 2048), np.complex64)
+    sel_dev = torch.from_numpy(sel).cuda()
+    rows = (np.arange(D)[:, None] * T + sel[None, :]).reshape(-1)
+    full_check = {0, 1, 50, 102, 103, 104, NC - 2, NC - 1}
+    prev, n_rule2, n_cand, searched = None, 0, [], 0
+    mult = [1, 1, 1]
+    for c in range(NC):
+        bk.filter_chunk(xs[:, c * 4096:(c + 1) * 4096].contiguous(), out)
+        z_sel[:, :, c * 2048:(c + 1) * 2048] = out[:, sel_dev].cpu().numpy().view(np.complex64)[..., 0]
+        tr, cnt = bk.peaks(THR, 0)
+        torch.cuda.synchronize()
+        trig = sp.triggers_to_numpy(tr).copy()
+        n_cand.append(int(cnt.cpu()[0]))
+        # the sampled templates' peaks of this chunk: stage-isolated + end to end
+        n_rule2 += U.check_peaks_mode0(_subset_trig(trig[rows], sel, D), z_sel[:, :, c * 2048:(c + 1) * 2048],
+                                       z_ref[:, :, c * 2048:(c + 1) * 2048], c * 2048, THR)
+        if c in full_check:                                                   # all 60 000 peaks, stage-isolated
+            z_all = out.cpu().numpy().view(np.complex64)[..., 0]
+            k_iso, v_iso = oracle.peaks_mode0(z_all.reshape(D * T, 2048), THR)
+            assert np.array_equal(trig["k"] - c * 2048, k_iso) and np.array_equal(trig["valid"], v_iso)
+            assert n_cand[-1] == int(v_iso.sum())
+            del z_all
+        if c >= NC - 2 and prev is not None:
+            # search the previous chunk's candidates (one-chunk lag, A13): the ring has wrapped (k_newest >= L)
+            view = bk.snr_view()
+            k_new = (c + 1) * 2048 - 1
+            assert int(view.c.k_newest) == k_new and k_new + 1 > L
+            fg_d = plan.search(view, prev[0], D * T)
+            bg_d = plan.background(view, prev[0], D * T, S, 2048, mult)
+            xi_f = sp.xi2_to_numpy(sp.signal_consistency(view, dl_dev, prev[0], fg_d, D * T, ac_dev, nj))
+            xi_b = sp.xi2_to_numpy(sp.signal_consistency(view, dl_dev, prev[0], bg_d, D * T, ac_dev, nj, n_slides=S,
+                                                         step=2048, mult=mult)).reshape(D * T, S)
+            torch.cuda.synchronize()
+            fg, bg = sp.results_to_numpy(fg_d), sp.results_to_numpy(bg_d).reshape(D * T, S)
+            tp = prev[1]
+            # every candidate of the chunk was searched on the foreground and on every one of the 100 slides
+            assert np.all((fg["pix"] >= 0) == (tp["valid"] == 1)) and np.all((bg["pix"] >= 0) == (tp["valid"] == 1)[:, None])
+            # the ring of the sampled templates as the device holds it: element k mod L is sample k
+            kk = np.arange(k_new + 1 - L, k_new + 1)
+            zr = np.zeros((D, ns, L), np.complex64)
+            zr[:, :, kk % L] = z_sel[:, :, kk]
+            dev_rows = bk.ring_rows(sel_dev).cpu().numpy().view(np.complex64)[..., 0]
+            assert np.array_equal(dev_rows, zr)                               # the wrapped ring holds exactly the last L samples
+            sub = _subset_trig(tp[rows], sel, D)
+            assert sub["valid"].sum() >= 6
+            st_f = U.check_sky(fg[rows], zr, L, k_new, u2, delay, sub)
+            st_b = U.check_sky(bg[rows].reshape(-1), zr, L, k_new, u2, delay, sub, n_slides=S, step=2048, mult=mult)
+            searched += st_f["n"] + st_b["n"]
+            assert st_b["n"] == S * st_f["n"]
+            # xi^2 (Eq. 11, 12) at the GPU's pixels, foreground and every slide
+            A_sel = acorr[sel].astype(np.complex128)
+            for xg, pixg, kw in ((xi_f[rows], fg["pix"][rows], {}),
+                                 (xi_b[rows], bg["pix"][rows], dict(n_slides=S, step=2048, slide_mult=mult))):
+                ref = oracle.xi2(delay, zr, ns * L, L, L, k_new, sub["valid"], sub["tmpl"], sub["det"], sub["k"],
+                                 pixg, A_sel, nj, **kw)
+                used = ref[..., D + 1] == 1
+                assert np.array_equal(xg["used"].reshape(used.shape), used.astype(np.int32)) and used.sum() >= 6
+                gc = xg["xi2_c"].reshape(used.shape)
+                assert np.all(np.abs(gc - ref[..., D])[used] <= 1e-4 * ref[..., D][used] + 1e-5)
+        prev = (tr.clone(), trig)
+    err = U.check_snr(z_sel, z_ref)
+    # steady state: about two thirds of the (detector, template, second) slots are above SNR 4 (what bench.py searches:
+    # ~40 500 candidates per chunk), against a handful in the first seconds while the low-rate bands fill
+    assert 0.5 * D * T < np.median(n_cand[-20:]) < 0.85 * D * T and n_cand[0] < 0.2 * D * T
+    assert searched >= 2 * 6 * (1 + S)
+    print("cfg4 steady state: max |dz| %.2e over 128 s, %d near-tie peaks (A12), %d sky results checked" % (err, n_rule2, searched))
+
+
 def _subset_trig(trig_rows, sel, D):
     """Trigger slots of the selected templates with `tmpl` renumbered to rows of the sampled view."""
     t = trig_rows.copy()
     t["tmpl"] = np.tile(np.arange(len(sel)), D)
     return t
+
+
+# ------------------------------------------------------------------ views that are not 16-byte friendly
+@pytest.mark.parametrize("kernel", ["three-detector", "general"])
+def test_sky_unaligned_view(sp, U, kernel, monkeypatch):
+    """A view whose rows are not 16-byte friendly (odd ring_len 501, base pointer 8 bytes past an aligned address):
+    the window staging cannot use TMA bulk copies and takes the 8-byte cp.async path of each kernel.  Foreground,
+    slides and a wrapped ring against O6 / O7, for the three-detector kernel and (SPIIR_SKY_KERNEL=general) the
+    general one."""
+    import torch
+    if kernel == "general":
+        monkeypatch.setenv("SPIIR_SKY_KERNEL", "general")
+    else:
+        monkeypatch.delenv("SPIIR_SKY_KERNEL", raising=False)
+    cfg = workloads.config(1)
+    u2, delay = _table(cfg, nside=8, gmst=1.1)
+    D, rows, L, k_new, S, step = 3, 40, 501, 1300, 3, 90
+    rng = np.random.default_rng(501)
+    z = (rng.standard_normal((D, rows, L)) + 1j * rng.standard_normal((D, rows, L))).astype(np.complex64)
+    flat = torch.zeros(D * rows * L * 2 + 2, dtype=torch.float32, device="cuda")
+    flat[2:] = torch.from_numpy(np.ascontiguousarray(z).view(np.float32).reshape(-1)).cuda()
+    assert flat.data_ptr() % 16 == 0
+    raw = sp.spiir_snr_view(flat.data_ptr() + 8, rows * L, L, L, k_new, rows)
+    view = sp.SnrView(raw=raw)
+    view._keep = flat
+    n = 64
+    trig = np.zeros(n, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1; trig["valid"][5] = 0
+    trig["tmpl"] = rng.integers(0, rows, n); trig["det"] = rng.integers(0, D, n)
+    trig["k"] = rng.integers(k_new - L + 1, k_new + 1, n)            # some windows leave the view on either side
+    td = sp.triggers_from_numpy(trig)
+    plan = sp.SkyPlan(u2, delay, max_slots=n)
+    fg = sp.results_to_numpy(plan.search(view, td, n))
+    bg = sp.results_to_numpy(plan.background(view, td, n, S, step, [1, 1, 1]))
+    torch.cuda.synchronize()
+    st_f = U.check_sky(fg, z, L, k_new, u2, delay, trig)
+    st_b = U.check_sky(bg, z, L, k_new, u2, delay, trig, n_slides=S, step=step, mult=[1, 1, 1])
+    assert st_f["n"] >= 30 and st_b["n"] >= 60 and (fg["pix"] == -1).sum() >= 2
 
 
 # ------------------------------------------------------------------ degenerate inputs
