@@ -11,6 +11,7 @@ import numpy as np
 from .build import build as _build
 from .sky import healpix_ring_centres, sky_table, g_sigma, table_set, nearest_table  # noqa: F401
 from .upsample import lagrange4, upsample_windows  # noqa: F401
+from . import frontend  # noqa: F401
 
 _lib = None
 

@@ -956,3 +956,135 @@ def test_p27_sub_sample_alignment_removes_the_integer_delay_loss():
     assert np.mean(null_fine) < 0.1 * np.mean(null_int)
     assert np.mean(loss_fine) < 0.25 * np.mean(loss_int) and np.max(loss_fine) < 5e-3
     assert np.mean(loss_int) > 2e-3                                 # the loss being removed is real
+
+
+# ---- NEXT-4: front end — pins P30-P35 of oracle/frontend.py ---------------------------------
+def test_p30_downsampler_is_scipy_lfilter_decimated():
+    """W1 reduces to a library routine: y = lfilter(h, 1, x)[R-1::R]."""
+    from oracle import frontend as fe
+    rng = np.random.default_rng(30)
+    for R, nt in ((8, 192), (4, 64), (1, 5)):
+        h = rng.standard_normal(nt)
+        x = rng.standard_normal(R * 300)
+        y = fe.downsample(x, h, R)
+        np.testing.assert_allclose(y, scipy.signal.lfilter(h, 1.0, x)[R - 1::R], rtol=0, atol=1e-12)
+    # a unit impulse at n = 5 comes out as the taps sampled every R-th with that offset
+    h = np.arange(1.0, 25.0)
+    x = np.zeros(80); x[5] = 1.0
+    y = fe.downsample(x, h, 8)
+    want = np.array([h[8 * m + 7 - 5] if 0 <= 8 * m + 7 - 5 < 24 else 0.0 for m in range(10)])
+    assert np.array_equal(y, want)
+
+
+def test_p31_whitener_is_the_identity_for_a_flat_psd_and_scales_a_line():
+    """W2-W3: with S_n f_s / 2 = 1 the Hann blocks overlap-add back to the input exactly (window sum = 1, forward and
+    inverse transform normalised); a sinusoid on a bin of known S_n comes out divided by sqrt(S_n f_s / 2)."""
+    from oracle import frontend as fe
+    rng = np.random.default_rng(31)
+    H, fs = 128, 2048.0
+    d = rng.standard_normal(H * 9)
+    dw, S, P = fe.whiten_stream(d, H, fs, 27, psd_true=np.full(H + 1, 2.0 / fs))
+    np.testing.assert_allclose(dw[:-H], d[:-H], rtol=0, atol=1e-13)          # (the last hop is only half added)
+    w = fe.hann_periodic(2 * H)
+    np.testing.assert_allclose(w[:H] + w[H:], 1.0, rtol=0, atol=1e-15)
+    k0 = 20
+    psd = np.full(H + 1, 2.0 / fs); psd[k0] = 9.0 * 2.0 / fs                 # S_n f_s / 2 = 9 on that bin: amplitude / 3
+    t = np.arange(H * 9)
+    line = np.cos(2 * np.pi * k0 * t / (2 * H))
+    dw, _, _ = fe.whiten_stream(line, H, fs, 27, psd_true=psd)
+    # the Hann window spreads a block's line over bins k0 - 1 .. k0 + 1 (amplitudes -1/4, 1/2, -1/4); only the central one
+    # is divided by 3, and the side terms of two half-overlapped blocks cancel (their windows' cosines are in anti-phase):
+    # what is left is the line itself, divided by 3
+    want = line / 3.0
+    np.testing.assert_allclose(dw[H:-H], want[H:-H], rtol=0, atol=1e-12)
+    # Parseval on one block: sum |D|^2 = N sum (w d)^2, and the one-sided periodogram integrates to the windowed power
+    blk = rng.standard_normal(2 * H) * w
+    D = np.fft.rfft(blk)
+    p1 = 2.0 * np.abs(D) ** 2 / (fs * np.sum(w * w))
+    p1[0] /= 2; p1[-1] /= 2
+    assert abs(p1.sum() * fs / (2 * H) - np.sum(blk ** 2) / np.sum(w * w)) < 1e-12
+
+
+def test_p32_median_bias_and_unit_variance_out_of_white_noise():
+    """W4: b(n) = sum (-1)^(i+1) / i is the textbook bias of the median of n exponential variates (b(1) = 1,
+    b(3) = 5/6, -> ln 2), checked against a Monte-Carlo median; white noise of variance 9 is whitened to unit
+    variance by the running estimate ("converges quickly"), with the small upward bias of 1 / S-hat."""
+    from oracle import frontend as fe
+    assert fe.median_bias(1) == 1.0 and abs(fe.median_bias(3) - 5.0 / 6.0) < 1e-15
+    assert abs(fe.median_bias(27) - 0.71132) < 1e-5 and abs(fe.median_bias(9999) - math.log(2)) < 1e-4
+    rng = np.random.default_rng(32)
+    for n in (3, 9, 27):
+        med = np.median(rng.exponential(1.0, size=(40000, n)), axis=1).mean()
+        assert abs(med - fe.median_bias(n)) < 0.01
+    H, fs = 256, 2048.0
+    d = 3.0 * rng.standard_normal(H * 160)
+    dw, S, P = fe.whiten_stream(d, H, fs, 27)
+    assert np.all(S[0] == 0) and np.all(P[0] > 0) and np.all(S[1] == P[0])   # block 0 has no past: it only feeds the estimate
+    assert abs((S[40:] * fs / 2).mean() - 9.0) < 0.2                         # the PSD estimate is unbiased
+    assert 0.98 < dw[30 * H:-H].var() < 1.15                                 # unit variance (E 1/S-hat > 1/S by a few %)
+    # one loud glitch in the history does not move the median estimate ("robust against glitches")
+    d2 = d.copy(); d2[50 * H:50 * H + 40] += 500.0
+    _, S2, _ = fe.whiten_stream(d2, H, fs, 27)
+    _, _, P2 = fe.whiten_stream(d2, H, fs, 27)
+    r = S2[60] / S[60]                           # two of the 27 blocks hold the glitch: the median moves by a rank, the mean by > 20 x
+    assert np.median(r) < 1.2 and r.max() < 2.5 and np.median((P2[33:60].mean(axis=0) / P[33:60].mean(axis=0))[:20]) > 20
+
+
+def test_p33_coloured_noise_comes_out_flat():
+    """Eq. 1 on noise of KNOWN spectrum (AR(1) down-sampled): the whitened stream's Welch spectrum is flat at the
+    unit-variance level 2 / f_s within the estimator's scatter, while the input's varies by a factor > 5."""
+    from oracle import frontend as fe
+    R, H, fs = 8, 256, 2048.0
+    taps = workloads.frontend_taps(R, 192)
+    x = workloads.frontend_strain(33, 1, R * H * 150)[0]
+    y = fe.downsample(x, taps, R)
+    dw, S, P = fe.whiten_stream(y, H, fs, 27)
+    f, pin = scipy.signal.welch(y[40 * H:], fs=fs, nperseg=512)
+    f, pout = scipy.signal.welch(dw[40 * H:-H], fs=fs, nperseg=512)
+    band = (f > 20) & (f < 850)                                             # inside the down-sampler's pass band
+    assert pin[band].max() / pin[band].min() > 5.0
+    flat = pout[band] * fs / 2.0
+    assert abs(flat.mean() - 1.05) < 0.1 and flat.std() < 0.12
+    # and the estimate itself follows the known PSD of the generator (averaged over 8 adjacent bins of the 110 blocks;
+    # below 650 Hz, where the down-sampler's response is flat)
+    fk = np.arange(H + 1) * fs / (2 * H)
+    lo = (fk > 20) & (fk < 650)
+    ratio = (np.mean(S[40:], axis=0) / workloads.frontend_psd(fk))[lo]
+    ratio = ratio[:len(ratio) // 8 * 8].reshape(-1, 8).mean(axis=1)
+    assert np.all(np.abs(ratio - 1.0) < 0.12)
+
+
+def test_p34_gate_zeroes_exactly_the_excursion_and_its_pads():
+    """W5 (PAPER.md:87): with excursions on samples t0..t1 exactly [t0 - pad, t1 + pad] is zeroed, nothing else;
+    two excursions closer than 2 pad merge; the stream's edges clip the window."""
+    from oracle import frontend as fe
+    d = np.ones(4000) * 0.5
+    d[1000:1003] = 50.0; d[2500] = -60.0; d[2600] = 70.0; d[10] = 99.0
+    m = fe.gate_mask(d, 8.0, 64)
+    want = np.zeros(4000, bool)
+    want[1000 - 64:1002 + 64 + 1] = True; want[2500 - 64:2600 + 64 + 1] = True; want[0:10 + 64 + 1] = True
+    assert np.array_equal(m, want)
+    assert not fe.gate_mask(np.full(100, 8.0), 8.0, 5).any()                 # strict: |d_w| > threshold
+
+
+def test_p35_frontend_stream_latency_and_glitch_removal():
+    """W6: the stream the front end emits is the gated whitened stream delayed by one hop plus the pad; a glitch in
+    the raw data is gone from the output together with its pads, and nothing else is touched."""
+    from oracle import frontend as fe
+    R, H, fs, pad = 4, 256, 2048.0, 64
+    taps = workloads.frontend_taps(R, 96)
+    n_hops = 40
+    x = workloads.frontend_strain(35, 2, R * H * n_hops, fs_in=fs * R, glitches=[(1, 30.3 * H / fs, 400.0)])
+    out, dw = fe.frontend(x, taps, R, H, fs, 27, 8.0, pad)
+    lag = H + pad
+    for I in range(2):
+        m = fe.gate_mask(dw[I, :(n_hops - 1) * H], 8.0, pad)
+        want = np.where(m, 0.0, dw[I, :(n_hops - 1) * H])
+        assert np.array_equal(out[I, lag:], want[:n_hops * H - lag]) and np.all(out[I, :lag] == 0)
+    # once the PSD estimate has a few blocks (the first ones are whitened by one or three raw periodograms and gate
+    # themselves), the only zeros are the glitch and its pads
+    g0, warm = int(30.3 * H), 12 * H                                         # the glitch in output samples
+    m1 = fe.gate_mask(dw[1, :(n_hops - 1) * H], 8.0, pad)
+    z = np.nonzero(m1[warm:])[0] + warm
+    assert z.min() <= g0 - pad + 12 and z.max() >= g0 + pad and z.max() - z.min() < 2 * pad + 40 and abs(z.mean() - g0) < 20
+    assert not fe.gate_mask(dw[0, :(n_hops - 1) * H], 8.0, pad)[warm:].any()

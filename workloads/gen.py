@@ -406,3 +406,34 @@ def strain_for_config(idx, seconds=None):
             infos.append(info)
     return dict(strain=x, pos=pos, resp=resp, gmst=gmst, sigma=np.array(c["sigma"], float),
                 injections=infos, f_in=f_in)
+
+
+# ----------------------------------------------------------------------------- NEXT-4: front-end inputs
+def frontend_taps(decim=8, n_taps=192, beta=8.0):
+    """Down-sampling FIR (an INPUT of the front end): Kaiser-windowed sinc, cut-off at 90 % of the output Nyquist
+    frequency, unit DC gain.  PAPER.md:354: N_FIR-D ~ 192."""
+    j = np.arange(n_taps) - 0.5 * (n_taps - 1)
+    h = np.sinc(0.9 * j / decim) * np.kaiser(n_taps, beta)
+    return (h / h.sum()).astype(np.float32)
+
+
+def frontend_psd(f, fs_in=16384.0, rho=0.9, sigma=1.0):
+    """One-sided PSD (per Hz) of the AR(1) noise `frontend_strain` draws: sigma^2 (2 / fs) / |1 - rho e^{-i w}|^2."""
+    w = 2.0 * np.pi * np.asarray(f, float) / fs_in
+    return sigma ** 2 * (2.0 / fs_in) / (1.0 - 2.0 * rho * np.cos(w) + rho * rho)
+
+
+def frontend_strain(seed, n_det, n_samples, fs_in=16384.0, rho=0.9, sigma=1.0, glitches=()):
+    """Raw strain for the front end: stationary coloured noise x[n] = rho x[n-1] + sigma e[n] (a known PSD of modest
+    dynamic range standing in for a detector's spectrum, which is not available here) per detector, plus short
+    glitches (detector, time in s, amplitude): a few samples wide, far above the noise.  float32 [n_det][n_samples]."""
+    rng = np.random.default_rng(seed)
+    import scipy.signal
+    x = np.zeros((n_det, n_samples))
+    for I in range(n_det):
+        e = rng.standard_normal(n_samples + 2000)
+        x[I] = scipy.signal.lfilter([sigma], [1.0, -rho], e)[2000:]
+    for I, t, amp in glitches:
+        i = int(round(t * fs_in))
+        x[I, i:i + 24] += amp * np.hanning(24)
+    return x.astype(np.float32)
