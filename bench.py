@@ -633,6 +633,27 @@ def run_ours(args):
                     "note": "not part of the timed step"}
         del plan_s, wview, wtrig, sub_out
 
+    # ---- NEXT-4: the front end (down-sampling 16 384 -> 2048 Hz, Eq. 1 whitening, gating) on seeded coloured noise,
+    #      one 2-s hop per call, outside the timed step (the configs' strain is already whitened)
+    fe_info = None
+    if rank == 0:
+        Rf, Hf = 8, 4096
+        fe_ = sp.FrontEnd(D, workloads.frontend_taps(Rf, 192), decim=Rf, hop=Hf, n_hist=27, gate_pad=512,
+                          out_rate_hz=2048.0, gate_threshold=8.0)
+        raw = torch.from_numpy(workloads.frontend_strain(cfg["seed"], D, Rf * Hf * 4)).to(dev)
+        fo = torch.empty(D, Hf, dtype=torch.float32, device=dev)
+        ef = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        for rep in range(34):
+            if rep == 30: ef[0].record()
+            fe_.chunk(raw[:, (rep % 4) * Rf * Hf:(rep % 4 + 1) * Rf * Hf].contiguous(), out=fo)
+        ef[1].record()
+        torch.cuda.synchronize()
+        ms_f = ef[0].elapsed_time(ef[1]) / 4.0
+        fe_info = {"ms_per_hop": ms_f, "hop_seconds": Hf / 2048.0, "transform_points": 2 * Hf,
+                   "algorithmic_bytes_per_hop": D * (Rf * Hf + Hf) * 4,
+                   "note": "one CTA per detector, latency-bound by 2 x 13 barrier-separated FFT stages; not part of the timed step"}
+        del fe_, raw, fo
+
     # ---- end to end: pinned host strain in, host candidates and results out, every step
     e2e = None
     if not args.no_e2e:
@@ -736,7 +757,7 @@ def run_ours(args):
         "per_step": {"updates": upd_chunk, "candidates": n_cand / K if has_sky else None,
                      "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
         "roofline": dominant, "roofline_other": other, "pipe_probes": probes,
-        "next_rows": {"xi2": xi2_info, "rank": rank_info, "sub_sample_foreground": sub_info},
+        "next_rows": {"xi2": xi2_info, "rank": rank_info, "sub_sample_foreground": sub_info, "frontend": fe_info},
         "background_on_paper_grid_nside8": bg8_info,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }

@@ -299,6 +299,40 @@ int spiir_rank_candidates(const void* dev_ws, const spiir_rank_bins* bins, const
                           const spiir_sky_result* dev_fg, const spiir_xi2_result* dev_xi, int32_t n_slots,
                           double background_seconds, spiir_rank_result* dev_out, void* stream);
 
+/* NEXT-4 — the front end on the device (Sec. II A): FIR down-sampling of the raw
+ * strain (16 384 -> 2048 Hz, N_FIR ~ 192 taps), frequency-domain whitening (Eq. 1) against the running median PSD
+ * of the immediate past, and amplitude gating with zero padding on either side.  The paper describes the stage in
+ * words; the readings W1-W6 are stated in DESIGN.md section 11d:
+ *   y[m]   = sum_j taps[j] x[decim m + decim - 1 - j]                                   (x before the stream = 0)
+ *   block c = Hann(2 hop) * [hop c-1 | hop c] of y;  D = FFT(block);
+ *   S_n[k] = median over the n most recent PAST blocks' periodograms 2 |D[k]|^2 / (f_s sum w^2), n = min(c, n_hist)
+ *            made odd, divided by the median bias sum_{i<=n} (-1)^(i+1) / i;  block 0 is not emitted (no past);
+ *   d_w    = overlap-add of IFFT(D / sqrt(S_n f_s / 2))                                  (unit variance out)
+ *   gate   : |d_w| > gate_threshold zeroes that sample and gate_pad samples on either side.
+ * One call consumes ONE hop per detector and returns the `hop` gated samples t in [(c-1) hop - gate_pad,
+ * c hop - gate_pad) (zeros before the start of the stream): one hop plus gate_pad of latency.
+ * The Fourier transforms are hand-written shared-memory kernels inside the library (no cuFFT). */
+typedef struct spiir_frontend spiir_frontend;              /* opaque */
+typedef struct {
+  int32_t n_det;            /* 1..SPIIR_MAX_DET                                                        */
+  int32_t decim;            /* input rate / output rate, 1..16 (paper: 8)                              */
+  int32_t n_taps;           /* 1..512 and <= hop * decim (paper: ~192)                                 */
+  int32_t hop;              /* output samples per call, a power of two in 256..4096 (paper: 2 s = 4096) */
+  int32_t n_hist;           /* PSD history in blocks, 1..31 (paper: 56 s of 4-s blocks at a 2-s hop = 27) */
+  int32_t gate_pad;         /* output samples zeroed on either side of an excursion, <= hop / 2 (paper: 0.25 s = 512) */
+  float   out_rate_hz;      /* f_s of the output (2048)                                               */
+  float   gate_threshold;   /* in units of the whitened standard deviation                            */
+  const float* host_taps;   /* [n_taps], copied at init                                               */
+} spiir_frontend_desc;
+int spiir_frontend_workspace_bytes(const spiir_frontend_desc* desc, size_t* bytes);
+/* dev_workspace: 256-byte aligned, alive until spiir_frontend_free.  Synchronises the stream once (set-up). */
+int spiir_frontend_init(spiir_frontend** out, const spiir_frontend_desc* desc, void* dev_workspace, size_t bytes, void* stream);
+int spiir_frontend_reset(spiir_frontend* fe, void* stream);        /* back to the start of a stream */
+int spiir_frontend_free(spiir_frontend* fe);
+/*   dev_raw [n_det][hop * decim] float32; dev_out [n_det][hop] float32; dev_psd (optional, may be NULL)
+ *   [n_det][hop + 1]: the S_n used for this block (zeros for block 0).  Asynchronous on `stream`. */
+int spiir_frontend_chunk(spiir_frontend* fe, const float* dev_raw, float* dev_out, float* dev_psd, void* stream);
+
 /* Introspection: the layout chosen for a band (lanes per unit G, filters per lane
  * F, units, padded slots, shared-memory history depth) and counters for bench. */
 typedef struct {

@@ -43,6 +43,12 @@ class spiir_snr_view(C.Structure):
                 ("ring_len", C.c_int64), ("k_newest", C.c_int64), ("n_rows", C.c_int64)]
 
 
+class spiir_frontend_desc(C.Structure):
+    _fields_ = [("n_det", C.c_int32), ("decim", C.c_int32), ("n_taps", C.c_int32), ("hop", C.c_int32),
+                ("n_hist", C.c_int32), ("gate_pad", C.c_int32), ("out_rate_hz", C.c_float),
+                ("gate_threshold", C.c_float), ("host_taps", C.c_void_p)]
+
+
 class spiir_band_plan(C.Structure):
     _fields_ = [("lanes_per_unit", C.c_int32), ("filters_per_lane", C.c_int32), ("n_units", C.c_int32),
                 ("n_units_long", C.c_int32), ("smem_history", C.c_int32), ("smem_bytes", C.c_int32),
@@ -97,6 +103,11 @@ _SIGNATURES = {
     "spiir_rank_finalize": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "spiir_rank_candidates": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                         C.c_double, C.c_void_p, C.c_void_p]),
+    "spiir_frontend_workspace_bytes": (C.c_int, [C.POINTER(spiir_frontend_desc), C.POINTER(C.c_size_t)]),
+    "spiir_frontend_init": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(spiir_frontend_desc), C.c_void_p, C.c_size_t, C.c_void_p]),
+    "spiir_frontend_reset": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "spiir_frontend_free": (C.c_int, [C.c_void_p]),
+    "spiir_frontend_chunk": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "spiir_sky_table_set_build": (C.c_int, [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
                                            C.c_double, C.c_int32, C.c_double, C.c_void_p, C.c_void_p]),
     "spiir_sky_table_nearest": (C.c_int, [C.c_double, C.c_double, C.c_double, C.c_int32, C.c_void_p]),
@@ -496,3 +507,41 @@ class Ranker:
 
 def rank_to_numpy(out):
     return out.cpu().numpy().view(RANK_DTYPE).reshape(-1)
+
+
+class FrontEnd:
+    """Owns the workspace of one spiir_frontend (NEXT-4) and forwards to the C ABI."""
+
+    def __init__(self, n_det, taps, decim=8, hop=4096, n_hist=27, gate_pad=512, out_rate_hz=2048.0, gate_threshold=8.0):
+        import torch
+        self._taps = np.ascontiguousarray(taps, dtype=np.float32)
+        self.desc = spiir_frontend_desc(int(n_det), int(decim), len(self._taps), int(hop), int(n_hist), int(gate_pad),
+                                        float(out_rate_hz), float(gate_threshold), self._taps.ctypes.data)
+        n = C.c_size_t(0)
+        _check(lib().spiir_frontend_workspace_bytes(C.byref(self.desc), C.byref(n)))
+        self.ws = torch.empty(n.value + 256, dtype=torch.uint8, device="cuda")
+        base = (self.ws.data_ptr() + 255) // 256 * 256
+        self.h = C.c_void_p()
+        _check(lib().spiir_frontend_init(C.byref(self.h), C.byref(self.desc), C.c_void_p(base), n, _stream()))
+        self.n_det, self.hop, self.decim = int(n_det), int(hop), int(decim)
+
+    def reset(self):
+        _check(lib().spiir_frontend_reset(self.h, _stream()))
+
+    def chunk(self, raw, out=None, psd=None):
+        """raw float32 cuda [n_det][hop * decim] -> float32 cuda [n_det][hop] (spiir_frontend_chunk)."""
+        import torch
+        assert raw.is_cuda and raw.is_contiguous() and raw.dtype == torch.float32
+        assert raw.numel() == self.n_det * self.hop * self.decim
+        if out is None:
+            out = torch.empty(self.n_det, self.hop, dtype=torch.float32, device="cuda")
+        _check(lib().spiir_frontend_chunk(self.h, C.c_void_p(raw.data_ptr()), C.c_void_p(out.data_ptr()),
+                                          C.c_void_p(psd.data_ptr()) if psd is not None else None, _stream()))
+        return out
+
+    def __del__(self):
+        try:
+            if getattr(self, "h", None):
+                lib().spiir_frontend_free(self.h)
+        except Exception:
+            pass

@@ -1056,3 +1056,62 @@ def test_sub_sample_alignment(sp, U):
     assert np.mean(res["null2"][sig]) < np.mean(res1["null2"][sig])
     assert np.mean(res["pix"][sig] == p_true[sig]) >= np.mean(res1["pix"][sig] == p_true[sig])
     assert np.mean(res["pix"][sig] == p_true[sig]) > 0.5
+
+
+# ------------------------------------------------------------------ NEXT-4: front end on the device
+@pytest.mark.parametrize("shape", ["paper", "small"])
+def test_frontend_downsample_whiten_gate(sp, U, shape):
+    """spiir_frontend_chunk against oracle/frontend.py (W1-W6) on seeded coloured noise with glitches, hop by hop from
+    the start of a stream: the paper's shape (16 384 -> 2048 Hz, 192 taps, 2-s hops = 8192-point transforms, 27
+    blocks of PSD history, 0.25 s pads) and a small one (decimation 4, 512-point transforms,
+    odd history).  Tolerance: 1e-4 of the whitened standard deviation (= 1) once the estimate has three blocks; the
+    first emitted hops divide by single raw periodograms and are compared at 5e-3 of the hop's rms.
+    The gate decision |d_w| > threshold is float32 on the device: exact agreement is required wherever the oracle's
+    |d_w| is not within 1e-3 of the threshold (nowhere, for these inputs)."""
+    import torch
+    from oracle import frontend as fe
+    if shape == "paper":
+        D, R, nt, H, nh, pad, fs, n_hops, thr = 3, 8, 192, 4096, 27, 512, 2048.0, 34, 8.0
+        gl = [(0, 41.3, 300.0), (2, 20.05, -500.0), (2, 20.4, 400.0), (1, 59.99, 350.0)]
+    else:
+        D, R, nt, H, nh, pad, fs, n_hops, thr = 2, 4, 64, 256, 9, 100, 2048.0, 30, 6.0
+        gl = [(0, 1.51, 300.0), (1, 2.999, 250.0)]
+    taps = workloads.frontend_taps(R, nt)
+    x = workloads.frontend_strain(70 + n_hops, D, R * H * n_hops, fs_in=fs * R, glitches=gl)
+    ref, dw_ref = fe.frontend(x, taps, R, H, fs, nh, thr, pad)
+    # knife-edge gate decisions (|d_w| within 1e-3 of the threshold) may fall either way in float32: the device's zeros
+    # must contain those of threshold + 1e-3 and be contained in those of threshold - 1e-3
+    ref_hi, _ = fe.frontend(x, taps, R, H, fs, nh, thr + 1e-3, pad)
+    ref_lo, _ = fe.frontend(x, taps, R, H, fs, nh, thr - 1e-3, pad)
+    f = sp.FrontEnd(D, taps, decim=R, hop=H, n_hist=nh, gate_pad=pad, out_rate_hz=fs, gate_threshold=thr)
+    xd = torch.from_numpy(x).cuda()
+    psd = torch.zeros(D, H + 1, dtype=torch.float32, device="cuda")
+    got = np.zeros((D, n_hops * H), np.float32)
+    for c in range(n_hops):
+        o = f.chunk(xd[:, c * H * R:(c + 1) * H * R].contiguous(), psd=psd)
+        got[:, c * H:(c + 1) * H] = o.cpu().numpy()
+        if c == 12:                                                          # the PSD used for block 12 against the oracle's
+            y = fe.downsample(x[1], taps, R)
+            _, S, _ = fe.whiten_stream(y, H, fs, nh)
+            np.testing.assert_allclose(psd[1].cpu().numpy(), S[12], rtol=2e-4, atol=1e-12)
+    torch.cuda.synchronize()
+    zero_ref, zero_got = ref == 0.0, got == 0.0
+    assert np.all(zero_got[ref_hi == 0.0]) and np.all((ref_lo == 0.0)[zero_got]), "gated samples differ"
+    ref = np.where(zero_got, 0.0, np.where(zero_ref, ref_hi, ref))           # values compared where the device kept them
+    assert zero_ref[:, 6 * H:].sum() >= (len(gl) - 1) * 2 * pad              # the glitches and their pads are gone (two windows overlap)
+    warm = 5 * H + pad                                                       # output index from which >= 3 blocks back the estimate
+    err = np.abs(got - ref)
+    assert err[:, warm:].max() <= 1e-4, err[:, warm:].max()
+    # warm-up: the first emitted hops divide by one or three raw periodograms, whose smallest bins are float32
+    # cancellation noise of the transform relative to the largest ones; compared against the hop's rms
+    for c in range(warm // H + 1):
+        sl = slice(c * H, min((c + 1) * H, warm))
+        rms = max(1.0, float(np.sqrt(np.mean(ref[:, sl] ** 2))))
+        assert err[:, sl].max() <= 5e-3 * rms, (c, err[:, sl].max(), rms)
+    assert 0.9 < got[:, 12 * H:][~zero_got[:, 12 * H:]].std() < (1.15 if nh >= 27 else 1.3)   # unit variance out (a short history biases 1 / S-hat up)
+    # reset: the same stream again gives the same output bit for bit
+    f.reset()
+    o0 = f.chunk(xd[:, :H * R].contiguous())
+    o1 = f.chunk(xd[:, H * R:2 * H * R].contiguous())
+    torch.cuda.synchronize()
+    assert np.array_equal(o0.cpu().numpy(), got[:, :H]) and np.array_equal(o1.cpu().numpy(), got[:, H:2 * H])
