@@ -195,6 +195,19 @@ int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const 
                                int32_t n_slots, int32_t factor, int32_t half_width, spiir_c32* dev_out,
                                spiir_trigger* dev_trig_out, spiir_snr_view* out_view, void* stream);
 
+/* The same for the time-slide background, so that foreground and background are the SAME statistic when
+ * the sub-sample alignment is on: row s * n_slides + (slide - 1) of dev_out holds, for detector I, the window around
+ * k_s - slide * step_samples * host_slide_mult[I] (the trigger detector's window is not moved), resampled as above;
+ * dev_trig_out [n_slots * n_slides] re-addresses the candidate to that row (valid = 0 and zero windows when ANY
+ * detector's window or its one-sample interpolation margin leaves the view).  coherent_sky_search on *out_view with
+ * these slots returns results laid out [n_slots][n_slides], as timeslide_background does.
+ * dev_out: n_slides * spiir_snr_upsample_elems() complex elements. */
+int spiir_snr_upsample_windows_slides(const spiir_snr_view* view, int32_t n_det, const spiir_trigger* dev_trig,
+                                      int32_t n_slots, int32_t n_slides, int64_t step_samples,
+                                      const int32_t* host_slide_mult, int32_t factor, int32_t half_width,
+                                      spiir_c32* dev_out, spiir_trigger* dev_trig_out, spiir_snr_view* out_view,
+                                      void* stream);
+
 /* A look-up table prepared for the device (opaque).  The plan re-orders the
  * directions so that those sharing one tuple of inter-detector delays are
  * adjacent, and stores for each direction the projector U2 U2^T (Eq. 28,

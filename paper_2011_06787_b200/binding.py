@@ -112,6 +112,9 @@ _SIGNATURES = {
                                            C.c_double, C.c_int32, C.c_double, C.c_void_p, C.c_void_p]),
     "spiir_sky_table_nearest": (C.c_int, [C.c_double, C.c_double, C.c_double, C.c_int32, C.c_void_p]),
     "spiir_snr_upsample_elems": (C.c_int, [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]),
+    "spiir_snr_upsample_windows_slides": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_int64,
+                                                   C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                   C.c_void_p]),
     "spiir_snr_upsample_windows": (C.c_int, [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "spiir_template_autocorr": (C.c_int, [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]),
@@ -204,18 +207,27 @@ class SnrView:
                                 ring_len - 1 if k_newest is None else int(k_newest), rows)
 
 
-def upsample_windows(view, n_det, trig, n_slots, factor, half_width):
-    """spiir_snr_upsample_windows: returns (SnrView over the resampled windows, re-addressed triggers
-    uint8 cuda [n_slots][40]); the view keeps the window tensor alive."""
+def upsample_windows(view, n_det, trig, n_slots, factor, half_width, n_slides=0, step=0, mult=None):
+    """spiir_snr_upsample_windows (n_slides = 0) / spiir_snr_upsample_windows_slides: returns (SnrView over the
+    resampled windows, re-addressed triggers uint8 cuda [n_slots * max(1, n_slides)][40]); the view keeps the window
+    tensor alive."""
     import torch
     n = C.c_size_t(0)
     _check(lib().spiir_snr_upsample_elems(n_det, n_slots, int(factor), int(half_width), C.byref(n)))
-    out = torch.empty(max(int(n.value), 2), 2, dtype=torch.float32, device="cuda")
-    trig_out = torch.empty(n_slots, 40, dtype=torch.uint8, device="cuda")
+    S1 = max(1, int(n_slides))
+    out = torch.empty(max(int(n.value) * S1, 2), 2, dtype=torch.float32, device="cuda")
+    trig_out = torch.empty(n_slots * S1, 40, dtype=torch.uint8, device="cuda")
     ov = spiir_snr_view()
-    _check(lib().spiir_snr_upsample_windows(C.byref(view.c), n_det, C.c_void_p(trig.data_ptr()), n_slots, int(factor),
-                                            int(half_width), C.c_void_p(out.data_ptr()),
-                                            C.c_void_p(trig_out.data_ptr()), C.byref(ov), _stream()))
+    if n_slides:
+        m = (C.c_int32 * n_det)(*[int(x) for x in mult])
+        _check(lib().spiir_snr_upsample_windows_slides(C.byref(view.c), n_det, C.c_void_p(trig.data_ptr()), n_slots,
+                                                       int(n_slides), C.c_int64(int(step)), m, int(factor), int(half_width),
+                                                       C.c_void_p(out.data_ptr()), C.c_void_p(trig_out.data_ptr()),
+                                                       C.byref(ov), _stream()))
+    else:
+        _check(lib().spiir_snr_upsample_windows(C.byref(view.c), n_det, C.c_void_p(trig.data_ptr()), n_slots, int(factor),
+                                                int(half_width), C.c_void_p(out.data_ptr()),
+                                                C.c_void_p(trig_out.data_ptr()), C.byref(ov), _stream()))
     v = SnrView(raw=ov)
     v._keep = out
     return v, trig_out

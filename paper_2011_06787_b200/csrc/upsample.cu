@@ -12,6 +12,8 @@
 // One CTA per (slot, detector), threads stride over the output samples (coalesced stores, reads of 2 H + 3
 // consecutive ring samples served by L1 across the R phases; one 64-bit modulo per thread, then wraps).
 // HBM-bound: 8 (2 H + 3) B read + 8 (2 R H + 2) B written per (slot, detector).
+#include <cstring>
+
 #include "spiir_internal.cuh"
 
 namespace spiir {
@@ -22,41 +24,60 @@ constexpr int kUpMaxFactor = 16;
 struct UpParams {
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest, n_rows;
   const spiir_trigger* trig; int32_t n_slots, n_det;
+  int32_t S1;                                        // rows per slot: 1 (foreground) or the number of slides
+  int32_t slides;                                    // 1: row (slot, s) holds the windows of slide s + 1
+  int64_t step; int32_t mult[SPIIR_MAX_DET];
   int32_t R, H, Lw; int64_t Lp;
   float4 w[kUpMaxFactor];
   float2* out; spiir_trigger* trig_out;
 };
 
-// the re-addressed candidates (one thread per slot)
-__global__ void __launch_bounds__(kUpThreads) k_upsample_trig(const __grid_constant__ UpParams P) {
-  const int s = blockIdx.x * kUpThreads + threadIdx.x;
-  if (s >= P.n_slots) return;
-  const spiir_trigger t = P.trig[s];
+// Centre of detector I's window for row (slot, si): the candidate's sample, moved s step mult[I] earlier in the
+// detectors other than the trigger detector for slide s = si + 1; ok = every detector's window and
+// its interpolation margin lie in the view.
+__device__ __forceinline__ bool up_row(const UpParams& P, const spiir_trigger& t, int si, int64_t* centre) {
   const int64_t k_old = P.k_newest - P.ring_len + 1 > 0 ? P.k_newest - P.ring_len + 1 : 0;
-  const bool ok = t.valid && t.tmpl >= 0 && t.tmpl < P.n_rows && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
+  bool ok = t.valid && t.tmpl >= 0 && t.tmpl < P.n_rows && t.det >= 0 && t.det < P.n_det;
+  for (int I = 0; I < P.n_det; ++I) {
+    const int64_t c = t.k - ((P.slides && I != t.det) ? (int64_t)(si + 1) * P.step * P.mult[I] : 0);
+    centre[I] = c;
+    ok = ok && c - P.H - 1 >= k_old && c + P.H + 1 <= P.k_newest;
+  }
+  return ok;
+}
+
+// the re-addressed candidates (one thread per row)
+__global__ void __launch_bounds__(kUpThreads) k_upsample_trig(const __grid_constant__ UpParams P) {
+  const int w = blockIdx.x * kUpThreads + threadIdx.x;
+  if (w >= P.n_slots * P.S1) return;
+  const int s = w / P.S1, si = w - s * P.S1;
+  const spiir_trigger t = P.trig[s];
+  int64_t centre[SPIIR_MAX_DET];
+  const bool ok = up_row(P, t, si, centre);
   spiir_trigger o = t;
-  o.valid = ok ? 1 : 0; o.tmpl = s; o.k = (int64_t)P.R * P.H;
+  o.valid = ok ? 1 : 0; o.tmpl = w; o.k = (int64_t)P.R * P.H;
   if (!t.valid) { o.det = 0; o.z_re = o.z_im = o.snr = 0.f; }
   o._pad = 0; o._pad2 = 0.f;
-  P.trig_out[s] = o;
+  P.trig_out[w] = o;
 }
 
 // the windows: one CTA per (slot, detector), threads stride over the output samples (coalesced stores; the
 // 2 H + 3 ring samples a window reads are consecutive and stay in L1 across the R phases).  One 64-bit
 // modulo per thread places the window in the ring; after that a sample's neighbours are conditional wraps.
 __global__ void __launch_bounds__(kUpThreads) k_upsample(const __grid_constant__ UpParams P) {
-  const int s = blockIdx.x, I = blockIdx.y;
+  const int w = blockIdx.x, I = blockIdx.y;
+  const int s = w / P.S1, si = w - s * P.S1;
   const spiir_trigger t = P.trig[s];
-  const int64_t k_old = P.k_newest - P.ring_len + 1 > 0 ? P.k_newest - P.ring_len + 1 : 0;
-  const bool ok = t.valid && t.tmpl >= 0 && t.tmpl < P.n_rows && t.k - P.H - 1 >= k_old && t.k + P.H + 1 <= P.k_newest;
-  float2* out = P.out + ((size_t)I * P.n_slots + s) * P.Lp;
+  int64_t centre[SPIIR_MAX_DET];
+  const bool ok = up_row(P, t, si, centre);
+  float2* out = P.out + ((size_t)I * P.n_slots * P.S1 + w) * P.Lp;
   if (!ok) {
     for (int u = threadIdx.x; u < P.Lp; u += kUpThreads) out[u] = make_float2(0.f, 0.f);
     return;
   }
   const float2* zr = P.z + (size_t)I * P.det_stride + (size_t)t.tmpl * P.row_stride;
   const int64_t L = P.ring_len;
-  const int64_t i0 = (t.k - P.H) % L;                    // t.k - H >= 1 here
+  const int64_t i0 = (centre[I] - P.H) % L;              // centre - H >= 1 here
   auto wrap = [L](int64_t i) { return i >= L ? i - L : (i < 0 ? i + L : i); };
   for (int u = threadIdx.x; u < P.Lp; u += kUpThreads) {
     float2 v = make_float2(0.f, 0.f);
@@ -93,20 +114,26 @@ int spiir_snr_upsample_elems(int32_t n_det, int32_t n_slots, int32_t factor, int
   return SPIIR_OK;
 }
 
-int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const spiir_trigger* dev_trig,
-                               int32_t n_slots, int32_t factor, int32_t half_width, spiir_c32* dev_out,
-                               spiir_trigger* dev_trig_out, spiir_snr_view* out_view, void* stream) {
+static int upsample_run(const spiir_snr_view* view, int32_t n_det, const spiir_trigger* dev_trig, int32_t n_slots,
+                        int32_t n_slides, int64_t step, const int32_t* mult, int32_t factor, int32_t half_width,
+                        spiir_c32* dev_out, spiir_trigger* dev_trig_out, spiir_snr_view* out_view, void* stream) {
   size_t elems = 0;
   int rc = spiir_snr_upsample_elems(n_det, n_slots, factor, half_width, &elems);
   if (rc) return rc;
   SPIIR_REQUIRE(view && view->dev_z && dev_trig && dev_out && dev_trig_out && out_view, "a pointer is NULL");
   SPIIR_REQUIRE(view->ring_len >= 1 && view->k_newest >= 0 && view->n_rows >= 1, "bad view");
   SPIIR_REQUIRE(((uintptr_t)dev_out & 15) == 0, "dev_out must be 16-byte aligned");
+  SPIIR_REQUIRE(n_slides >= 0 && (n_slides == 0 || (mult && step >= 0)), "time slides need host_slide_mult and step >= 0");
+  const int S1 = n_slides > 0 ? n_slides : 1;
+  SPIIR_REQUIRE((long long)n_slots * S1 <= 0x7fffffffLL, "too many rows");
   UpParams P;
+  memset(&P, 0, sizeof(P));
   P.z = (const float2*)view->dev_z;
   P.det_stride = view->det_stride; P.row_stride = view->row_stride;
   P.ring_len = view->ring_len; P.k_newest = view->k_newest; P.n_rows = view->n_rows;
   P.trig = dev_trig; P.n_slots = n_slots; P.n_det = n_det;
+  P.S1 = S1; P.slides = n_slides > 0 ? 1 : 0; P.step = step;
+  for (int I = 0; I < SPIIR_MAX_DET; ++I) P.mult[I] = (n_slides > 0 && I < n_det) ? mult[I] : 0;
   P.R = factor; P.H = half_width; P.Lw = 2 * factor * half_width + 1;
   P.Lp = ((int64_t)P.Lw + 1) & ~(int64_t)1;
   for (int r = 0; r < kUpMaxFactor; ++r) {
@@ -116,18 +143,35 @@ int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const 
                          (float)(-(m + 1.0) * m * (m - 2.0) / 2.0), (float)((m + 1.0) * m * (m - 1.0) / 6.0));
   }
   P.out = (float2*)dev_out; P.trig_out = dev_trig_out;
+  const long long n_rows = (long long)n_slots * S1;
   out_view->dev_z = dev_out;
-  out_view->det_stride = (int64_t)n_slots * P.Lp;
+  out_view->det_stride = n_rows * P.Lp;
   out_view->row_stride = P.Lp;
   out_view->ring_len = P.Lp;
   out_view->k_newest = P.Lw - 1;
-  out_view->n_rows = n_slots;
-  if (n_slots == 0) return SPIIR_OK;
-  k_upsample_trig<<<(n_slots + kUpThreads - 1) / kUpThreads, kUpThreads, 0, (cudaStream_t)stream>>>(P);
-  k_upsample<<<dim3((unsigned)n_slots, (unsigned)n_det), kUpThreads, 0, (cudaStream_t)stream>>>(P);
+  out_view->n_rows = n_rows;
+  if (n_rows == 0) return SPIIR_OK;
+  k_upsample_trig<<<(unsigned)((n_rows + kUpThreads - 1) / kUpThreads), kUpThreads, 0, (cudaStream_t)stream>>>(P);
+  k_upsample<<<dim3((unsigned)n_rows, (unsigned)n_det), kUpThreads, 0, (cudaStream_t)stream>>>(P);
   count_launch(2);
   SPIIR_CUDA_OK(cudaGetLastError());
   return SPIIR_OK;
+}
+
+int spiir_snr_upsample_windows(const spiir_snr_view* view, int32_t n_det, const spiir_trigger* dev_trig,
+                               int32_t n_slots, int32_t factor, int32_t half_width, spiir_c32* dev_out,
+                               spiir_trigger* dev_trig_out, spiir_snr_view* out_view, void* stream) {
+  return upsample_run(view, n_det, dev_trig, n_slots, 0, 0, nullptr, factor, half_width, dev_out, dev_trig_out, out_view, stream);
+}
+
+int spiir_snr_upsample_windows_slides(const spiir_snr_view* view, int32_t n_det, const spiir_trigger* dev_trig,
+                                      int32_t n_slots, int32_t n_slides, int64_t step_samples,
+                                      const int32_t* host_slide_mult, int32_t factor, int32_t half_width,
+                                      spiir_c32* dev_out, spiir_trigger* dev_trig_out, spiir_snr_view* out_view,
+                                      void* stream) {
+  SPIIR_REQUIRE(n_slides >= 1, "n_slides must be >= 1");
+  return upsample_run(view, n_det, dev_trig, n_slots, n_slides, step_samples, host_slide_mult, factor, half_width,
+                      dev_out, dev_trig_out, out_view, stream);
 }
 
 }  // extern "C"

@@ -1055,6 +1055,40 @@ def test_sub_sample_alignment(sp, U):
     sig = np.arange(rows) >= 6
     assert np.mean(res["null2"][sig]) < np.mean(res1["null2"][sig])
     assert np.mean(res["pix"][sig] == p_true[sig]) >= np.mean(res1["pix"][sig] == p_true[sig])
+    # ---- the time-slide background on the same finer grid: companions read s * step earlier, every
+    #      detector's window resampled around its own centre; rows [slot][slide]
+    S, step, mult = 4, 60, [1, 1, 1]
+    sview, strig = sp.upsample_windows(view, D, sp.triggers_from_numpy(trig), rows, R, H, n_slides=S, step=step, mult=mult)
+    torch.cuda.synchronize()
+    gs = sview._keep.cpu().numpy().reshape(-1)[:D * rows * S * Lp * 2].view(np.complex64).reshape(D, rows * S, Lp)
+    refs, oks = oracle.upsample_windows(z32, L, k_newest, trig["valid"], trig["tmpl"], trig["det"], trig["k"], R, H,
+                                        n_slides=S, step=step, slide_mult=mult)
+    t3 = strig.cpu().numpy().view(sp.TRIGGER_DTYPE).reshape(-1)
+    assert np.array_equal(t3["valid"], oks) and 0.3 * rows * S < oks.sum() < rows * S      # late slides leave the ring
+    assert np.array_equal(t3["tmpl"], np.arange(rows * S)) and int(sview.c.n_rows) == rows * S
+    vs = oks == 1
+    assert np.all(gs[:, ~vs] == 0) and np.array_equal(gs[:, vs, 0:Lw:R], refs[:, vs, 0:Lw:R].astype(np.complex64))
+    assert np.all(np.abs(gs[:, :, :Lw] - refs) <= 1e-6 * np.abs(refs).max(axis=2, keepdims=True) + 1e-30)
+    plan_s = sp.SkyPlan(UR.astype(np.float32), dR, max_slots=rows * S)
+    res_s = sp.results_to_numpy(plan_s.search(sview, strig, rows * S))
+    torch.cuda.synchronize()
+    U.check_sky(res_s, np.ascontiguousarray(gs), Lp, Lw - 1, UR.astype(np.float32), dR, t3)  # O6 on the device's windows
+    refsp = np.zeros((D, rows * S, Lp), complex)
+    refsp[:, :, :Lw] = refs
+    os_, ps_, _ = oracle.sky_search(UR.astype(np.float32), dR, refsp, rows * S * Lp, Lp, Lp, Lw - 1, oks,
+                                    np.arange(rows * S), np.repeat(trig["det"], S), np.full(rows * S, R * H))
+    assert np.all(np.abs(res_s["coh2"][vs] - os_[vs, 0, 0]) <= 1e-4 * os_[vs, 0, 0]) and np.all(res_s["pix"][~vs] == -1)
+    # with factor 1 the windows are bit copies and the search on them IS timeslide_background on the integer grid
+    # (same samples, same arithmetic): identical results wherever both windows exist
+    v1, t1 = sp.upsample_windows(view, D, sp.triggers_from_numpy(trig), rows, 1, H, n_slides=S, step=step, mult=mult)
+    plan_1s = sp.SkyPlan(U1.astype(np.float32), d1, max_slots=rows * S)
+    r_w = sp.results_to_numpy(plan_1s.search(v1, t1, rows * S))
+    r_b = sp.results_to_numpy(plan_1s.background(view, sp.triggers_from_numpy(trig), rows, S, step, mult))
+    torch.cuda.synchronize()
+    both = (r_w["pix"] >= 0) & (r_b["pix"] >= 0)
+    assert both.sum() >= 0.3 * rows * S and np.all((r_w["pix"] >= 0) <= (r_b["pix"] >= 0))   # (the windows need one sample of margin more)
+    for fld in ("coh2", "tot2", "null2", "pix"):
+        assert np.array_equal(r_w[fld][both], r_b[fld][both]), fld
     assert np.mean(res["pix"][sig] == p_true[sig]) > 0.5
 
 
