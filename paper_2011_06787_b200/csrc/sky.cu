@@ -539,9 +539,13 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
   pl->ws = (char*)dev_workspace;
   cudaStream_t st = (cudaStream_t)stream;
   std::vector<float> slots;
-  // debugging knob: SPIIR_SKY_KERNEL=general makes three-detector plans run the general kernel (A/B comparisons)
+  // Which kernel three-detector plans run.  Default: the general kernel k_sky — measured equal to k_sky3 (sky3.cu) at
+  // 12 288 and 49 152 directions and faster on coarse grids (768 directions: 4.3 against 5.5 ms for the same 4.06 M
+  // events; profiles/r2_ncu_summary.md section 2).  SPIIR_SKY_KERNEL=three-detector selects k_sky3 (kept for its
+  // asynchronous staging pipeline and as the record of why restructuring did not pay: both are bound by the delivery of
+  // operands from shared memory).
   const char* knob = getenv("SPIIR_SKY_KERNEL");
-  const bool force_general = knob && strcmp(knob, "general") == 0;
+  const bool force_general = !(knob && strcmp(knob, "three-detector") == 0);
   for (int T = 0; T < D; ++T) {
     spiir_sky_stream& S = pl->st[T];
     int ps = 0;

@@ -183,7 +183,16 @@ def _snippet_case(sp, n_rows, nside, n_windows, half, seed, gmst=0.7):
     return u2, delay, zc, zd, trig, truth
 
 
-def test_sky_foreground_and_signal_recovery(sp, U):
+@pytest.mark.parametrize("kernel", ["general", "three-detector"])
+def test_sky_foreground_and_signal_recovery(sp, U, kernel, monkeypatch):
+    if kernel == "three-detector":
+        monkeypatch.setenv("SPIIR_SKY_KERNEL", "three-detector")
+    else:
+        monkeypatch.delenv("SPIIR_SKY_KERNEL", raising=False)
+    _sky_foreground_and_signal_recovery(sp, U)
+
+
+def _sky_foreground_and_signal_recovery(sp, U):
     import torch
     u2, delay, zc, zd, trig, truth = _snippet_case(sp, 200, 16, 1, 102, seed=21)
     trig["valid"][::7] = 0                                   # some empty slots
@@ -206,8 +215,13 @@ def test_sky_foreground_and_signal_recovery(sp, U):
     assert np.mean(res["coh2"][sig]) > 4 * np.mean(res["coh2"][~truth["is_signal"] & (trig["valid"] == 1)])
 
 
-def test_sky_time_slides(sp, U):
+@pytest.mark.parametrize("kernel", ["general", "three-detector"])
+def test_sky_time_slides(sp, U, kernel, monkeypatch):
     import torch
+    if kernel == "three-detector":                                           # k_sky3 (sky3.cu) instead of the default k_sky
+        monkeypatch.setenv("SPIIR_SKY_KERNEL", "three-detector")
+    else:
+        monkeypatch.delenv("SPIIR_SKY_KERNEL", raising=False)
     n_rows, S, half = 96, 7, 102
     W = 2 * half + 1
     u2, delay, zc, zd, trig, truth = _snippet_case(sp, n_rows, 16, S + 1, half, seed=22)
@@ -513,11 +527,10 @@ def _subset_trig(trig_rows, sel, D):
 def test_sky_unaligned_view(sp, U, kernel, monkeypatch):
     """A view whose rows are not 16-byte friendly (odd ring_len 501, base pointer 8 bytes past an aligned address):
     the window staging cannot use TMA bulk copies and takes the 8-byte cp.async path of each kernel.  Foreground,
-    slides and a wrapped ring against O6 / O7, for the three-detector kernel and (SPIIR_SKY_KERNEL=general) the
-    general one."""
+    slides and a wrapped ring against O6 / O7, for the general kernel and (SPIIR_SKY_KERNEL=three-detector) k_sky3."""
     import torch
-    if kernel == "general":
-        monkeypatch.setenv("SPIIR_SKY_KERNEL", "general")
+    if kernel == "three-detector":
+        monkeypatch.setenv("SPIIR_SKY_KERNEL", "three-detector")
     else:
         monkeypatch.delenv("SPIIR_SKY_KERNEL", raising=False)
     cfg = workloads.config(1)
@@ -1149,3 +1162,104 @@ def test_frontend_downsample_whiten_gate(sp, U, shape):
     o1 = f.chunk(xd[:, H * R:2 * H * R].contiguous())
     torch.cuda.synchronize()
     assert np.array_equal(o0.cpu().numpy(), got[:, :H]) and np.array_equal(o1.cpu().numpy(), got[:, H:2 * H])
+
+
+# ------------------------------------------------------------------ out-of-bounds writes (compute-sanitizer is closed on this pool)
+def test_workspace_guard_bands(sp, U):
+    """compute-sanitizer cannot be run on this pool (gpurun refuses it), so out-of-bounds WRITES are looked for
+    directly: every buffer the library writes — the bank's workspace, the sky plan's workspace, the trigger / result /
+    SNR outputs, the front end's workspace and output — is carved out of a larger allocation filled with a byte
+    pattern, the whole path runs (multirate bank with a long-delay template, both peak modes, the three-detector and
+    the general sky kernel with slides on a wrapped ring, xi^2, the front end), and the guard bands on both sides of
+    every buffer must still hold the pattern."""
+    import ctypes as C
+    import torch
+    G = 1 << 16                                                               # 64 KB of guard on either side
+    guards = []
+
+    def guarded(nbytes, align=256):
+        raw = torch.full((nbytes + 2 * G + align,), 0xA5, dtype=torch.uint8, device="cuda")
+        off = (-(raw.data_ptr() + G)) % align + G
+        guards.append((raw, off, nbytes))
+        return raw, raw.data_ptr() + off
+
+    L_ = sp.lib()
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    cfg = workloads.config(4)
+    T, D = 48, 3
+    bank = workloads.bank_for_config(4, n_templates=T)                       # 20 chirp-matched long-delay templates + random
+    dec, itp = workloads.halfband_taps()
+    ring = 5 * 2048
+    desc, keep = sp.make_desc(bank, D, 4096, ring, 16, dec, itp)
+    nb = C.c_size_t(0)
+    assert L_.spiir_bank_workspace_bytes(C.byref(desc), C.byref(nb)) == 0
+    _, ws = guarded(nb.value)
+    h = C.c_void_p()
+    assert L_.spiir_bank_init(C.byref(h), C.byref(desc), C.c_void_p(ws), nb, st) == 0
+    x = torch.from_numpy(workloads.strain_for_config(4, seconds=8)["strain"]).cuda()
+    _, p_out = guarded(D * T * 2048 * 8)
+    _, p_trig = guarded(D * T * 40)
+    _, p_cnt = guarded(4, align=16)
+    u2, delay = _table(cfg, nside=8, gmst=0.4)
+    pb = C.c_size_t(0)
+    plans = []
+    for kern in ("", "three-detector"):
+        import os
+        if kern:
+            os.environ["SPIIR_SKY_KERNEL"] = kern
+        else:
+            os.environ.pop("SPIIR_SKY_KERNEL", None)
+        assert L_.spiir_sky_plan_workspace_bytes(D, len(u2), D * T, C.byref(pb)) == 0
+        _, pws = guarded(pb.value)
+        ph = C.c_void_p()
+        u2c, dlc = np.ascontiguousarray(u2, np.float32), np.ascontiguousarray(delay, np.int32)
+        assert L_.spiir_sky_plan_init(C.byref(ph), D, len(u2), D * T, u2c.ctypes.data_as(C.c_void_p),
+                                      dlc.ctypes.data_as(C.c_void_p), C.c_void_p(pws), pb, st) == 0
+        plans.append(ph)
+    os.environ.pop("SPIIR_SKY_KERNEL", None)
+    S = 3
+    _, p_fg = guarded(D * T * 16)
+    _, p_bg = guarded(D * T * S * 16)
+    _, p_xi = guarded(D * T * S * 24)
+    nj = 20
+    ac = torch.zeros(T, 2 * nj + 1, 2, device="cuda"); ac[:, nj, 0] = 1.0
+    dl_dev = torch.from_numpy(np.ascontiguousarray(delay, np.int32)).cuda()
+    mult = (C.c_int32 * D)(1, 1, 1)
+    view = sp.spiir_snr_view()
+    for c in range(8):                                                        # the 5-s ring wraps
+        xc = x[:, c * 4096:(c + 1) * 4096].contiguous()
+        assert L_.spiir_filter_chunk(h, C.c_void_p(xc.data_ptr()), 4096, C.c_void_p(p_out), st) == 0
+        for mode in (1, 0):
+            assert L_.spiir_peaks(h, C.c_float(1.0), mode, C.c_void_p(p_trig), C.c_void_p(p_cnt), st) == 0
+        assert L_.spiir_bank_snr_view(h, C.byref(view)) == 0
+        for ph in plans:
+            assert L_.coherent_sky_search(ph, C.byref(view), C.c_void_p(p_trig), D * T, C.c_void_p(p_fg), None, st) == 0
+            assert L_.timeslide_background(ph, C.byref(view), C.c_void_p(p_trig), D * T, S, C.c_int64(2048), mult,
+                                           C.c_void_p(p_bg), st) == 0
+        assert L_.spiir_signal_consistency(C.byref(view), D, len(u2), C.c_void_p(dl_dev.data_ptr()), C.c_void_p(p_trig),
+                                           C.c_void_p(p_bg), D * T, S, C.c_int64(2048), mult, C.c_void_p(ac.data_ptr()),
+                                           nj, C.c_void_p(p_xi), st) == 0
+    # the front end
+    taps = workloads.frontend_taps(8, 192)
+    fd = sp.spiir_frontend_desc(D, 8, 192, 1024, 9, 256, 2048.0, 8.0, taps.ctypes.data)
+    fb = C.c_size_t(0)
+    assert L_.spiir_frontend_workspace_bytes(C.byref(fd), C.byref(fb)) == 0
+    _, fws = guarded(fb.value)
+    fh = C.c_void_p()
+    assert L_.spiir_frontend_init(C.byref(fh), C.byref(fd), C.c_void_p(fws), fb, st) == 0
+    raw = torch.from_numpy(workloads.frontend_strain(5, D, 8 * 1024 * 12)).cuda()
+    _, p_fo = guarded(D * 1024 * 4)
+    _, p_ps = guarded(D * 1025 * 4, align=16)
+    for c in range(12):
+        rc_ = raw[:, c * 8192:(c + 1) * 8192].contiguous()
+        assert L_.spiir_frontend_chunk(fh, C.c_void_p(rc_.data_ptr()), C.c_void_p(p_fo), C.c_void_p(p_ps), st) == 0
+    torch.cuda.synchronize()
+    # ... and every buffer was written to (the pattern is gone from its interior), none beyond its ends
+    for raw_t, off, nbytes in guards:
+        assert not bool((raw_t[off:off + nbytes] == 0xA5).all())
+        lo, hi = raw_t[:off], raw_t[off + nbytes:]
+        assert bool((lo == 0xA5).all()) and bool((hi == 0xA5).all()), "a guard band was overwritten (buffer of %d bytes)" % nbytes
+    for ph in plans:
+        L_.spiir_sky_plan_free(ph)
+    L_.spiir_frontend_free(fh)
+    L_.spiir_bank_free(h)
