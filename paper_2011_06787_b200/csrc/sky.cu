@@ -42,19 +42,25 @@ constexpr int kSkyKMax = 4;                 // (trigger, slide) pairs per thread
 template <int D> struct SkyFmt {
   static constexpr int NO = D - 1;                       // detectors other than the trigger detector
   static constexpr int NQ = D * (D + 1) / 2;             // independent entries of the projector
-  static constexpr int SW = (NQ + 2 + 3) / 4 * 4;        // words per slot: NQ weights + pixel + control, padded to 16 B
+  static constexpr int SW = (NQ + 1 + 3) / 4 * 4;        // words per slot: NQ - 1 weights + control + pixel, padded to 16 B
 };
-// One slot per direction, SW words: words [0,NQ) weights, word NQ = pixel, word NQ+1 = control.
-//   Weight order (T = trigger detector, o = others in increasing detector index): M_TT; M_oo (o = 0..NO-1);
-//   2 M_To; 2 M_o'o for o' < o, (0,1) (0,2) (1,2).
+// One slot per direction, SW words: words [0, NQ-1) weights, word NQ-1 = control, word NQ = pixel.
+//   The weight of |z_T|^2 is not stored: the projector has trace 2, so M_TT = 2 - sum_o M_oo and the kernel evaluates
+//   rho_c^2 - 2 |z_T|^2 = sum_o M_oo (|z_o|^2 - |z_T|^2) + cross terms.  Weight order (T = trigger detector, o = others
+//   in increasing detector index): M_oo (o = 0..NO-1); 2 M_To; 2 M_o'o for o' < o, (0,1) (0,2) (1,2).
+//   Weights and control come first so that the main loop reads NQ words per slot — for three detectors one LDS.128 and
+//   one LDS.64 (3 shared-memory wavefronts per warp instead of 4: the broadcast reads of the slot are half of the
+//   kernel's shared-memory traffic, which co-limits it with the FP32 pipe; profiles/r2_ncu_summary.md section 2).
 //   control = nref | f_0 << 2 | f_1 << 12 | f_2 << 22: f_o = element offset, inside a pair's block of
 //   windows, of the sample of other detector o this direction reads (segment offset + row, < 1024);
 //   nref = NO - (first other detector whose row differs from the previous slot): the last nref
 //   detectors are refreshed (NO for the first slot of a warp's share of the stream: refresh
 //   everything; 0: same delay tuple, nothing to refresh — one bit test on the common path).
 // The last chunk is padded with copies of the last direction (nref 0).
+
 struct SkyParams {
-  const float* stream; int32_t n_chunks, chunks_per_warp;     // this trigger detector's stream; contiguous share per warp
+  const float* stream; int32_t n_chunks;                      // this trigger detector's stream
+  int16_t cb[kSkyWarps + 1];                                  // chunks [cb[w], cb[w+1]) are warp w's share (balanced by cost)
   int32_t n_pix;
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
   const spiir_trigger* trig;
@@ -74,9 +80,9 @@ struct PairInfo { int32_t slot, slide, valid, row; float2 vT; long long k; unsig
 
 template <int NQ>
 __device__ __forceinline__ float quad_form(const float* __restrict__ w, const float (&q)[NQ]) {
-  float c = __fmul_rn(w[1], q[1]);                     // the term of q[0] = |z_T|^2 is the constant 2 q[0] (trace of the projector)
+  float c = __fmul_rn(w[0], q[1]);                     // the term of q[0] = |z_T|^2 is the constant 2 q[0] (trace of the projector)
 #pragma unroll
-  for (int e = 2; e < NQ; ++e) c = __fmaf_rn(w[e], q[e], c);
+  for (int e = 2; e < NQ; ++e) c = __fmaf_rn(w[e - 1], q[e], c);
   return c;
 }
 
@@ -100,7 +106,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
   const int64_t kmin = (P.k_newest - P.ring_len + 1 > 0) ? P.k_newest - P.ring_len + 1 : 0;
   float* mytile = tiles + warp * kTileWords;
   // a contiguous share of chunks per warp: only a share's first slot has to refresh everything
-  const int c_beg = min(P.n_chunks, warp * P.chunks_per_warp), c_end = min(P.n_chunks, c_beg + P.chunks_per_warp);
+  const int c_beg = P.cb[warp], c_end = P.cb[warp + 1];
 
   __shared__ uint64_t bar;                             // completion of a batch's TMA window copies
   if (tid == 0) {
@@ -255,20 +261,28 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c) pre[c] = __ldg(src + c);
       }
-      float4 nxt[SW / 4];
+      // words of a slot the loop needs: NQ - 1 weights and the control word (and the pixel for the sky map), read as
+      // N4 float4 and, when two words or fewer remain, one float2
+      constexpr int LW = NQ + (MAP ? 1 : 0);
+      constexpr bool H2 = (LW % 4 == 1 || LW % 4 == 2);
+      constexpr int N4 = H2 ? LW / 4 : (LW + 3) / 4;
+      float4 nxt[N4 > 0 ? N4 : 1]; float2 nxt2 = make_float2(0.f, 0.f);
 #pragma unroll
-      for (int c = 0; c < SW / 4; ++c) nxt[c] = reinterpret_cast<const float4*>(mytile)[c];
+      for (int c = 0; c < N4; ++c) nxt[c] = reinterpret_cast<const float4*>(mytile)[c];
+      if (H2) nxt2 = reinterpret_cast<const float2*>(mytile)[2 * N4];
       float pend[K];
 #pragma unroll 4
       for (int s = 0; s < kSkyChunk; ++s) {
-        float w[SW];
+        float w[SW + 2];
 #pragma unroll
-        for (int c = 0; c < SW / 4; ++c) { w[4 * c] = nxt[c].x; w[4 * c + 1] = nxt[c].y; w[4 * c + 2] = nxt[c].z; w[4 * c + 3] = nxt[c].w; }
+        for (int c = 0; c < N4; ++c) { w[4 * c] = nxt[c].x; w[4 * c + 1] = nxt[c].y; w[4 * c + 2] = nxt[c].z; w[4 * c + 3] = nxt[c].w; }
+        if (H2) { w[4 * N4] = nxt2.x; w[4 * N4 + 1] = nxt2.y; }
         // the next slot is fetched (broadcast read) before this one is consumed
+        const float* nslot = mytile + ((s + 1) & (kSkyChunk - 1)) * SW;
 #pragma unroll
-        for (int c = 0; c < SW / 4; ++c)
-          nxt[c] = reinterpret_cast<const float4*>(mytile + ((s + 1) & (kSkyChunk - 1)) * SW)[c];
-        const int ctrl = __float_as_int(w[NQ + 1]);
+        for (int c = 0; c < N4; ++c) nxt[c] = reinterpret_cast<const float4*>(nslot)[c];
+        if (H2) nxt2 = reinterpret_cast<const float2*>(nslot)[2 * N4];
+        const int ctrl = __float_as_int(w[NQ - 1]);
         const int nref = ctrl & 3;
         if (nref) {
           // new delay tuple: gather the rows that changed, refresh the products they enter
@@ -294,15 +308,15 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         float cval[K];
 #pragma unroll
         for (int i = 0; i < K / 2; ++i) {
-          float2 c2 = __fmul2_rn(make_float2(w[1], w[1]), qp[i][1]);
+          float2 c2 = __fmul2_rn(make_float2(w[0], w[0]), qp[i][1]);
 #pragma unroll
-          for (int e = 2; e < NQ; ++e) c2 = __ffma2_rn(make_float2(w[e], w[e]), qp[i][e], c2);
+          for (int e = 2; e < NQ; ++e) c2 = __ffma2_rn(make_float2(w[e - 1], w[e - 1]), qp[i][e], c2);
           cval[2 * i] = c2.x; cval[2 * i + 1] = c2.y;
         }
         if (K & 1) {
-          float c = __fmul_rn(w[1], qp[K / 2][1].x);
+          float c = __fmul_rn(w[0], qp[K / 2][1].x);
 #pragma unroll
-          for (int e = 2; e < NQ; ++e) c = __fmaf_rn(w[e], qp[K / 2][e].x, c);
+          for (int e = 2; e < NQ; ++e) c = __fmaf_rn(w[e - 1], qp[K / 2][e].x, c);
           cval[K - 1] = c;
         }
 #pragma unroll
@@ -364,7 +378,7 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
         for (int c = 0; c < SW / 4; ++c) {
           w[4 * c] = wv4[u][c].x; w[4 * c + 1] = wv4[u][c].y; w[4 * c + 2] = wv4[u][c].z; w[4 * c + 3] = wv4[u][c].w;
         }
-        const int ctrl = __float_as_int(w[NQ + 1]);
+        const int ctrl = __float_as_int(w[NQ - 1]);
         float qq[NQ]; float2 vv[NO];
         qq[0] = re_prod(pi.vT, pi.vT);
         float tot = qq[0];
@@ -425,7 +439,7 @@ __global__ void __launch_bounds__(256) k_sky_bin(const spiir_trigger* trig, int 
 using namespace spiir;
 
 static size_t sky_align(size_t x) { return (x + 255) / 256 * 256; }
-static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 2 + 3) / 4 * 4; }
+static int sky_slot_words(int D) { return (D * (D + 1) / 2 + 1 + 3) / 4 * 4; }
 static int sky_win_elems(int ps, int K) { return ps * 32 * K; }          // ps is even
 static size_t sky_smem_bytes(int ps, int SW, int K) {
   const int NP = 32 * K, tile = std::max(kSkyChunk * SW, 2 * NP);
@@ -466,50 +480,73 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
       if (rows[(size_t)x * 3 + o] != rows[(size_t)y * 3 + o]) return rows[(size_t)x * 3 + o] < rows[(size_t)y * 3 + o];
     return x < y;
   });
-  const int cpw = (pl->cap_slots / kSkyChunk + kSkyWarps - 1) / kSkyWarps;   // chunks per warp
-  slots.assign((size_t)pl->cap_slots * SW, 0.f);
+  // how many of the other detectors' rows each slot refreshes (the last ones), before the warps' shares are cut
+  const int n_chunks = pl->cap_slots / kSkyChunk;
+  std::vector<int> nrf(pl->cap_slots, 0);
   S.n_tuples = 0;
+  for (int r = 0; r < n_pix; ++r) {
+    int level = 0;
+    if (r > 0) {
+      const int32_t* pr = &rows[(size_t)order[r - 1] * 3];
+      const int32_t* rw = &rows[(size_t)order[r] * 3];
+      while (level < NO && pr[level] == rw[level]) ++level;
+    }
+    nrf[r] = NO - level;
+    if (nrf[r]) ++S.n_tuples;
+  }
+  // the 16 warps take contiguous runs of chunks of about equal COST (a refreshed row costs about as much as one
+  // direction and a half): the warps whose share is dense in delay tuples no longer finish last
+  {
+    std::vector<double> cost(n_chunks, 0.0);
+    double total = 0;
+    for (int c = 0; c < n_chunks; ++c) {
+      double x = kSkyChunk;
+      for (int r = c * kSkyChunk; r < (c + 1) * kSkyChunk; ++r) x += 1.5 * nrf[r];
+      cost[c] = x; total += x;
+    }
+    double acc = 0; int wv = 1;
+    S.cb[0] = 0;
+    for (int c = 0; c < n_chunks && wv < kSkyWarps; ++c) {
+      acc += cost[c];
+      if (acc >= total * wv / kSkyWarps) S.cb[wv++] = (int16_t)(c + 1);
+    }
+    for (; wv <= kSkyWarps; ++wv) S.cb[wv] = (int16_t)n_chunks;
+  }
+  slots.assign((size_t)pl->cap_slots * SW, 0.f);
   for (int r = 0; r < pl->cap_slots; ++r) {
     float* w = &slots[(size_t)r * SW];
     if (r >= n_pix) {                      // padding: the last direction again, nothing to refresh
       memcpy(w, w - SW, (size_t)SW * 4);
-      int32_t ctrl; memcpy(&ctrl, w + NQ + 1, 4);
+      int32_t ctrl; memcpy(&ctrl, w + NQ - 1, 4);
       ctrl &= ~3;
-      memcpy(w + NQ + 1, &ctrl, 4);
+      memcpy(w + NQ - 1, &ctrl, 4);
       continue;
     }
     const int p = order[r];
     const int32_t* rw = &rows[(size_t)p * 3];
-    int level = 0;
-    if (r > 0) {
-      const int32_t* pr = &rows[(size_t)order[r - 1] * 3];
-      while (level < NO && pr[level] == rw[level]) ++level;
-      if (level < NO) ++S.n_tuples;
-    } else {
-      ++S.n_tuples;
-    }
-    if (r % (kSkyChunk * cpw) == 0) level = 0;   // a warp's share of the stream starts from nothing
+    int nref = nrf[r];
+    for (int wv = 0; wv < kSkyWarps; ++wv)
+      if (r == S.cb[wv] * kSkyChunk) nref = NO;   // a warp's share of the stream starts from nothing
     const float* u = u2 + (size_t)p * D * 2;
     auto M = [&](int I, int J) { return (double)u[2 * I] * u[2 * J] + (double)u[2 * I + 1] * u[2 * J + 1]; };
-    // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order
+    // projector U2 U2^T in float64 from the float32 table, rounded once, in the kernel's order.
     // U2 has orthonormal columns (Eq. 27: the left singular vectors), so the projector has trace 2 and
     // M_TT = 2 - sum_o M_oo: the kernel evaluates rho_c^2 - 2 |z_T|^2 = sum_o M_oo (|z_o|^2 - |z_T|^2) + cross terms,
     // one multiply-add fewer per direction, and adds the constant back at the end
-    w[0] = 0.f;
     {
       double tr = M(T, T);
       for (int o = 0; o < NO; ++o) tr += M(oth[o], oth[o]);
       if (!(tr > 2.0 - 1e-4 && tr < 2.0 + 1e-4)) S.bad_trace = 1;
     }
-    for (int o = 0; o < NO; ++o) w[1 + o] = (float)M(oth[o], oth[o]);
-    for (int o = 0; o < NO; ++o) w[1 + NO + o] = (float)(2.0 * M(T, oth[o]));
+    for (int o = 0; o < NO; ++o) w[o] = (float)M(oth[o], oth[o]);
+    for (int o = 0; o < NO; ++o) w[NO + o] = (float)(2.0 * M(T, oth[o]));
     for (int o = 1; o < NO; ++o)
-      for (int o2 = 0; o2 < o; ++o2) w[1 + 2 * NO + o * (o - 1) / 2 + o2] = (float)(2.0 * M(oth[o2], oth[o]));
+      for (int o2 = 0; o2 < o; ++o2) w[2 * NO + o * (o - 1) / 2 + o2] = (float)(2.0 * M(oth[o2], oth[o]));
+    int32_t ctrl = nref;                   // how many of the other detectors' rows to refresh, the last ones
+    for (int o = 0; o < NO; ++o) ctrl |= rw[o] << (2 + kSkyRowBits * o);
+    memcpy(w + NQ - 1, &ctrl, 4);
     const int32_t pix = p;
     memcpy(w + NQ, &pix, 4);
-    int32_t ctrl = NO - level;             // how many of the other detectors' rows to refresh, the last ones
-    for (int o = 0; o < NO; ++o) ctrl |= rw[o] << (2 + kSkyRowBits * o);
-    memcpy(w + NQ + 1, &ctrl, 4);
   }
   S.n_chunks = pl->cap_slots / kSkyChunk;
 }
@@ -678,7 +715,7 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
     SkyParams P;
     memset(&P, 0, sizeof(P));
     P.stream = (const float*)(pl->ws + S.off_slots); P.n_chunks = S.n_chunks;
-    P.chunks_per_warp = (S.n_chunks + kSkyWarps - 1) / kSkyWarps;
+    for (int wv = 0; wv <= kSkyWarps; ++wv) P.cb[wv] = S.cb[wv];
     P.n_pix = pl->n_pix;
     P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;
     P.ring_len = view->ring_len; P.k_newest = view->k_newest;
