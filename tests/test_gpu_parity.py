@@ -1263,3 +1263,59 @@ def test_workspace_guard_bands(sp, U):
         L_.spiir_sky_plan_free(ph)
     L_.spiir_frontend_free(fh)
     L_.spiir_bank_free(h)
+
+
+# ------------------------------------------------------------------ the N > 1 path on the CUDA side (one GPU available)
+def test_template_shards_on_the_cuda_path(sp, U):
+    """The multi-GPU path shards by template with no exchange step.  Only one
+    GPU is available, and ranks must not be emulated as concurrent processes on it, so the two ranks' shards are run
+    one after the other through the C ABI: each rank's sub-bank (shard.template_shard / slice_bank, whole banks of
+    `bank_size`) must reproduce its rows of the unsharded run — SNR to float32 rounding, peaks, sky results of its
+    candidates — and the merged trigger lists must cover the unsharded list (the world-size-2 gloo test covers the
+    host-side merge and timing reductions)."""
+    import torch
+    from paper_2011_06787_b200 import shard as shd
+    cfg = workloads.config(2)
+    T, D, NC, bs = 24, 3, 3, 4
+    bank = workloads.bank_for_config(2, n_templates=T)
+    dec, itp = workloads.halfband_taps()
+    x = workloads.gaussian_strain(np.random.default_rng(9), D, NC * 4096)
+    u2, delay = _table(workloads.config(1), nside=8, gmst=0.2)
+
+    def run(b):
+        z, trigs, bk = U.run_bank(b, x, 4096, ring_len=NC * 2048, bank_size=bs, taps=(dec, itp), peak_thr=2.0)
+        plan = sp.SkyPlan(u2, delay, max_slots=D * b["n_templates"])
+        prev = sp.triggers_from_numpy(trigs[NC - 2][0])
+        res = sp.results_to_numpy(plan.search(bk.snr_view(), prev, D * b["n_templates"]))
+        torch.cuda.synchronize()
+        return z, trigs, res
+
+    z_full, trig_full, res_full = run(bank)
+    merged = []
+    for rank in range(2):
+        t0, t1 = shd.template_shard(rank, 2, T, bank_size=bs)
+        assert (t0, t1) == ((0, 12), (12, 24))[rank]
+        z, trigs, res = run(shd.slice_bank(bank, t0, t1))
+        # a shard is an exact sub-problem: the same filters, states and inputs; only the order in which a template's
+        # filters are summed may differ (the lane layout is planned per bank), i.e. float32 rounding
+        assert np.abs(z - z_full[:, t0:t1]).max() <= 2e-6
+        rows = (np.arange(D)[:, None] * T + np.arange(t0, t1)[None, :]).reshape(-1)
+        for c in range(NC):
+            tf, ts = trig_full[c][0][rows], trigs[c][0]
+            same = tf["k"] == ts["k"]
+            assert same.mean() >= 0.97                                       # (near-ties of the maximum, A12)
+            assert np.array_equal(tf["valid"][same], ts["valid"][same]) and np.array_equal(tf["det"], ts["det"])
+            assert np.array_equal(tf["tmpl"], ts["tmpl"] + t0)
+            assert np.all(np.abs(tf["snr"][same] - ts["snr"][same]) <= 2e-6)
+        tf, ts = trig_full[NC - 2][0][rows], trigs[NC - 2][0]
+        ok = (tf["k"] == ts["k"]) & (tf["valid"] == 1) & (ts["valid"] == 1)
+        assert ok.sum() >= 10 and np.array_equal(res_full[rows]["pix"][ok] >= 0, res["pix"][ok] >= 0)
+        hit = ok & (res["pix"] >= 0)
+        assert np.all(np.abs(res_full[rows]["coh2"][hit] - res["coh2"][hit]) <= 1e-5 * res["coh2"][hit])
+        merged.append(shd.merge_triggers(trigs[NC - 1][0], t0))              # single process: the rank's own list, global indices
+    allm = np.concatenate(merged)
+    full = trig_full[NC - 1][0]
+    full = full[full["valid"] == 1]
+    assert abs(len(allm) - len(full)) <= 2
+    common = set(zip(allm["det"], allm["tmpl"], allm["k"])) & set(zip(full["det"], full["tmpl"], full["k"]))
+    assert len(common) >= 0.97 * len(full)
