@@ -187,7 +187,10 @@ int spiir_sky_table_nearest(double t_s, double t0_s, double interval_s, int32_t 
  *   k = factor * H, det / z / snr kept; valid = 0 (and an all-zero window) when
  *   the slot is empty or k - H - 1 .. k + H + 1 is not inside the view.
  *   *out_view describes dev_out (rows = slots).  factor 1..16; H must cover the
- *   largest inter-detector delay in input samples.  dev_out: 16-byte aligned,
+ *   largest inter-detector delay in input samples.  (The search on the windows needs
+ *   the factor-times wider delay windows of at least 32 candidates in shared memory:
+ *   for H1-L1-V1 at 2048 Hz that holds up to factor 3, 4 when the trigger is not in
+ *   V1; spiir_sky_plan_init reports a table that does not fit as EINVAL.)  dev_out: 16-byte aligned,
  *   spiir_snr_upsample_elems() complex elements, caller-owned.  Asynchronous on
  *   `stream`.  Errors: EINVAL, ECUDA. */
 int spiir_snr_upsample_elems(int32_t n_det, int32_t n_slots, int32_t factor, int32_t half_width, size_t* elems);
