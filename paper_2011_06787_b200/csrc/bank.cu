@@ -113,18 +113,27 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
     }
     choose_shape(cnt, &hb.G, &hb.F);
     const int G = hb.G, F = hb.F, cap_unit = G * F, upw = 32 / G;
-    hb.Hcap = std::max(32, round_up(d->max_delay[b], 4));
-    const int nsubmax = std::min(hb.nmax, kSubChunkMax);
+    const int odd = (b == 0 && d->out_band == 1) ? 1 : 0;      // the band above the output rate: two samples per step
+    // That band's launch is bound by shared-memory bandwidth, a third of it bank conflicts between the 8 lanes of an
+    // LDS.128 phase (profiles/r2_ncu_summary.md section 3): it gets 8 shifted replicas instead of 4, so that every filter
+    // has TWO aligned places to read its samples from (replica al or al + 4: a different 16-byte bank group) and the
+    // placement below can balance the groups; the staged sub-chunk shrinks to 1024 samples to keep two CTAs per SM.
+    hb.nrep = odd ? kReplicas2 : kReplicas;
+    hb.pad = odd ? 4 : 0;
+    hb.Hcap = std::max(32, round_up(d->max_delay[b], 4)) + hb.pad;
+    int nsubmax = std::min(hb.nmax, kSubChunkMax);
+    if (hb.nrep == kReplicas2) nsubmax = std::min(nsubmax, 1024);
+    hb.nsubmax = nsubmax;
     // shared history depth: the deepest template that still fits the shared-memory budget;
     // templates beyond it (chirp-matched ones) read their input from L1/L2
     {
-      const int budget = (kSmemFloatsMax - nsubmax) / 4 * 4;
+      const int budget = (kSmemFloatsMax * kReplicas / hb.nrep - nsubmax - hb.pad) / 4 * 4;
       int h = 0;
       for (int t = 0; t < T; ++t) if (cnt[t] && maxd[t] <= budget) h = std::max(h, maxd[t]);
-      hb.Hs = std::min(std::max(round_up(h, 4), 4), hb.Hcap);
+      hb.Hs = std::min(std::max(round_up(h, 4), 4), hb.Hcap - hb.pad);
     }
     hb.cap = round_up(hb.Hcap + hb.nmax + 4, 32);
-    hb.reps = hb.Hs + nsubmax;
+    hb.reps = hb.pad + hb.Hs + nsubmax;
     // units: short classes first
     std::vector<int> first(T, 0), nun(T, 0);
     int nus = 0, nul = 0;
@@ -142,7 +151,6 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
     hb.n_wu_long = nul_pad / upw;
     const size_t slots = (size_t)hb.n_units * cap_unit;
     hb.off_coef = take(slots * sizeof(float4));
-    const int odd = (b == 0 && d->out_band == 1) ? 1 : 0;      // the band above the output rate: two samples per step
     if (odd) hb.off_coef2 = take(slots * sizeof(float2));
     hb.off_off = take(slots * sizeof(int32_t));
     // launch groups, one per (G, F); the long-delay CTAs of a group are listed first (they start first
@@ -163,7 +171,7 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
         add.push_back(CtaWork{b, wu0 + w, wu0 + std::min(nwu, w + kBankWarps), cls});
       if (cls) g.work.insert(g.work.begin(), add.begin(), add.end());
       else     g.work.insert(g.work.end(), add.begin(), add.end());
-      if (!cls) g.smem_bytes = std::max(g.smem_bytes, kReplicas * hb.reps * 4 + 16);
+      if (!cls) g.smem_bytes = std::max(g.smem_bytes, hb.nrep * hb.reps * 4 + 16);
     }
     if (img) {
       img->coef[b].assign(slots, make_float4(0.f, 0.f, 0.f, 0.f));
@@ -178,22 +186,27 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
         img->tb_count[(size_t)t * B + b] = nun[t];
         if (!cnt[t]) continue;
         const bool lng = maxd[t] > hb.Hs;
-        order.clear();
-        for (int64_t l : ids[t]) {
+        // where a filter may read its samples: `off` = float offset of its first sample in the staged replica set (or,
+        // for the long-delay class, in the global one), and the 16-byte bank group it starts in.  With 8 replicas a
+        // filter has two choices (replica al or al + 4).
+        const bool two = !lng && hb.nrep == kReplicas2;
+        auto choice = [&](int64_t l, int which, int* off_out) {
           const int dl = d->host_delay[l];
-          const int e = (lng ? hb.Hcap : hb.Hs) - dl;
-          const int al = e & 3;
-          const int off = al * (lng ? hb.cap : hb.reps) + (e - al);
-          order.push_back({((off >> 2) & 7), l});
-          (void)off;
-        }
+          const int e = lng ? hb.Hcap - dl : hb.pad + hb.Hs - dl;
+          const int r = (e & 3) + 4 * which;
+          const int off = r * (lng ? hb.cap : hb.reps) + (e - r);
+          if (off_out) *off_out = off;
+          return (off >> 2) & 7;
+        };
+        order.clear();
+        for (int64_t l : ids[t]) order.push_back({choice(l, 0, nullptr), l});
         // Place the filters on the phase-rows (8 lanes x one LDS.128 = one shared-memory wavefront when
         // the 8 addresses fall in 8 different 16-byte bank groups).  A row costs as many wavefronts as its
-        // most frequent group, so the total cannot go below the size of the template's largest group;
-        // dealing class by class, largest first, each filter to the row where it raises that maximum
-        // least, lands the surplus of every oversubscribed group in the same rows (on uniformly random
-        // groups 1.44 wavefronts per row against 1.64 for a plain round-robin, bound 1.42; measured on
-        // config 4: bank conflicts of the band-0 launch 4.7e8 -> 3.7e8, 5.06 -> 5.01 ms).
+        // most frequent group, so with one choice per filter the total cannot go below the size of the template's
+        // largest group; dealing class by class, largest first, each filter to the row (and, with two replicas to
+        // choose from, the replica) where it raises that maximum least, lands the surplus of every oversubscribed
+        // group in the same rows (one choice, uniformly random groups: 1.44 wavefronts per row against 1.64 for a plain
+        // round-robin, bound 1.42; measured on config 4: bank conflicts of the band-0 launch 4.7e8 -> 3.7e8).
         std::stable_sort(order.begin(), order.end(),
                          [](const std::pair<int, int64_t>& x, const std::pair<int, int64_t>& y) { return x.first < y.first; });
         const int PR = nun[t] * prpu;
@@ -205,19 +218,75 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
         std::stable_sort(corder, corder + 8, [&](int x, int y) { return ccnt[x] > ccnt[y]; });
         row_fill.assign(PR, 0); row_max.assign(PR, 0); row_cls.assign((size_t)PR * 8, 0);
         place.assign(order.size(), std::pair<int, int>(0, 0));
+        std::vector<int> which_of(order.size(), 0);
+        if (two) {
+          // Two choices per filter: first balance the GROUPS — every filter takes one of its two bank groups so that no
+          // group holds more filters than there are rows (PR); then a group's filters go to distinct rows, and a row (8
+          // lanes, 8 groups) never sees a group twice: no conflict at all when the balance exists.  The balance is a
+          // tiny flow problem (8 groups): start from the less loaded choice, then move filters along augmenting paths
+          // from overfull groups to groups with room.
+          const int nf = (int)order.size();
+          std::vector<int> g0(nf), g1(nf), cur(nf);
+          int load[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+          for (int j = 0; j < nf; ++j) {
+            g0[j] = order[j].first; g1[j] = choice(order[j].second, 1, nullptr);
+            which_of[j] = load[g1[j]] < load[g0[j]] ? 1 : 0;
+            cur[j] = which_of[j] ? g1[j] : g0[j];
+            ++load[cur[j]];
+          }
+          for (int guard = 0; guard < 8 * nf; ++guard) {
+            int over = -1;
+            for (int g = 0; g < 8; ++g) if (load[g] > PR && (over < 0 || load[g] > load[over])) over = g;
+            if (over < 0) break;
+            // breadth-first search over groups from `over` to any group with room, along filters that can switch
+            int prev_f[8], seen[8] = {0, 0, 0, 0, 0, 0, 0, 0}, queue[8], qh = 0, qt = 0, target = -1;
+            queue[qt++] = over; seen[over] = 1; prev_f[over] = -1;
+            while (qh < qt && target < 0) {
+              const int g = queue[qh++];
+              for (int j = 0; j < nf && target < 0; ++j) {
+                if (cur[j] != g) continue;
+                const int h = which_of[j] ? g0[j] : g1[j];
+                if (seen[h]) continue;
+                seen[h] = 1; prev_f[h] = j; queue[qt++] = h;
+                if (load[h] < PR) target = h;
+              }
+            }
+            if (target < 0) break;                                    // no balance exists: the surplus stays (conflicts)
+            for (int h = target; prev_f[h] >= 0;) {                   // switch the filters on the path, back to front
+              const int j = prev_f[h], g = cur[j];
+              which_of[j] ^= 1; cur[j] = h; ++load[h]; --load[g];
+              h = g;
+            }
+          }
+          // rows: a group's filters to distinct rows, emptiest rows first; a surplus beyond PR wraps around
+          for (int g = 0; g < 8; ++g) {
+            std::vector<int> rows_by_fill(PR);
+            for (int r = 0; r < PR; ++r) rows_by_fill[r] = r;
+            std::stable_sort(rows_by_fill.begin(), rows_by_fill.end(), [&](int x, int y) { return row_fill[x] < row_fill[y]; });
+            int k = 0;
+            for (int j = 0; j < nf; ++j) {
+              if (cur[j] != g) continue;
+              int r = rows_by_fill[k % PR];
+              for (int tries = 0; row_fill[r] >= 8 && tries < PR; ++tries) r = rows_by_fill[(++k) % PR];
+              place[j] = std::pair<int, int>(r, row_fill[r]);
+              ++row_fill[r];
+              ++k;
+            }
+          }
+        } else
         for (int ci = 0; ci < 8; ++ci) {
-          const int c = corder[ci];
-          for (int j = cbeg[c]; j < cbeg[c + 1]; ++j) {
+          const int c0 = corder[ci];
+          for (int j = cbeg[c0]; j < cbeg[c0 + 1]; ++j) {
             int best = -1; long best_key = 0;
             for (int r = 0; r < PR; ++r) {
               if (row_fill[r] >= 8) continue;
-              const int have = row_cls[(size_t)r * 8 + c];
+              const int have = row_cls[(size_t)r * 8 + c0];
               const long key = ((long)std::max(0, have + 1 - row_max[r]) << 40) | ((long)have << 20) | (long)row_fill[r];
               if (best < 0 || key < best_key) { best = r; best_key = key; }
             }
             place[j] = std::pair<int, int>(best, row_fill[best]);
             ++row_fill[best];
-            row_max[best] = std::max(row_max[best], ++row_cls[(size_t)best * 8 + c]);
+            row_max[best] = std::max(row_max[best], ++row_cls[(size_t)best * 8 + c0]);
           }
         }
         for (size_t j = 0; j < order.size(); ++j) {
@@ -227,9 +296,6 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
           const int unit = first[t] + ul, g8 = half * 8 + pos;
           const int wu = unit / upw, lane = (unit % upw) * G + g8;
           const size_t slot = ((size_t)wu * F + f) * 32 + lane;
-          const int dl = d->host_delay[l];
-          const int e = (lng ? hb.Hcap : hb.Hs) - dl;
-          const int al = e & 3;
           img->coef[b][slot] = make_float4(d->host_a[l].re, d->host_a[l].im, d->host_b[l].re, d->host_b[l].im);
           if (odd) {                                           // a^2 and a b in float64 from the float32 a, b, rounded once
             const double ar = d->host_a[l].re, ai = d->host_a[l].im, br = d->host_b[l].re, bi = d->host_b[l].im;
@@ -237,7 +303,9 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
             img->coef[b][slot].y = (float)(2.0 * ar * ai);
             img->coef2[b][slot] = make_float2((float)(ar * br - ai * bi), (float)(ar * bi + ai * br));
           }
-          img->off[b][slot] = al * (lng ? hb.cap : hb.reps) + (e - al);
+          int off = 0;
+          choice(l, which_of[j], &off);
+          img->off[b][slot] = off;
         }
       }
     }
@@ -248,8 +316,8 @@ static int plan(const spiir_bank_desc* d, spiir_bank* bk, PlanImages* img) {
     spiir_bank_host_band& hb = bk->band[b];
     const size_t slots = (size_t)hb.n_units * hb.G * hb.F;
     hb.off_state = take((size_t)D * slots * sizeof(float2));
-    hb.off_x[0] = take((size_t)D * kReplicas * hb.cap * sizeof(float));
-    hb.off_x[1] = take((size_t)D * kReplicas * hb.cap * sizeof(float));
+    hb.off_x[0] = take((size_t)D * hb.nrep * hb.cap * sizeof(float));
+    hb.off_x[1] = take((size_t)D * hb.nrep * hb.cap * sizeof(float));
     hb.off_uphist = take((size_t)D * T * kUpHist * sizeof(float2));
   }
   bk->off_peak = take((size_t)D * T * sizeof(PeakRec));
@@ -418,7 +486,8 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     const int n = n_samples >> b;
     pp.xnew[b] = (float*)(bk->ws + hb.off_x[newp]);
     pp.xold[b] = (const float*)(bk->ws + hb.off_x[bk->parity]);
-    pp.x_det_stride[b] = (int64_t)kReplicas * hb.cap;
+    pp.x_det_stride[b] = (int64_t)hb.nrep * hb.cap;
+    pp.nrep[b] = hb.nrep;
     pp.cap[b] = hb.cap; pp.Hcap[b] = hb.Hcap; pp.n[b] = n; pp.prev_n[b] = hb.prev_n;
     BandDev& bd = P.band[b];
     const size_t slots = (size_t)hb.n_units * hb.G * hb.F;
@@ -432,7 +501,8 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     bd.state_det_stride = (int64_t)slots;
     bd.S_det_stride = (int64_t)hb.n_units * hb.nmax;
     bd.n = n; bd.nmax = hb.nmax; bd.Hcap = hb.Hcap; bd.Hs = hb.Hs; bd.cap = hb.cap; bd.reps = hb.reps;
-    bd.nsub = std::min(n, std::min(hb.nmax, kSubChunkMax));
+    bd.nsub = std::min(n, hb.nsubmax);
+    bd.nrep = hb.nrep; bd.pad = hb.pad;
     bd.odd = (b == 0 && d.out_band == 1) ? 1 : 0;
   }
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -530,7 +600,7 @@ int spiir_bank_band_plan(const spiir_bank* bk, int32_t band, spiir_band_plan* p)
   const auto& hb = bk->band[band];
   p->lanes_per_unit = hb.G; p->filters_per_lane = hb.F;
   p->n_units = hb.n_units; p->n_units_long = hb.n_units_long;
-  p->smem_history = hb.Hs; p->smem_bytes = kReplicas * hb.reps * 4 + 16;
+  p->smem_history = hb.Hs; p->smem_bytes = hb.nrep * hb.reps * 4 + 16;
   p->n_filters = hb.n_filters; p->n_slots = (int64_t)hb.n_units * hb.G * hb.F;
   return SPIIR_OK;
 }

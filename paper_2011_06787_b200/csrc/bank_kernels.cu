@@ -89,11 +89,10 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepParams p) {
       }
     }
     __syncthreads();
-    // (c) replicas r = 1..3: rep_r[j] = rep_0[j + r]  (aligned float4 reads for any delay)
-    const int tot = H + n;
+    // (c) replicas r = 1..nrep-1: rep_r[j] = rep_0[j + r]  (aligned float4 reads for any delay)
+    const int tot = H + n, nrep = p.nrep[b];
     for (int j = tid; j < tot; j += kPrepThreads) {
-#pragma unroll
-      for (int r = 1; r < kReplicas; ++r) xn[(size_t)r * cap + j] = (j + r < tot) ? xn[j + r] : 0.f;
+      for (int r = 1; r < nrep; ++r) xn[(size_t)r * cap + j] = (j + r < tot) ? xn[j + r] : 0.f;
     }
   }
 }
@@ -358,19 +357,18 @@ k_bank(const __grid_constant__ BankParams P, const CtaWork* __restrict__ work) {
       run_samples<G, F, true, ODD>(r, x, n, Sout, lane, g);
     }
   } else {
-    uint64_t* bar = reinterpret_cast<uint64_t*>(xs + kReplicas * B.reps);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(xs + B.nrep * B.reps);
     if (threadIdx.x == 0) mbar_init(bar, 1);
     __syncthreads();
     uint32_t phase = 0;
-    const float* src0 = B.xrep + (size_t)det * B.x_det_stride + (B.Hcap - B.Hs);
+    const float* src0 = B.xrep + (size_t)det * B.x_det_stride + (B.Hcap - B.Hs - B.pad);
     for (int m0 = 0; m0 < n; m0 += B.nsub) {
       const int len = min(B.nsub, n - m0);
       if (m0 > 0) __syncthreads();                   // every warp finished reading the previous window
       if (threadIdx.x == 0) {
-        const uint32_t bytes = (uint32_t)(B.Hs + len) * 4u;
-        mbar_expect_tx(bar, bytes * kReplicas);
-#pragma unroll
-        for (int rep = 0; rep < kReplicas; ++rep)
+        const uint32_t bytes = (uint32_t)(B.pad + B.Hs + len) * 4u;
+        mbar_expect_tx(bar, bytes * B.nrep);
+        for (int rep = 0; rep < B.nrep; ++rep)
           tma_load_1d(xs + rep * B.reps, src0 + (size_t)rep * B.cap + m0, bytes, bar);
       }
       mbar_wait(bar, phase);

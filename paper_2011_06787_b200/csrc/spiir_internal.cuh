@@ -44,6 +44,8 @@ inline bool first_use_on_device(unsigned long long& mask) {
   } while (0)
 
 constexpr int kReplicas = 4;        // pre-shifted copies of each band's input (aligned LDS.128 for any delay)
+constexpr int kReplicas2 = 8;       // ... in a band whose launch is bound by shared-memory conflicts: copy r + 4 gives every
+                                    // filter a second choice of 16-byte bank group (bank.cu, placement)
 constexpr int kBankThreads = 256;   // threads per CTA of the recursion kernel
 constexpr int kBankWarps = kBankThreads / 32;
 constexpr int kSubChunkMax = 2048;  // samples of one band staged in shared memory at a time
@@ -67,6 +69,7 @@ struct BandDev {
   int32_t reps;           // floats per replica in shared memory ( = Hs + sub-chunk capacity )
   int32_t nsub;           // sub-chunk length for this call
   int32_t odd;            // 1: only odd samples are summed and stored, S[..][m] = s[2m+1] (band above the output rate)
+  int32_t nrep, pad;      // replicas of this band (4 or 8); samples of extra history in front of a staged row (0 or 4)
 };
 
 struct BankParams {
@@ -82,7 +85,7 @@ struct PrepParams {
   float* xnew[SPIIR_MAX_BANDS];        // replica 0 of detector 0, new parity
   const float* xold[SPIIR_MAX_BANDS];  // replica 0 of detector 0, old parity
   int64_t x_det_stride[SPIIR_MAX_BANDS];
-  int32_t cap[SPIIR_MAX_BANDS], Hcap[SPIIR_MAX_BANDS], n[SPIIR_MAX_BANDS], prev_n[SPIIR_MAX_BANDS];
+  int32_t cap[SPIIR_MAX_BANDS], Hcap[SPIIR_MAX_BANDS], n[SPIIR_MAX_BANDS], prev_n[SPIIR_MAX_BANDS], nrep[SPIIR_MAX_BANDS];
   const float* taps_dec;   // device [32]
 };
 
@@ -128,7 +131,7 @@ struct spiir_bank_host_band {
   int G = 0, F = 0;
   int n_units = 0, n_units_long = 0;         // padded to whole warps, short first
   int n_wu_short = 0, n_wu_long = 0;
-  int Hcap = 0, Hs = 0, cap = 0, reps = 0, nmax = 0, rate = 0;
+  int Hcap = 0, Hs = 0, cap = 0, reps = 0, nmax = 0, rate = 0, nrep = 4, pad = 0, nsubmax = 0;
   int64_t n_filters = 0;
   // workspace offsets (bytes)
   size_t off_coef2 = 0;
