@@ -59,6 +59,7 @@ __device__ __forceinline__ float re_prod(float2 x, float2 y) { return __fmaf_rn(
 // so the wait is bounded (seconds) and traps: the launch then fails with an error instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait_bounded(uint32_t bar_addr, uint32_t parity) {
   uint32_t done = 0;
+#pragma unroll 1
   for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
     asm volatile(
         "{\n"
