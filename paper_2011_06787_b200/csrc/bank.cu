@@ -3,6 +3,7 @@
 // (include/spiir.h documents the contract; DESIGN.md §3-§4 the layout.)
 #include <algorithm>
 #include <cstdarg>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <tuple>
