@@ -453,6 +453,13 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
   // unit in a band gets that row as ONE TMA bulk copy (thread 0 issues them, completion on an mbarrier: the
   // LSU path of per-thread cp.async tops out near 14 GB/s per SM here), more units are added up on the way
   __shared__ uint64_t cbar;
+  // the interpolator histories of every band, requested up front: read stage by stage they were six serialised
+  // global-memory latencies on the critical path of a CTA (long_scoreboard 3.9 per issue, profiles/r2 section 4)
+  __shared__ float2 hsm[SPIIR_MAX_BANDS][kUpHist + 1];
+  for (int i = tid; i < SPIIR_MAX_BANDS * kUpHist; i += kCombineThreads) {
+    const int b = i / kUpHist, j = i - b * kUpHist;
+    if (b > ob && b < B) hsm[b][j] = p.uphist[b][((size_t)det * p.T + t) * kUpHist + j];
+  }
   if (tid == 0) mbar_init(&cbar, 1);
   __syncthreads();
   if (tid == 0) {
@@ -483,7 +490,7 @@ __global__ void __launch_bounds__(kCombineThreads) k_combine(const __grid_consta
     const int n = p.n[b];
     const float2* sb = sbuf + p.sb_off[b];
     float2* hist = (b > ob) ? p.uphist[b] + ((size_t)det * p.T + t) * kUpHist : nullptr;
-    if (hist && tid < kUpHist) cur[tid] = hist[tid];
+    if (hist && tid < kUpHist) cur[tid] = hsm[b][tid];
     if (b == B - 1) {
       for (int m = tid; m < n; m += kCombineThreads) cur[kUpHist + m] = sb[m];
     } else {
