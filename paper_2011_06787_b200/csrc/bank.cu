@@ -65,7 +65,7 @@ static int validate(const spiir_bank_desc* d) {
   SPIIR_REQUIRE((d->n_templates + d->bank_size - 1) / d->bank_size <= 65535, "too many template banks");
   for (int64_t l = 0; l < d->n_filters; ++l) {
     const int b = d->host_band[l];
-    SPIIR_REQUIRE(b < d->n_bands, "filter %lld: band %d out of range", (long long)l, b);
+    SPIIR_REQUIRE(b >= 0 && b < d->n_bands, "filter %lld: band %d out of range", (long long)l, b);
     SPIIR_REQUIRE(d->host_delay[l] >= 0 && d->host_delay[l] <= d->max_delay[b],
                   "filter %lld: delay %d outside [0, max_delay[%d]=%d]", (long long)l, d->host_delay[l], b,
                   d->max_delay[b]);

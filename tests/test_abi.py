@@ -68,6 +68,12 @@ def test_workspace_query_and_bad_arguments(sp):
     def small_delay(d):
         d.max_delay[0] = 5                                  # filters with larger delays exist
     bad(small_delay)
+    def negative_band(d):
+        band = np.array(bank["band"], dtype=np.int32).copy()
+        band[3] = -1
+        negative_band.keep = band                            # the descriptor holds a bare pointer
+        d.host_band = band.ctypes.data
+    bad(negative_band)
     assert sp.spiir_bank_workspace_bytes(None, C.byref(n)) == sp.SPIIR_EINVAL
     # band rates must halve
     bank8 = workloads.random_bank(np.random.default_rng(0), 2, 16, [4096, 2048, 1000], out_band=1)
