@@ -735,7 +735,7 @@ def run_ours(args):
     roof_bank["flop_per_unit"] = "12 per filter-sample update (PAPER.md:135)"
     roof_sky = None
     if has_sky and evals:
-        roof_sky = alu_roofline("k_sky3 / k_sky (coherent search + slides, H5+H6)", FLOP_PER_EVAL * evals, ms_sky,
+        roof_sky = alu_roofline("k_sky (coherent search + slides, H5+H6)", FLOP_PER_EVAL * evals, ms_sky,
                                 2 * D * K if S else D * K, ffma_rate, traffic["k_sky"],
                                 issue_ops=6.5 * evals, executed_ops=5.5 * evals)
         roof_sky["flop_per_unit"] = ("11 per (candidate or candidate-slide, direction) evaluation: the six-term quadratic form "
