@@ -53,7 +53,7 @@ def build(force=False, verbose=False):
         failed = failed or p.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    subprocess.run([_nvcc(), "-shared", "-o", LIB] + objs, check=True)
+    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + objs, check=True)
     return LIB
 
 
