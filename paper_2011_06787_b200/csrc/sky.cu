@@ -356,7 +356,10 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
     // ---- then a warp rescans the winning chunk of each of its 2 K pairs, lane = slot (the chunks of four
     //      pairs are requested before the first is consumed): every lane forms its own direction's products
     //      from scratch, the first lane holding the maximum gives the direction, tot2 and null2 there (Eq. 10)
-    constexpr int PPW = NP / kSkyWarps, RB = (PPW % 4 == 0) ? 4 : 2;
+    //      The pairs of a warp are taken RB at a time in three passes — every pair's value first, then the five
+    //      shuffle steps of all RB maxima side by side, then the results — so that the shuffle latencies overlap.
+    constexpr int PPW = NP / kSkyWarps;
+    constexpr int RB = (PPW * (SW / 4) <= 16) ? PPW : ((PPW % 4 == 0) ? 4 : 2);
     for (int u0 = 0; u0 < PPW; u0 += RB) {
       float4 wv4[RB][SW / 4];
 #pragma unroll
@@ -366,13 +369,12 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c) wv4[u][c] = __ldg(sp + c);
       }
+      float cc[RB], cm[RB], tt[RB], q0[RB]; int px[RB], slot[RB], slide[RB], valid[RB];
 #pragma unroll
       for (int u = 0; u < RB; ++u) {
-      const int j = warp + (u0 + u) * kSkyWarps;
-      const PairInfo pi = pinfo[j];
-      if (pi.slot < 0) continue;
-      spiir_sky_result res; res.coh2 = 0.f; res.null2 = 0.f; res.tot2 = 0.f; res.pix = -1;
-      if (pi.valid) {
+        const int j = warp + (u0 + u) * kSkyWarps;
+        const PairInfo pi = pinfo[j];
+        slot[u] = pi.slot; slide[u] = pi.slide; valid[u] = pi.valid;
         float w[SW];
 #pragma unroll
         for (int c = 0; c < SW / 4; ++c) {
@@ -394,17 +396,27 @@ __global__ void __launch_bounds__(kSkyThreads, 1) k_sky(const __grid_constant__ 
           for (int o2 = 0; o2 < o; ++o2) qq[1 + 2 * NO + o * (o - 1) / 2 + o2] = re_prod(vv[o2], x);
           tot += xx;
         }
-        const float c = quad_form<NQ>(w, qq);
-        float cm = c;
-#pragma unroll
-        for (int o = 16; o; o >>= 1) cm = fmaxf(cm, __shfl_xor_sync(0xffffffffu, cm, o));
-        const int src = __ffs(__ballot_sync(0xffffffffu, c == cm)) - 1;
-        res.coh2 = __fmaf_rn(2.f, qq[0], cm);
-        res.tot2 = __shfl_sync(0xffffffffu, tot, src);
-        res.pix = __shfl_sync(0xffffffffu, __float_as_int(w[NQ]), src);
-        res.null2 = fmaxf(res.tot2 - res.coh2, 0.f);
+        cc[u] = quad_form<NQ>(w, qq); cm[u] = cc[u]; tt[u] = tot; q0[u] = qq[0]; px[u] = __float_as_int(w[NQ]);
       }
-      if (lane == 0) P.out[(size_t)pi.slot * S1 + (P.n_slides > 0 ? pi.slide - 1 : 0)] = res;
+#pragma unroll
+      for (int o = 16; o; o >>= 1) {
+#pragma unroll
+        for (int u = 0; u < RB; ++u) cm[u] = fmaxf(cm[u], __shfl_xor_sync(0xffffffffu, cm[u], o));
+      }
+#pragma unroll
+      for (int u = 0; u < RB; ++u) {
+        const int src = __ffs(__ballot_sync(0xffffffffu, cc[u] == cm[u])) - 1;
+        const float tot2 = __shfl_sync(0xffffffffu, tt[u], src);
+        const int pix = __shfl_sync(0xffffffffu, px[u], src);
+        if (slot[u] < 0) continue;
+        spiir_sky_result res; res.coh2 = 0.f; res.null2 = 0.f; res.tot2 = 0.f; res.pix = -1;
+        if (valid[u]) {
+          res.coh2 = __fmaf_rn(2.f, q0[u], cm[u]);
+          res.tot2 = tot2;
+          res.pix = pix;
+          res.null2 = fmaxf(res.tot2 - res.coh2, 0.f);
+        }
+        if (lane == 0) P.out[(size_t)slot[u] * S1 + (P.n_slides > 0 ? slide[u] - 1 : 0)] = res;
       }
     }
   }
