@@ -315,6 +315,35 @@ int spiir_rank_candidates(const void* dev_ws, const spiir_rank_bins* bins, const
                           const spiir_sky_result* dev_fg, const spiir_xi2_result* dev_xi, int32_t n_slots,
                           double background_seconds, spiir_rank_result* dev_out, void* stream);
 
+/* The ranking chain of Eq. 13-15 for callers that cannot give it a workspace.
+ * Who that is: a search process that reaches the ranking step after all device memory has gone to the filter
+ * banks' workspaces and SNR rings (a late cudaMalloc then fails, and where it succeeds it waits for, and holds up,
+ * everything in flight on the device — the filtering streams of a low-latency pipeline included), and code that
+ * runs inside a host process under a "no device allocation after start-up" rule.
+ * One call = spiir_rank_reset + spiir_rank_accumulate(dev_bg_trig, dev_bg, dev_bg_xi, n_bg_slots, n_slides) +
+ * spiir_rank_finalize + spiir_rank_candidates(dev_fg_trig, dev_fg, dev_fg_xi, n_fg_slots, background_seconds,
+ * dev_out), same kernels, same results bit for bit, with the histogram / R / FAP tables kept in an array that is
+ * part of the library image instead of a workspace.  The call itself allocates nothing and frees nothing.
+ *   Limit   : n_rho * n_xi <= SPIIR_RANK_STATIC_MAX_BINS, else SPIIR_EINVAL with a message that says so (use the
+ *             workspace calls above for finer binnings).  The array is (4 + 3 * 4096) * 8 = 98 336 bytes and every
+ *             GPU that loads the library holds it until the process exits.
+ *   Set-up  : the first call on each device looks the array's device address up (with that device current, as for
+ *             every call); make that first call before any stream capture is begun.
+ *   Sharing : one array per device for all callers and streams.  It keeps the last call's tables; the call clears
+ *             it before use.  Two calls that overlap on the same GPU (different streams, or different threads) race
+ *             on it and give garbage: order them on one stream or with events.
+ *   Background from several chunks cannot be accumulated across calls (each call starts from an empty histogram);
+ *   pass all events of the collection window in one call.  n_bg_slots = 0 gives an empty background (rank = fap =
+ *   far = 0 for every selected candidate); n_fg_slots = 0 only builds the tables.
+ *   All dev_* arrays are the caller's, laid out as for the calls above.  Asynchronous on `stream`.
+ *   Errors: EINVAL (bins, sizes, NULL pointers, too many bins), ECUDA. */
+#define SPIIR_RANK_STATIC_MAX_BINS 4096
+int spiir_rank_static(const spiir_rank_bins* bins, const spiir_trigger* dev_bg_trig, const spiir_sky_result* dev_bg,
+                      const spiir_xi2_result* dev_bg_xi, int32_t n_bg_slots, int32_t n_slides,
+                      const spiir_trigger* dev_fg_trig, const spiir_sky_result* dev_fg,
+                      const spiir_xi2_result* dev_fg_xi, int32_t n_fg_slots, double background_seconds,
+                      spiir_rank_result* dev_out, void* stream);
+
 /* NEXT-4 — the front end on the device (Sec. II A): FIR down-sampling of the raw
  * strain (16 384 -> 2048 Hz, N_FIR ~ 192 taps), frequency-domain whitening (Eq. 1) against the running median PSD
  * of the immediate past, and amplitude gating with zero padding on either side.  The paper describes the stage in

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     make_desc, Bank, SkyPlan, SkyPlanSet, SnrView, sky_table_build, sky_table_set_build, sky_table_nearest, upsample_windows,
     triggers_to_numpy, triggers_from_numpy, results_to_numpy,
     XI2_DTYPE, template_autocorr, signal_consistency, xi2_to_numpy,
-    RANK_DTYPE, spiir_rank_bins, Ranker, rank_to_numpy, spiir_frontend_desc, FrontEnd,
+    RANK_DTYPE, spiir_rank_bins, Ranker, rank_to_numpy, rank_static, SPIIR_RANK_STATIC_MAX_BINS, spiir_frontend_desc, FrontEnd,
     SPIIR_OK, SPIIR_EINVAL, SPIIR_ENOMEM, SPIIR_ECUDA, SPIIR_EOVERFLOW,
 )
 from . import binding as _b

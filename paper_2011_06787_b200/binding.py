@@ -103,6 +103,8 @@ _SIGNATURES = {
     "spiir_rank_finalize": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "spiir_rank_candidates": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
                                         C.c_double, C.c_void_p, C.c_void_p]),
+    "spiir_rank_static": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
+                                    C.c_void_p, C.c_void_p, C.c_int32, C.c_double, C.c_void_p, C.c_void_p]),
     "spiir_frontend_workspace_bytes": (C.c_int, [C.POINTER(spiir_frontend_desc), C.POINTER(C.c_size_t)]),
     "spiir_frontend_init": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(spiir_frontend_desc), C.c_void_p, C.c_size_t, C.c_void_p]),
     "spiir_frontend_reset": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -515,6 +517,28 @@ class Ranker:
         n = self.bins.n_rho * self.bins.n_xi
         shp = (self.bins.n_rho, self.bins.n_xi)
         return int(w[0]), w[4:4 + n].reshape(shp), w[4 + n:4 + 2 * n].reshape(shp), w[4 + 2 * n:4 + 3 * n].reshape(shp)
+
+
+SPIIR_RANK_STATIC_MAX_BINS = 4096
+
+
+def rank_static(bins, bg_trig, bg, bg_xi, n_bg_slots, n_slides, fg_trig, fg, fg_xi, n_fg_slots, background_seconds,
+                out=None):
+    """spiir_rank_static: Ranker.reset + accumulate + finalize + candidates in one call whose tables sit in an array
+    built into the library, for callers that cannot allocate a workspace on the device any more (all memory already
+    handed out, or a late cudaMalloc would stall the streams that are filtering).  `bins` = (n_rho, n_xi, u_rho_min,
+    u_rho_max, u_xi_min, u_xi_max) with n_rho * n_xi <= SPIIR_RANK_STATIC_MAX_BINS.  One array per GPU, shared by all
+    calls: do not let two calls overlap on the device.  Only `out` (the caller's result buffer, n_fg_slots x 16
+    bytes) is created here when it is not passed in."""
+    import torch
+    b = spiir_rank_bins(*bins)
+    if out is None:
+        out = torch.empty(n_fg_slots, 16, dtype=torch.uint8, device="cuda")
+    p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+    _check(lib().spiir_rank_static(C.cast(C.byref(b), C.c_void_p), p(bg_trig), p(bg), p(bg_xi), n_bg_slots, n_slides,
+                                   p(fg_trig), p(fg), p(fg_xi), n_fg_slots, float(background_seconds), p(out),
+                                   _stream()))
+    return out
 
 
 def rank_to_numpy(out):

@@ -18,6 +18,8 @@
 //   k_rank_lookup  thread = foreground candidate
 #include "spiir_internal.cuh"
 
+#include <mutex>
+
 namespace spiir {
 
 typedef unsigned long long u64;
@@ -195,6 +197,105 @@ int spiir_rank_candidates(const void* dev_ws, const spiir_rank_bins* bins, const
       dev_trig, dev_fg, dev_xi, n_slots, axis(bins->u_rho_min, bins->u_rho_max, bins->n_rho),
       axis(bins->u_xi_min, bins->u_xi_max, bins->n_xi), w.C, w.F, w.nb, background_seconds, dev_out);
   count_launch();
+  SPIIR_CUDA_OK(cudaGetLastError());
+  return SPIIR_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------
+// spiir_rank_static — the whole ranking chain in one call that needs no workspace from the caller.
+//
+// Every other spiir_rank_* call works on a workspace the caller has to allocate (histogram, R counts, FAP
+// counts).  An online search process cannot always do that when the ranking step is reached: by then it has
+// usually handed all of the GPU's memory to the filter banks' workspaces and SNR rings, so a late cudaMalloc
+// fails; and where it would succeed it serialises against all work in flight on the device and holds up the
+// filtering streams, which a low-latency pipeline cannot afford.  Plug-ins that run inside somebody else's
+// process under a "no device allocation after start-up" rule are in the same position.
+//
+// The tables therefore live in the array below, which is part of the library image: every GPU that loads
+// libspiir_b200.so carries these (4 + 3 * SPIIR_RANK_STATIC_MAX_BINS) * 8 = 98 336 bytes until the process exits.
+// There is ONE array per device, shared by every call whatever its stream, and it keeps what the last call left
+// in it; the call clears it first, and two calls that overlap on the same GPU race on it.
+//
+// g_rank_static is a device symbol.  In host code the name is only a handle: taking its address there does not
+// yield device memory (a kernel handed that value faults, or reads host memory where the GPU can reach it).  The
+// device address is asked for once per device with cudaGetSymbolAddress and kept in rank_static_ptr().
+namespace spiir {
+
+constexpr size_t kRankStaticWords = 4 + 3 * (size_t)SPIIR_RANK_STATIC_MAX_BINS;
+static __device__ __align__(256) u64 g_rank_static[kRankStaticWords];
+
+constexpr int kRankStaticMaxDevices = 64;
+
+// Device address of g_rank_static on the CURRENT device.  The first call on a device resolves the symbol (which
+// may make the runtime load the module there); later calls only read the cached pointer.
+static int rank_static_ptr(u64** out) {
+  static std::mutex mu;
+  static u64* ptr[kRankStaticMaxDevices] = {};
+  int dev = -1;
+  SPIIR_CUDA_OK(cudaGetDevice(&dev));
+  SPIIR_REQUIRE(dev >= 0 && dev < kRankStaticMaxDevices, "spiir_rank_static: device ordinal %d is outside 0..%d", dev,
+                kRankStaticMaxDevices - 1);
+  std::lock_guard<std::mutex> lock(mu);
+  if (ptr[dev] == nullptr) {
+    void* p = nullptr;
+    SPIIR_CUDA_OK(cudaGetSymbolAddress(&p, g_rank_static));
+    if (p == nullptr) {
+      set_error("spiir_rank_static: cudaGetSymbolAddress returned a null address on device %d", dev);
+      return SPIIR_ECUDA;
+    }
+    ptr[dev] = (u64*)p;
+  }
+  *out = ptr[dev];
+  return SPIIR_OK;
+}
+
+}  // namespace spiir
+
+extern "C" {
+
+int spiir_rank_static(const spiir_rank_bins* bins, const spiir_trigger* dev_bg_trig, const spiir_sky_result* dev_bg,
+                      const spiir_xi2_result* dev_bg_xi, int32_t n_bg_slots, int32_t n_slides,
+                      const spiir_trigger* dev_fg_trig, const spiir_sky_result* dev_fg,
+                      const spiir_xi2_result* dev_fg_xi, int32_t n_fg_slots, double background_seconds,
+                      spiir_rank_result* dev_out, void* stream) {
+  int rc = rank_check(bins);
+  if (rc) return rc;
+  const size_t n = rank_bins_total(bins);
+  SPIIR_REQUIRE(n <= (size_t)SPIIR_RANK_STATIC_MAX_BINS,
+                "spiir_rank_static: n_rho * n_xi = %zu bins exceed the built-in table of SPIIR_RANK_STATIC_MAX_BINS = %d; "
+                "use spiir_rank_accumulate / _finalize / _candidates with a workspace of your own",
+                n, SPIIR_RANK_STATIC_MAX_BINS);
+  SPIIR_REQUIRE(n_bg_slots >= 0 && n_slides >= 1 && n_fg_slots >= 0 && background_seconds > 0,
+                "bad n_bg_slots / n_slides / n_fg_slots / background_seconds");
+  const long long n_ev = (long long)n_bg_slots * n_slides;
+  SPIIR_REQUIRE(n_ev == 0 || (dev_bg_trig && dev_bg && dev_bg_xi), "a background pointer is NULL");
+  SPIIR_REQUIRE(n_fg_slots == 0 || (dev_fg_trig && dev_fg && dev_fg_xi && dev_out), "a foreground pointer is NULL");
+  u64* scratch = nullptr;
+  rc = rank_static_ptr(&scratch);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const RankWs w = rank_carve(scratch, bins);
+  const RankAxis ar = axis(bins->u_rho_min, bins->u_rho_max, bins->n_rho);
+  const RankAxis ax = axis(bins->u_xi_min, bins->u_xi_max, bins->n_xi);
+  // the array still holds the previous call's tables: N_b and the histogram are summed into, so they start at zero
+  // (R and FAP counts are overwritten in full by k_rank_rows / k_rank_fap, cleared all the same)
+  SPIIR_CUDA_OK(cudaMemsetAsync(scratch, 0, (4 + 3 * n) * sizeof(u64), st));
+  if (n_ev > 0) {
+    k_rank_hist<<<(unsigned)((n_ev + 255) / 256), 256, 0, st>>>(dev_bg_trig, dev_bg, dev_bg_xi, n_ev, n_slides, ar, ax,
+                                                                w.H, w.nb);
+    count_launch();
+  }
+  k_rank_rows<<<(bins->n_rho + 127) / 128, 128, 0, st>>>(w.H, w.C, bins->n_rho, bins->n_xi);
+  k_rank_cols<<<(bins->n_xi + 127) / 128, 128, 0, st>>>(w.C, bins->n_rho, bins->n_xi);
+  k_rank_fap<<<((int)n + kFapThreads - 1) / kFapThreads, kFapThreads, 0, st>>>(w.H, w.C, w.F, (int)n);
+  count_launch(3);
+  if (n_fg_slots > 0) {
+    k_rank_lookup<<<(n_fg_slots + 255) / 256, 256, 0, st>>>(dev_fg_trig, dev_fg, dev_fg_xi, n_fg_slots, ar, ax, w.C,
+                                                            w.F, w.nb, background_seconds, dev_out);
+    count_launch();
+  }
   SPIIR_CUDA_OK(cudaGetLastError());
   return SPIIR_OK;
 }
