@@ -127,7 +127,10 @@ int spiir_peaks(spiir_bank* bank, float snr_threshold, int32_t mode,
 /* A window onto complex SNR series: z(det,row,k) = dev_z[det*det_stride +
  * row*row_stride + (k mod ring_len)] (strides in complex elements), defined for
  * 0 <= row < n_rows and max(0, k_newest - ring_len + 1) <= k <= k_newest.  A trigger
- * slot whose tmpl is not a row of the view is treated as an empty slot.  48 bytes. */
+ * slot whose tmpl is not a row of the view is treated as an empty slot.  48 bytes.
+ * The struct carries no size or version field: zero-initialise it and set EVERY field (n_rows is the newest one; a
+ * view with n_rows outside 1..2^31-1, a NULL dev_z, ring_len < 1 or a negative stride is refused with SPIIR_EINVAL by
+ * every call that takes a view). */
 typedef struct {
   const spiir_c32* dev_z;
   int64_t det_stride, row_stride;
@@ -392,12 +395,16 @@ int64_t spiir_bank_updates_per_chunk(const spiir_bank* bank, int32_t n_samples);
 int64_t spiir_launch_count(void);
 
 /* Profiling aid for bench.py (off by default; the hot path records no events when
- * off): when enabled, every spiir_filter_chunk records CUDA events on the caller's
- * stream at its begin and end and around its recursion-kernel launches (k_bank).
+ * off).  spiir_bank_timing_enable(bank, n_chunks) with n_chunks >= 1 creates the
+ * CUDA events for n_chunks calls (the only place events are created — never inside
+ * spiir_filter_chunk) and switches recording on: each of the next n_chunks
+ * spiir_filter_chunk calls records events on the caller's stream at its begin and
+ * end and around its recursion-kernel launches (k_bank); further calls go
+ * unrecorded.  n_chunks = 0 switches it off.
  * spiir_bank_timing_read synchronises those events, returns the summed durations
  * (ms) of the recursion brackets and of the whole calls and the number of calls
- * recorded since the last read, and clears the record. */
-int spiir_bank_timing_enable(spiir_bank* bank, int32_t enable);
+ * recorded since the last read, and clears the record (the enabled count stands). */
+int spiir_bank_timing_enable(spiir_bank* bank, int32_t n_chunks);
 int spiir_bank_timing_read(spiir_bank* bank, double* ms_recursion, double* ms_chunk, int32_t* n_chunks);
 
 const char* spiir_last_error(void);

@@ -298,8 +298,9 @@ class Bank:
         _check(lib().spiir_bank_band_plan(self.h, band, C.byref(p)))
         return {f[0]: getattr(p, f[0]) for f in spiir_band_plan._fields_}
 
-    def timing_enable(self, on=True):
-        _check(lib().spiir_bank_timing_enable(self.h, 1 if on else 0))
+    def timing_enable(self, n_chunks):
+        """Record the next n_chunks filter_chunk calls (events are created here, not in the call); 0 = off."""
+        _check(lib().spiir_bank_timing_enable(self.h, int(n_chunks)))
 
     def timing_read(self):
         """(ms in the recursion kernels, ms in whole filter_chunk calls, number of calls) since the last read."""

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspiir_b200.so")
-SOURCES = ["bank.cu", "bank_kernels.cu", "peaks.cu", "sky.cu", "sky3.cu", "sky_table.cu", "xi2.cu", "rank.cu", "upsample.cu", "frontend.cu"]
+SOURCES = ["bank.cu", "bank_kernels.cu", "peaks.cu", "sky.cu", "sky_table.cu", "xi2.cu", "rank.cu", "upsample.cu", "frontend.cu"]
 HEADERS = [os.path.join(CSRC, "spiir_internal.cuh"), os.path.join(CSRC, "sky_internal.cuh"), os.path.join(HERE, "..", "include", "spiir.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]

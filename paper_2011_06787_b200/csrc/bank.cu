@@ -437,7 +437,16 @@ int spiir_bank_reset(spiir_bank* bk, void* stream) {
 
 int spiir_bank_timing_enable(spiir_bank* bk, int32_t enable) {
   SPIIR_REQUIRE(bk != nullptr, "bank is NULL");
+  SPIIR_REQUIRE(enable >= 0 && enable <= (1 << 20), "n_chunks %d out of range", enable);
+  // all events are created HERE, so that spiir_filter_chunk itself never creates anything (spiir.h: no allocation
+  // after init on the hot path): four per chunk to be recorded
+  while (bk->ev_pool.size() < (size_t)enable * 4) {
+    cudaEvent_t e;
+    SPIIR_CUDA_OK(cudaEventCreate(&e));
+    bk->ev_pool.push_back(e);
+  }
   bk->timing = enable != 0;
+  bk->ev_cap = (size_t)enable * 4;
   bk->ev_used = 0;
   return SPIIR_OK;
 }
@@ -507,25 +516,21 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     bd.odd = (b == 0 && d.out_band == 1) ? 1 : 0;
   }
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
-  if (bk->timing) {
-    while (bk->ev_pool.size() < bk->ev_used + 4) {
-      cudaEvent_t e;
-      SPIIR_CUDA_OK(cudaEventCreate(&e));
-      bk->ev_pool.push_back(e);
-    }
+  const bool timed = bk->timing && bk->ev_used + 4 <= bk->ev_cap;     // chunks beyond the enabled count go unrecorded
+  if (timed) {
     for (int i = 0; i < 4; ++i) ev[i] = bk->ev_pool[bk->ev_used + i];
     bk->ev_used += 4;
     SPIIR_CUDA_OK(cudaEventRecord(ev[0], st));
   }
   launch_prep(pp, D, st);
   SPIIR_CUDA_OK(cudaGetLastError());
-  if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[1], st));
+  if (timed) SPIIR_CUDA_OK(cudaEventRecord(ev[1], st));
   for (auto& g : bk->groups) {
     int rc = launch_bank_group(g.G, g.F, g.odd, P, (const CtaWork*)(bk->ws + g.off_work), (int)g.work.size(), D,
                                g.smem_bytes, st);
     if (rc) return rc;
   }
-  if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[2], st));
+  if (timed) SPIIR_CUDA_OK(cudaEventRecord(ev[2], st));
   CombineParams cp;
   memset(&cp, 0, sizeof(cp));
   for (int b = 0; b < B; ++b) {
@@ -555,7 +560,7 @@ int spiir_filter_chunk(spiir_bank* bk, const float* dev_strain, int32_t n_sample
     cp.sb_total += (cp.sb_n[b] + 1) & ~1;
   }
   { const int rcc = launch_combine(cp, D, st); if (rcc) return rcc; }
-  if (bk->timing) SPIIR_CUDA_OK(cudaEventRecord(ev[3], st));
+  if (timed) SPIIR_CUDA_OK(cudaEventRecord(ev[3], st));
 
   bk->parity = newp;
   for (int b = 0; b < B; ++b) bk->band[b].prev_n = n_samples >> b;

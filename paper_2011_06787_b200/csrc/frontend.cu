@@ -202,6 +202,11 @@ static void fe_layout(spiir_frontend* fe) {
   fe->smem = (size_t)fe->N * 8 + (size_t)fe->N / 2 * 8 + (size_t)(H + 1) * 4 + (size_t)d.n_taps * 4 + (size_t)(H + 2 * d.gate_pad) + 16;
 }
 
+// fe_layout's shared-memory formula at the largest shape fe_validate lets through (hop 4096 -> N 8192, 512 taps,
+// gate_pad hop / 2): 124 948 bytes, inside the 227 KB a CTA may opt in to.
+constexpr size_t kFeSmemMax = (size_t)8192 * 8 + (size_t)4096 * 8 + (size_t)(4096 + 1) * 4 + (size_t)512 * 4 +
+                              (size_t)(4096 + 2 * 2048) + 16;
+
 extern "C" {
 
 int spiir_frontend_workspace_bytes(const spiir_frontend_desc* desc, size_t* bytes) {
@@ -241,7 +246,6 @@ int spiir_frontend_init(spiir_frontend** out, const spiir_frontend_desc* desc, v
   if (e == cudaSuccess) e = cudaMemcpyAsync(fe->ws + fe->off_win, win.data(), (size_t)N * 4, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(fe->ws + fe->off_bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);       // the host images die with this scope
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_frontend, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fe->smem);
   if (e != cudaSuccess) { set_error("front-end set-up failed: %s", cudaGetErrorString(e)); delete fe; return SPIIR_ECUDA; }
   fe->d.host_taps = nullptr;
   rc = spiir_frontend_reset(fe, stream);
@@ -278,6 +282,13 @@ int spiir_frontend_chunk(spiir_frontend* fe, const float* dev_raw, float* dev_ou
   P.p_norm = (float)(2.0 / ((double)d.out_rate_hz * fe->sw2));
   P.half_fs = 0.5f * d.out_rate_hz;
   P.thr = d.gate_threshold;
+  // The opt-in shared-memory limit is a property of the FUNCTION on a device, not of this instance: it is set once
+  // per device, to what the largest valid descriptor needs, so that instances of different shapes never lower it
+  // for one another and a front end works on whichever device is current when it is run.
+  static unsigned long long configured = 0;
+  if (first_use_on_device(configured))
+    SPIIR_CUDA_OK(cudaFuncSetAttribute(k_frontend, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFeSmemMax));
+  SPIIR_REQUIRE(fe->smem <= kFeSmemMax, "front end needs %zu bytes of shared memory (> %zu)", fe->smem, kFeSmemMax);
   k_frontend<<<d.n_det, kFeThreads, fe->smem, (cudaStream_t)stream>>>(P);
   count_launch();
   SPIIR_CUDA_OK(cudaGetLastError());

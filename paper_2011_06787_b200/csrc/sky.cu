@@ -60,7 +60,7 @@ template <int D> struct SkyFmt {
 
 struct SkyParams {
   const float* stream; int32_t n_chunks;                      // this trigger detector's stream
-  int16_t cb[kSkyWarps + 1];                                  // chunks [cb[w], cb[w+1]) are warp w's share (balanced by cost)
+  int32_t cb[kSkyWarps + 1];                                  // chunks [cb[w], cb[w+1]) are warp w's share (balanced by cost)
   int32_t n_pix;
   const float2* z; int64_t det_stride, row_stride, ring_len, k_newest;
   const spiir_trigger* trig;
@@ -520,9 +520,9 @@ static void sky_build_stream(spiir_sky_plan* pl, int T, const float* u2, const i
     S.cb[0] = 0;
     for (int c = 0; c < n_chunks && wv < kSkyWarps; ++c) {
       acc += cost[c];
-      if (acc >= total * wv / kSkyWarps) S.cb[wv++] = (int16_t)(c + 1);
+      if (acc >= total * wv / kSkyWarps) S.cb[wv++] = c + 1;
     }
-    for (; wv <= kSkyWarps; ++wv) S.cb[wv] = (int16_t)n_chunks;
+    for (; wv <= kSkyWarps; ++wv) S.cb[wv] = n_chunks;
   }
   slots.assign((size_t)pl->cap_slots * SW, 0.f);
   for (int r = 0; r < pl->cap_slots; ++r) {
@@ -588,13 +588,6 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
   pl->ws = (char*)dev_workspace;
   cudaStream_t st = (cudaStream_t)stream;
   std::vector<float> slots;
-  // Which kernel three-detector plans run.  Default: the general kernel k_sky — measured equal to k_sky3 (sky3.cu) at
-  // 12 288 and 49 152 directions and faster on coarse grids (768 directions: 4.3 against 5.5 ms for the same 4.06 M
-  // events; profiles/r2_ncu_summary.md section 2).  SPIIR_SKY_KERNEL=three-detector selects k_sky3 (kept for its
-  // asynchronous staging pipeline and as the record of why restructuring did not pay: both are bound by the delivery of
-  // operands from shared memory).
-  const char* knob = getenv("SPIIR_SKY_KERNEL");
-  const bool force_general = !(knob && strcmp(knob, "three-detector") == 0);
   for (int T = 0; T < D; ++T) {
     spiir_sky_stream& S = pl->st[T];
     int ps = 0;
@@ -611,36 +604,20 @@ int spiir_sky_plan_init(spiir_sky_plan** out, int32_t n_det, int32_t n_pix, int3
     }
     if (ps % 4 == 0) ps += 2;               // ps / 2 odd: a half-warp's 16 blocks start on distinct bank pairs
     S.rows = ps; S.ps = ps;
-    S.k_max = 0; S.fmt3 = 0; S.k3 = 0;
-    if (D == 3 && !force_general) {
-      // three detectors: the stream walks the other detector with the narrower window fast (its windows are the
-      // ones kept in shared memory; on equal widths the higher index, as the general kernel does)
-      const int o0 = (T == 0) ? 1 : 0, o1 = (T == 2) ? 1 : 2;
-      const int If = (S.W[o0] < S.W[o1]) ? o0 : o1, Is = (If == o0) ? o1 : o0;
-      // four pairs per thread must fit: with two, the broadcast reads of the weights (per slot and warp, whatever the
-      // number of pairs) make the kernel shared-memory bound and the general kernel is faster (V1 as the trigger
-      // detector: 9.1 against 7.2 ms, profiles/r2_ncu_summary.md)
-      if (sky3_smem_bytes(S.W[If], 4) <= (size_t)kSkySmemMax) S.k3 = 4;
-      if (S.k3 && S.W[Is] < (1 << kSkyRowBits) && S.W[If] < (1 << kSkyRowBits) && pl->cap_slots / kSkyChunk < 32767) {
-        S.fmt3 = 1; S.I_s = Is; S.I_f = If;
-      }
+    S.k_max = 0;
+    for (int K = kSkyKMax; K >= 1; --K)
+      if (sky_smem_bytes(ps, pl->SW, K) <= (size_t)kSkySmemMax) { S.k_max = K; break; }
+    if (S.k_max == 0) {
+      set_error("delay span of trigger detector %d needs %zu bytes of shared memory (> %d)", T,
+                sky_smem_bytes(ps, pl->SW, 1), kSkySmemMax);
+      delete pl; return SPIIR_EINVAL;
     }
-    if (!S.fmt3) {
-      for (int K = kSkyKMax; K >= 1; --K)
-        if (sky_smem_bytes(ps, pl->SW, K) <= (size_t)kSkySmemMax) { S.k_max = K; break; }
-      if (S.k_max == 0) {
-        set_error("delay span of trigger detector %d needs %zu bytes of shared memory (> %d)", T,
-                  sky_smem_bytes(ps, pl->SW, 1), kSkySmemMax);
-        delete pl; return SPIIR_EINVAL;
-      }
-      if (ps >= (1 << kSkyRowBits)) {
-        set_error("delay span of trigger detector %d: %d window samples do not fit the control word", T, ps);
-        delete pl; return SPIIR_EINVAL;
-      }
+    if (ps >= (1 << kSkyRowBits)) {
+      set_error("delay span of trigger detector %d: %d window samples do not fit the control word", T, ps);
+      delete pl; return SPIIR_EINVAL;
     }
     S.bad_trace = 0;
-    if (S.fmt3) sky3_build_stream(pl, T, u2, delay, slots);
-    else        sky_build_stream(pl, T, u2, delay, slots);
+    sky_build_stream(pl, T, u2, delay, slots);
     if (S.bad_trace) {
       set_error("host_u2: the two columns of U2 must be orthonormal at every pixel (Eq. 27: left singular vectors)");
       delete pl; return SPIIR_EINVAL;
@@ -696,12 +673,11 @@ static int sky_launch_k(int K, const SkyParams& P, long long max_pairs, int num_
 static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_trigger* trig, int32_t n_slots,
                    int32_t n_slides, int64_t step, const int32_t* mult, spiir_sky_result* out, float* map,
                    cudaStream_t st) {
-  SPIIR_REQUIRE(pl && view && trig && out, "a pointer is NULL");
-  SPIIR_REQUIRE(view->dev_z && view->ring_len >= 1 && view->n_rows >= 1, "bad SNR view");
+  SPIIR_REQUIRE(pl && trig && out, "a pointer is NULL");
+  if (int rcv = check_snr_view(view)) return rcv;
   SPIIR_REQUIRE(n_slots >= 0 && n_slots <= pl->max_slots, "n_slots %d exceeds the plan's max_slots %d", n_slots,
                 pl->max_slots);
-  SPIIR_REQUIRE(n_slides >= 0, "n_slides < 0");
-  SPIIR_REQUIRE(n_slides == 0 || (mult != nullptr && step >= 0), "time slides need host_slide_mult and step >= 0");
+  if (int rcs = check_slides(n_slides, step, mult, pl->n_det)) return rcs;
   if (n_slots == 0) return SPIIR_OK;
   const int D = pl->n_det, S1 = n_slides > 0 ? n_slides : 1;
   int32_t* counts = (int32_t*)(pl->ws + pl->off_counts);
@@ -717,13 +693,6 @@ static int sky_run(spiir_sky_plan* pl, const spiir_snr_view* view, const spiir_t
   const long long max_pairs = (long long)n_slots * S1;
   for (int T = 0; T < D; ++T) {
     const spiir_sky_stream& S = pl->st[T];
-    if (S.fmt3) {
-      SPIIR_REQUIRE(view->ring_len < (1ll << 31), "ring_len must be below 2^31 samples");
-      int rc3 = sky3_launch(pl, T, view, lists + (size_t)T * pl->max_slots, counts, max_pairs, n_slides, step, mult, out,
-                            map, st);
-      if (rc3) return rc3;
-      continue;
-    }
     SkyParams P;
     memset(&P, 0, sizeof(P));
     P.stream = (const float*)(pl->ws + S.off_slots); P.n_chunks = S.n_chunks;

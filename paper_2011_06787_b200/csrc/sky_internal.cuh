@@ -1,5 +1,5 @@
-// Declarations shared by sky.cu (plan, binning, the general N_d = 2..4 kernel) and sky3.cu (the
-// three-detector kernel).  Nothing here is visible through include/spiir.h.
+// Declarations of the sky search (sky.cu: plan, binning, the N_d = 2..4 kernel) that other translation units may
+// need.  Nothing here is visible through include/spiir.h.
 #pragma once
 #include "spiir_internal.cuh"
 
@@ -21,7 +21,7 @@ struct __align__(16) SkyRec {
   int32_t k_ok, _pad;
 };
 
-// ---- PTX helpers common to both kernels
+// ---- PTX helpers
 __device__ __forceinline__ uint32_t sky_smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src_gmem) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sky_smem_u32(dst_smem)), "l"(src_gmem) : "memory");
@@ -87,11 +87,8 @@ struct spiir_sky_stream {                 // the direction stream of one trigger
   int lo[SPIIR_MAX_DET], W[SPIIR_MAX_DET], woff[SPIIR_MAX_DET];   // woff: offset of the detector's segment in a pair's block
   int ps = 0;                             // float2 elements of a pair's block (even)
   size_t off_slots = 0;
-  // three-detector kernel (sky3.cu): which of the two other detectors is walked slowly / fast by the stream,
-  // pairs per thread that fit shared memory (0: this trigger detector runs the general kernel)
-  int fmt3 = 0, I_s = 0, I_f = 0, k3 = 0;
   int bad_trace = 0;                      // set by the stream builders when U2 U2^T does not have trace 2
-  int16_t cb[17] = {0};                   // chunk boundaries of the 16 warps' shares, balanced by cost
+  int32_t cb[17] = {0};                   // chunk boundaries of the 16 warps' shares, balanced by cost (any n_pix: 32-bit)
 };
 
 struct spiir_sky_plan {
@@ -101,12 +98,3 @@ struct spiir_sky_plan {
   spiir_sky_stream st[SPIIR_MAX_DET];
   int num_sms = 148;
 };
-
-namespace spiir {
-// sky3.cu
-size_t sky3_smem_bytes(int W_f, int K);
-void sky3_build_stream(spiir_sky_plan* pl, int T, const float* u2, const int32_t* delay, std::vector<float>& slots);
-int sky3_launch(const spiir_sky_plan* pl, int T, const spiir_snr_view* view, const SkyRec* list, const int32_t* counts,
-                long long max_pairs, int32_t n_slides, int64_t step, const int32_t* mult, spiir_sky_result* out, float* map,
-                cudaStream_t st);
-}  // namespace spiir

@@ -43,6 +43,37 @@ inline bool first_use_on_device(unsigned long long& mask) {
     }                                                                               \
   } while (0)
 
+// A caller's spiir_snr_view, checked the same way by every entry point that takes one.  n_rows joined the struct
+// after its first five fields: a caller that fills only those on an uninitialised struct passes garbage there, and a
+// huge value would switch off the kernels' row test.  A trigger's tmpl is an int32, so no honest view has more rows
+// than that; strides are element counts and cannot be negative.  (No bound ties n_rows to det_stride: detector-
+// interleaved layouts with det_stride < row_stride are legitimate.)
+inline int check_snr_view(const spiir_snr_view* v) {
+  SPIIR_REQUIRE(v != nullptr, "view is NULL");
+  SPIIR_REQUIRE(v->dev_z != nullptr, "view: dev_z is NULL");
+  SPIIR_REQUIRE(v->ring_len >= 1, "view: ring_len %lld < 1", (long long)v->ring_len);
+  SPIIR_REQUIRE(v->n_rows >= 1 && v->n_rows <= 0x7fffffffLL,
+                "view: n_rows %lld outside 1..2^31-1 (zero-initialise spiir_snr_view and set every field)",
+                (long long)v->n_rows);
+  SPIIR_REQUIRE(v->det_stride >= 0 && v->row_stride >= 0, "view: negative stride");
+  return SPIIR_OK;
+}
+
+// Time-slide arguments common to the background search, xi^2 on slides and the slid windows:
+// the largest shift n_slides * step * |mult| must stay far inside int64 (2^40 samples is 17 years at 2048 Hz).
+inline int check_slides(int32_t n_slides, int64_t step, const int32_t* mult, int32_t n_det) {
+  SPIIR_REQUIRE(n_slides >= 0, "n_slides < 0");
+  if (n_slides == 0) return SPIIR_OK;
+  SPIIR_REQUIRE(mult != nullptr && step >= 0, "time slides need host_slide_mult and step >= 0");
+  SPIIR_REQUIRE(step <= (1ll << 40), "step_samples %lld is beyond 2^40", (long long)step);
+  for (int I = 0; I < n_det; ++I) {
+    const long long m = mult[I] < 0 ? -(long long)mult[I] : (long long)mult[I];
+    SPIIR_REQUIRE(m == 0 || step == 0 || (long long)n_slides * m <= (1ll << 40) / step,
+                  "slide shift n_slides * step_samples * |host_slide_mult[%d]| is beyond 2^40 samples", I);
+  }
+  return SPIIR_OK;
+}
+
 constexpr int kReplicas = 4;        // pre-shifted copies of each band's input (aligned LDS.128 for any delay)
 constexpr int kReplicas2 = 8;       // ... in a band whose launch is bound by shared-memory conflicts: copy r + 4 gives every
                                     // filter a second choice of 16-byte bank group (bank.cu, placement)
@@ -162,5 +193,5 @@ struct spiir_bank {
   // optional profiling (spiir_bank_timing_*): 4 events per chunk: call begin, k_bank begin/end, call end
   bool timing = false;
   std::vector<cudaEvent_t> ev_pool;
-  size_t ev_used = 0;
+  size_t ev_used = 0, ev_cap = 0;     // events handed out / enabled (4 per chunk), all created by spiir_bank_timing_enable
 };

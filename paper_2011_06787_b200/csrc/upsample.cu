@@ -120,10 +120,11 @@ static int upsample_run(const spiir_snr_view* view, int32_t n_det, const spiir_t
   size_t elems = 0;
   int rc = spiir_snr_upsample_elems(n_det, n_slots, factor, half_width, &elems);
   if (rc) return rc;
-  SPIIR_REQUIRE(view && view->dev_z && dev_trig && dev_out && dev_trig_out && out_view, "a pointer is NULL");
-  SPIIR_REQUIRE(view->ring_len >= 1 && view->k_newest >= 0 && view->n_rows >= 1, "bad view");
+  SPIIR_REQUIRE(dev_trig && dev_out && dev_trig_out && out_view, "a pointer is NULL");
+  if (int rcv = check_snr_view(view)) return rcv;
+  SPIIR_REQUIRE(view->k_newest >= 0, "view: k_newest < 0");
   SPIIR_REQUIRE(((uintptr_t)dev_out & 15) == 0, "dev_out must be 16-byte aligned");
-  SPIIR_REQUIRE(n_slides >= 0 && (n_slides == 0 || (mult && step >= 0)), "time slides need host_slide_mult and step >= 0");
+  if (int rcs = check_slides(n_slides, step, mult, n_det)) return rcs;
   const int S1 = n_slides > 0 ? n_slides : 1;
   SPIIR_REQUIRE((long long)n_slots * S1 <= 0x7fffffffLL, "too many rows");
   UpParams P;

@@ -98,13 +98,12 @@ int spiir_signal_consistency(const spiir_snr_view* view, int32_t n_det, int32_t 
                              const spiir_trigger* dev_trig, const spiir_sky_result* dev_sky, int32_t n_slots,
                              int32_t n_slides, int64_t step_samples, const int32_t* host_slide_mult,
                              const spiir_c32* dev_autocorr, int32_t n_j, spiir_xi2_result* dev_out, void* stream) {
-  SPIIR_REQUIRE(view && dev_delay && dev_trig && dev_sky && dev_autocorr && dev_out, "a pointer is NULL");
-  SPIIR_REQUIRE(view->dev_z && view->ring_len >= 1 && view->n_rows >= 1, "bad SNR view");
+  SPIIR_REQUIRE(dev_delay && dev_trig && dev_sky && dev_autocorr && dev_out, "a pointer is NULL");
+  if (int rcv = check_snr_view(view)) return rcv;
   SPIIR_REQUIRE(n_det >= 1 && n_det <= SPIIR_MAX_DET, "n_det %d out of range", n_det);
   SPIIR_REQUIRE(n_pix >= 1 && n_slots >= 0 && n_j >= 1, "bad n_pix / n_slots / n_j");
   SPIIR_REQUIRE(2 * (int64_t)n_j + 1 <= view->ring_len, "window of %d lags longer than the view", 2 * n_j + 1);
-  SPIIR_REQUIRE(n_slides >= 0 && (n_slides == 0 || (host_slide_mult && step_samples >= 0)),
-                "time slides need host_slide_mult and step >= 0");
+  if (int rcs = check_slides(n_slides, step_samples, host_slide_mult, n_det)) return rcs;
   if (n_slots == 0) return SPIIR_OK;
   Xi2Params P;
   P.z = (const float2*)view->dev_z; P.det_stride = view->det_stride; P.row_stride = view->row_stride;

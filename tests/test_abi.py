@@ -151,6 +151,44 @@ def test_upsample_window_sizing_and_argument_checks(sp):
     assert sp.lib().spiir_snr_upsample_windows(None, 3, None, 1, 2, 2, None, None, None, None) == sp.SPIIR_EINVAL
 
 
+def test_bad_views_and_slide_arguments_are_refused_before_any_device_work(sp):
+    """spiir_snr_view has no size field: a caller that leaves n_rows unset passes 0 or stack garbage.  Every entry
+    point that takes a view refuses n_rows outside 1..2^31-1, a NULL dev_z, ring_len < 1 and negative strides; slide
+    shifts that would overflow int64 are refused too.  The device pointers below are never dereferenced: the checks
+    come first (coherent_sky_search / timeslide_background need a plan, hence a device: their arm is in the -m gpu
+    test_sky_degenerate_inputs)."""
+    L = sp.lib()
+    fake = C.c_void_p(4096)                                                  # stands for device memory; not touched
+    mult = (C.c_int32 * 3)(1, 1, 1)
+    ov = sp.spiir_snr_view()
+
+    def xi2(view, n_slides=0, step=0, m=mult):
+        return L.spiir_signal_consistency(C.byref(view), 3, 768, fake, fake, fake, 4, n_slides, step, m, fake, 10, fake, None)
+
+    def ups(view, n_slides=1, step=10, m=mult):
+        return L.spiir_snr_upsample_windows_slides(C.byref(view), 3, fake, 4, n_slides, step, m, 2, 30, fake, fake,
+                                                   C.byref(ov), None)
+
+    def ups_fg(view):
+        return L.spiir_snr_upsample_windows(C.byref(view), 3, fake, 4, 2, 30, fake, fake, C.byref(ov), None)
+
+    good = dict(dev_z=4096, det_stride=1000, row_stride=100, ring_len=100, k_newest=99, n_rows=10)
+    for bad in (dict(n_rows=0), dict(n_rows=-3), dict(n_rows=1 << 31), dict(n_rows=0x7F7F7F7F7F7F7F7F), dict(dev_z=None),
+                dict(ring_len=0), dict(det_stride=-1), dict(row_stride=-100)):
+        v = sp.spiir_snr_view(**{**good, **bad})
+        for call in (xi2, ups, ups_fg):
+            assert call(v) == sp.SPIIR_EINVAL, (bad, call.__name__)
+            assert "view" in sp.last_error(), sp.last_error()
+    v = sp.spiir_snr_view(**good)
+    huge = (C.c_int32 * 3)(1, -(1 << 31), 1)
+    for call in (xi2, ups):
+        assert call(v, 100, 1 << 39, mult) == sp.SPIIR_EINVAL and "2^40" in sp.last_error()
+        assert call(v, 100, 1 << 20, huge) == sp.SPIIR_EINVAL and "2^40" in sp.last_error()
+        assert call(v, 1, 10, None) == sp.SPIIR_EINVAL
+        assert call(v, 1, -1, mult) == sp.SPIIR_EINVAL
+        assert call(v, -1, 10, mult) == sp.SPIIR_EINVAL
+
+
 def test_product_package_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2011_06787_b200")
     for dp, _, fs in os.walk(pkg):

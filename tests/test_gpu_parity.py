@@ -183,12 +183,7 @@ def _snippet_case(sp, n_rows, nside, n_windows, half, seed, gmst=0.7):
     return u2, delay, zc, zd, trig, truth
 
 
-@pytest.mark.parametrize("kernel", ["general", "three-detector"])
-def test_sky_foreground_and_signal_recovery(sp, U, kernel, monkeypatch):
-    if kernel == "three-detector":
-        monkeypatch.setenv("SPIIR_SKY_KERNEL", "three-detector")
-    else:
-        monkeypatch.delenv("SPIIR_SKY_KERNEL", raising=False)
+def test_sky_foreground_and_signal_recovery(sp, U):
     _sky_foreground_and_signal_recovery(sp, U)
 
 
@@ -215,13 +210,8 @@ def _sky_foreground_and_signal_recovery(sp, U):
     assert np.mean(res["coh2"][sig]) > 4 * np.mean(res["coh2"][~truth["is_signal"] & (trig["valid"] == 1)])
 
 
-@pytest.mark.parametrize("kernel", ["general", "three-detector"])
-def test_sky_time_slides(sp, U, kernel, monkeypatch):
+def test_sky_time_slides(sp, U):
     import torch
-    if kernel == "three-detector":                                           # k_sky3 (sky3.cu) instead of the default k_sky
-        monkeypatch.setenv("SPIIR_SKY_KERNEL", "three-detector")
-    else:
-        monkeypatch.delenv("SPIIR_SKY_KERNEL", raising=False)
     n_rows, S, half = 96, 7, 102
     W = 2 * half + 1
     u2, delay, zc, zd, trig, truth = _snippet_case(sp, n_rows, 16, S + 1, half, seed=22)
@@ -523,16 +513,11 @@ def _subset_trig(trig_rows, sel, D):
 
 
 # ------------------------------------------------------------------ views that are not 16-byte friendly
-@pytest.mark.parametrize("kernel", ["three-detector", "general"])
-def test_sky_unaligned_view(sp, U, kernel, monkeypatch):
+def test_sky_unaligned_view(sp, U):
     """A view whose rows are not 16-byte friendly (odd ring_len 501, base pointer 8 bytes past an aligned address):
-    the window staging cannot use TMA bulk copies and takes the 8-byte cp.async path of each kernel.  Foreground,
-    slides and a wrapped ring against O6 / O7, for the general kernel and (SPIIR_SKY_KERNEL=three-detector) k_sky3."""
+    the window staging cannot use TMA bulk copies and takes the 8-byte cp.async path.  Foreground, slides and a
+    wrapped ring against O6 / O7."""
     import torch
-    if kernel == "three-detector":
-        monkeypatch.setenv("SPIIR_SKY_KERNEL", "three-detector")
-    else:
-        monkeypatch.delenv("SPIIR_SKY_KERNEL", raising=False)
     cfg = workloads.config(1)
     u2, delay = _table(cfg, nside=8, gmst=1.1)
     D, rows, L, k_new, S, step = 3, 40, 501, 1300, 3, 90
@@ -557,6 +542,40 @@ def test_sky_unaligned_view(sp, U, kernel, monkeypatch):
     st_f = U.check_sky(fg, z, L, k_new, u2, delay, trig)
     st_b = U.check_sky(bg, z, L, k_new, u2, delay, trig, n_slides=S, step=step, mult=[1, 1, 1])
     assert st_f["n"] >= 30 and st_b["n"] >= 60 and (fg["pix"] == -1).sum() >= 2
+
+
+# ------------------------------------------------------------------ grids of more than 32 767 stream chunks
+def test_sky_grid_beyond_32767_chunks(sp, U):
+    """A table of 1 105 920 directions (34 560 chunks of 32: the warps' chunk shares no longer fit 16 bits, which an
+    earlier layout stored them in).  The table is the nside-32 one repeated 90 times, so by the tie rule of spiir.h
+    (tuples in increasing order, pixel index ascending within a tuple) every result — maximum, tot2, null2 AND pixel —
+    must be bit-identical to the 12 288-direction plan's, which the other tests hold against the oracle."""
+    import torch
+    cfg = workloads.config(1)
+    u2, delay = _table(cfg, nside=32, gmst=2.2)
+    reps = 90
+    u2_big, delay_big = np.tile(u2, (reps, 1, 1)), np.tile(delay, (reps, 1))
+    assert (len(u2_big) + 31) // 32 > 32767
+    D, rows, L, k_new, S, step = 3, 24, 400, 399, 2, 60
+    rng = np.random.default_rng(32767)
+    z = (rng.standard_normal((D, rows, L)) + 1j * rng.standard_normal((D, rows, L))).astype(np.complex64)
+    view = sp.SnrView(torch.from_numpy(np.ascontiguousarray(z).view(np.float32).reshape(D, rows, L, 2)).cuda())
+    view.c.k_newest = k_new
+    n = 48
+    trig = np.zeros(n, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1
+    trig["tmpl"] = rng.integers(0, rows, n); trig["det"] = np.arange(n) % D
+    trig["k"] = rng.integers(200, 360, n)
+    td = sp.triggers_from_numpy(trig)
+    small, big = sp.SkyPlan(u2, delay, max_slots=n), sp.SkyPlan(u2_big, delay_big, max_slots=n)
+    assert big.n_tuples == small.n_tuples
+    for run in (lambda pl: pl.search(view, td, n), lambda pl: pl.background(view, td, n, S, step, [1, 1, 1])):
+        a, b = sp.results_to_numpy(run(small)), sp.results_to_numpy(run(big))
+        torch.cuda.synchronize()
+        assert (a["pix"] >= 0).sum() >= n // 2
+        assert a.tobytes() == b.tobytes()
+    st = U.check_sky(sp.results_to_numpy(small.search(view, td, n)), z, L, k_new, u2, delay, trig)   # and the anchor itself
+    assert st["n"] >= n // 2
 
 
 # ------------------------------------------------------------------ degenerate inputs
@@ -591,6 +610,16 @@ def test_sky_degenerate_inputs(sp, U):
     assert np.all(res["coh2"] == 0) and np.all(res["tot2"] == 0) and np.all(res["null2"] == 0)
     zc = np.zeros((3, 16, L), np.complex64)
     U.check_sky(res, zc, L, L - 1, u2, delay, trig)
+    # a view whose n_rows was never set (0, or garbage beyond what an int32 tmpl can address) is refused, as are slide
+    # shifts that would overflow (tests/test_abi.py holds the same for the calls that need no plan)
+    for n_rows in (0, -1, 1 << 40):
+        bad = sp.SnrView(raw=sp.spiir_snr_view(zd.data_ptr(), 16 * L, L, L, L - 1, n_rows))
+        for call in (lambda: plan.search(bad, td, 16), lambda: plan.background(bad, td, 16, 3, 50, [1, 1, 1])):
+            with pytest.raises(sp.SpiirError) as ei:
+                call()
+            assert ei.value.code == sp.SPIIR_EINVAL and "n_rows" in str(ei.value)
+    with pytest.raises(sp.SpiirError):
+        plan.background(view, td, 16, 100, 1 << 39, [1, 1, 1])
 
 
 # ------------------------------------------------------------------ config 3 in FULL
@@ -1156,6 +1185,11 @@ def test_frontend_downsample_whiten_gate(sp, U, shape):
         rms = max(1.0, float(np.sqrt(np.mean(ref[:, sl] ** 2))))
         assert err[:, sl].max() <= 5e-3 * rms, (c, err[:, sl].max(), rms)
     assert 0.9 < got[:, 12 * H:][~zero_got[:, 12 * H:]].std() < (1.15 if nh >= 27 else 1.3)   # unit variance out (a short history biases 1 / S-hat up)
+    # a second front end of another shape, set up and run in between, must not disturb this one (the opt-in
+    # shared-memory limit belongs to the kernel, not to an instance: a smaller instance used to lower it)
+    other = sp.FrontEnd(1, workloads.frontend_taps(2, 16), decim=2, hop=256, n_hist=3, gate_pad=0, out_rate_hz=fs,
+                        gate_threshold=50.0)
+    other.chunk(xd[:1, :512].contiguous())
     # reset: the same stream again gives the same output bit for bit
     f.reset()
     o0 = f.chunk(xd[:, :H * R].contiguous())
@@ -1169,8 +1203,8 @@ def test_workspace_guard_bands(sp, U):
     """compute-sanitizer cannot be run on this pool (gpurun refuses it), so out-of-bounds WRITES are looked for
     directly: every buffer the library writes — the bank's workspace, the sky plan's workspace, the trigger / result /
     SNR outputs, the front end's workspace and output — is carved out of a larger allocation filled with a byte
-    pattern, the whole path runs (multirate bank with a long-delay template, both peak modes, the three-detector and
-    the general sky kernel with slides on a wrapped ring, xi^2, the front end), and the guard bands on both sides of
+    pattern, the whole path runs (multirate bank with a long-delay template, both peak modes, the sky
+    search with slides on a wrapped ring, xi^2, the front end), and the guard bands on both sides of
     every buffer must still hold the pattern."""
     import ctypes as C
     import torch
@@ -1203,12 +1237,7 @@ def test_workspace_guard_bands(sp, U):
     u2, delay = _table(cfg, nside=8, gmst=0.4)
     pb = C.c_size_t(0)
     plans = []
-    for kern in ("", "three-detector"):
-        import os
-        if kern:
-            os.environ["SPIIR_SKY_KERNEL"] = kern
-        else:
-            os.environ.pop("SPIIR_SKY_KERNEL", None)
+    for _ in range(1):
         assert L_.spiir_sky_plan_workspace_bytes(D, len(u2), D * T, C.byref(pb)) == 0
         _, pws = guarded(pb.value)
         ph = C.c_void_p()
@@ -1216,7 +1245,6 @@ def test_workspace_guard_bands(sp, U):
         assert L_.spiir_sky_plan_init(C.byref(ph), D, len(u2), D * T, u2c.ctypes.data_as(C.c_void_p),
                                       dlc.ctypes.data_as(C.c_void_p), C.c_void_p(pws), pb, st) == 0
         plans.append(ph)
-    os.environ.pop("SPIIR_SKY_KERNEL", None)
     S = 3
     _, p_fg = guarded(D * T * 16)
     _, p_bg = guarded(D * T * S * 16)
