@@ -659,6 +659,13 @@ def run_ours(args):
                    "note": "one CTA per detector, latency-bound by 2 x 13 barrier-separated FFT stages; not part of the timed step"}
         del fe_, raw, fo
 
+    # ---- NEXT-4, second half: the early-warning bank as a second workload — this config's bank
+    #      truncated at seeded cut-offs of 30-60 Hz (workloads.early_warning_bank): all filters in the bands of
+    #      <= 256 Hz, bands 0-3 empty.  Few updates per byte of state and SNR written: which resource binds?
+    ew_info = None
+    if rank == 0 and multirate and len(cfg["band_rates"]) == 8:
+        ew_info = early_warning_row(sp, workloads, torch, cfg, T, D, chunk, dec, itp, x_dev, dev)
+
     # ---- end to end: pinned host strain in, host candidates and results out, every step
     e2e = None
     if not args.no_e2e:
@@ -765,7 +772,8 @@ def run_ours(args):
         "per_step": {"updates": upd_chunk, "candidates": n_cand / K if has_sky else None,
                      "sky_evals": evals / K if has_sky else None, "searched_fraction": searched},
         "roofline": dict(dominant, other_kernel=other), "roofline_other": other, "pipe_probes": probes,
-        "next_rows": {"xi2": xi2_info, "rank": rank_info, "sub_sample_foreground": sub_info, "frontend": fe_info},
+        "next_rows": {"xi2": xi2_info, "rank": rank_info, "sub_sample_foreground": sub_info, "frontend": fe_info,
+                      "early_warning": ew_info},
         "background_on_paper_grid_nside8": bg8_info,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
@@ -777,6 +785,72 @@ def run_ours(args):
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def measured_hbm_gbs():
+    """HBM copy bandwidth of this pool's B200s from the driver-written MEASURED_PEAKS.json, else the profiling
+    guide's fallback (B200_PROFILING.md: ~6.5 TB/s measured copy rate); returns (GB/s, source)."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6500.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+def early_warning_row(sp, workloads, torch, cfg, T, D, chunk, dec, itp, x_dev, dev, n_warm=6, n_timed=20):
+    """bank stage (spiir_filter_chunk + spiir_peaks) on the early-warning variant of this config's bank, timed with
+    CUDA events outside the timed step.  Reports filter-sample updates/s, the FP32 lane fraction of the recursion
+    kernel and the algorithmic HBM bytes per chunk (coefficients once per detector as the kernel reads them, IIR
+    state read + written, SNR ring written) over the stage time against the measured copy bandwidth, and names the
+    larger of the two fractions as the binding resource."""
+    rng = np.random.default_rng(cfg["seed"] + 393)
+    full = workloads.random_bank(rng, T, cfg["filters_per_template"], cfg["band_rates"], cfg["out_band"], exact_norm=False)
+    ew = workloads.early_warning_bank(full, rng, exact_norm=False)
+    del full
+    n_filt = int(ew["tmpl_offset"][-1])
+    per_band = np.bincount(ew["band"], minlength=8)
+    bk = sp.Bank(ew, D, chunk, ring_len=2 * (chunk >> cfg["out_band"]), bank_size=1000, dec_taps=dec, int_taps=itp)
+    upd = bk.updates_per_chunk(chunk)
+    n_x = len(x_dev)
+    for j in range(n_warm):
+        bk.filter_chunk(x_dev[j % n_x]); bk.peaks(4.0, 0)
+    torch.cuda.synchronize()
+    bk.timing_enable(n_timed)
+    e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    e[0].record()
+    for j in range(n_timed):
+        bk.filter_chunk(x_dev[(n_warm + j) % n_x]); bk.peaks(4.0, 0)
+    e[1].record()
+    torch.cuda.synchronize()
+    ms = e[0].elapsed_time(e[1]) / n_timed
+    ms_rec, _, n_rec = bk.timing_read()
+    bk.timing_enable(0)
+    ms_rec /= max(1, n_rec)
+    n_out = chunk >> cfg["out_band"]
+    alg_bytes = D * n_filt * (20 + 16) + D * T * n_out * 8          # (float4 coef + int32 offset) + state r/w; ring write
+    hbm, hbm_src = measured_hbm_gbs()
+    gbs = alg_bytes / (ms * 1e-3) / 1e9
+    lane = 8.0 * upd / (ms_rec * 1e-3) / FP32_LANE_OPS_PER_S if ms_rec > 0 else None
+    lane_stage = 8.0 * upd / (ms * 1e-3) / FP32_LANE_OPS_PER_S
+    info = {"workload": "this config's bank truncated at seeded cut-offs of 30-60 Hz (PAPER.md:393): %d templates, %d filters "
+                        "(%.0f per template) in the bands of <= 256 Hz only, %d detectors" % (T, n_filt, n_filt / T, D),
+            "filters_per_band": [int(v) for v in per_band], "updates_per_chunk": int(upd),
+            "ms_per_chunk_bank_stage": ms, "ms_k_bank": ms_rec, "updates_per_s": upd / (ms * 1e-3),
+            "k_bank_updates_per_s": upd / (ms_rec * 1e-3) if ms_rec > 0 else None,
+            "algorithmic_bytes_per_chunk": int(alg_bytes), "achieved_GBps": gbs, "hbm_peak_GBps": hbm,
+            "hbm_peak_source": hbm_src, "hbm_frac": gbs / hbm,
+            "fp32_lane_frac_k_bank": lane, "fp32_lane_frac_stage": lane_stage,
+            "ms_other_kernels": ms - ms_rec,
+            "k_bank_hbm_frac": (D * n_filt * 36 / (ms_rec * 1e-3) / 1e9 / hbm) if ms_rec > 0 else None,
+            # k_bank alone: coefficients + state over its own time against its lane fraction; the stage: whichever of the
+            # two fractions is larger — when both are small the stage is bound by neither resource but by the fixed
+            # per-chunk cost of the decimator / cascade / ring kernels (ms_other_kernels), which does not shrink
+            # with the filter count
+            "binds_k_bank": ("hbm" if ms_rec > 0 and D * n_filt * 36 / (ms_rec * 1e-3) / 1e9 / hbm > (lane or 0) else "fp32 lanes"),
+            "binds_stage": ("hbm" if gbs / hbm > max(lane_stage, 0.5) else "fp32 lanes" if lane_stage > 0.5 else
+                            "neither (hbm_frac and fp32_lane_frac_stage both < 0.5): fixed per-chunk cost of k_prep + k_combine"),
+            "note": "not part of the timed step; diagonal noise normalisation (set-up time)"}
+    del bk
+    return info
 
 
 def len_groups(bk):

@@ -189,6 +189,35 @@ def test_bad_views_and_slide_arguments_are_refused_before_any_device_work(sp):
         assert call(v, -1, 10, mult) == sp.SPIIR_EINVAL
 
 
+def test_early_warning_bank_shape_and_host_planning(sp):
+    """workloads.early_warning_bank: only bands of <= 256 Hz keep filters, each filter below its
+    template's seeded cut-off, CSR consistent, the input bank untouched; the library's host-side planner accepts a
+    descriptor whose upper four bands are empty (no device needed for the workspace query)."""
+    rng = np.random.default_rng(7)
+    full = workloads.random_bank(rng, 30, 240, workloads.configs.RATES8, out_band=1, exact_norm=False)
+    before = {k: np.array(full[k]).copy() for k in ("a", "b", "delay", "band", "tmpl_offset")}
+    ew = workloads.early_warning_bank(full, rng, exact_norm=False)
+    for k, v in before.items():
+        assert np.array_equal(np.array(full[k]), v)
+    off = ew["tmpl_offset"]
+    assert off[0] == 0 and off[-1] == len(ew["a"]) == len(ew["b"]) == len(ew["delay"]) == len(ew["band"])
+    rates = np.array(ew["band_rates"], float)
+    assert ew["band"].min() >= 4 and rates[ew["band"]].max() <= 256
+    f = np.abs(np.angle(ew["a"].astype(np.complex128))) * rates[ew["band"]] / (2 * np.pi)
+    t_of = np.repeat(np.arange(30), np.diff(off))
+    assert np.all(f <= ew["f_cut"][t_of] + 1e-9) and np.all((ew["f_cut"] >= 30) & (ew["f_cut"] <= 60))
+    assert np.all(np.diff(ew["band"].astype(int))[np.diff(t_of) == 0] >= 0)           # still sorted by band inside a template
+    # every dropped filter is in a band above 256 Hz or above the cut-off: nothing else went missing
+    fa = np.abs(np.angle(full["a"].astype(np.complex128))) * rates[full["band"]] / (2 * np.pi)
+    want = (rates[full["band"]] <= 256) & (fa <= np.repeat(ew["f_cut"], 240))
+    assert want.sum() == len(ew["a"]) and np.array_equal(full["a"][want], ew["a"])
+    dec, itp = workloads.halfband_taps()
+    d, keep = sp.make_desc(ew, 3, 4096, 4096, 1000, dec, itp)
+    n = C.c_size_t(0)
+    assert sp.spiir_bank_workspace_bytes(C.byref(d), C.byref(n)) == sp.SPIIR_OK, sp.last_error()
+    assert n.value > 0
+
+
 def test_product_package_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2011_06787_b200")
     for dp, _, fs in os.walk(pkg):

@@ -146,6 +146,34 @@ def test_cfg2_shape_sample(sp, U):
     assert bk.updates_per_chunk(4096) == 2 * 16 * 75 * 8160
 
 
+# ------------------------------------------------------------------ early-warning bank (NEXT-4, second half)
+def test_early_warning_bank(sp, U):
+    """PAPER.md:393 (Sec. IV, early-warning configuration): templates truncated at a seeded cut-off of 30-60 Hz, so
+    that all of their filters sit in the bands of <= 256 Hz and bands 0-3 of the 8-band layout hold NO filter at all —
+    a shape the (lanes, filters-per-lane) chooser and the launch grouping never see in the other configs.  Streaming
+    in 1-s chunks against the one-shot oracle, peaks per chunk, ragged templates, chunk-split invariance."""
+    rng = np.random.default_rng(393)
+    full = workloads.random_bank(rng, 40, 700, workloads.configs.RATES8, out_band=1, exact_norm=False)
+    bank = workloads.early_warning_bank(full, rng, exact_norm=False)
+    per_band = np.bincount(bank["band"], minlength=8)
+    assert per_band[:4].sum() == 0 and per_band[4:].min() > 0
+    assert len(set(np.diff(bank["tmpl_offset"]).tolist())) > 10                 # ragged
+    dec, itp = workloads.halfband_taps()
+    x = workloads.gaussian_strain(rng, 2, 6 * 4096)
+    z_ref = oracle.filter_bank(x, bank, dec, itp)
+    z, trigs, bk = U.run_bank(bank, x, 4096, taps=(dec, itp), peak_thr=0.0)
+    U.check_snr(z, z_ref)
+    assert np.abs(z_ref[:, :, 2 * 2048:]).max() > 0.5                           # not a comparison of zeros
+    for c, (trig, cnt) in enumerate(trigs):
+        sl = slice(c * 2048, (c + 1) * 2048)
+        U.check_peaks_mode0(trig, z[:, :, sl], z_ref[:, :, sl], c * 2048, 0.0)
+    for b in range(4):
+        assert bk.band_plan(b)["n_filters"] == 0
+    assert bk.updates_per_chunk(4096) == 2 * sum(int(per_band[b]) * (4096 >> b) for b in range(8))
+    z2, _, _ = U.run_bank(bank, x, None, taps=(dec, itp), chunks=[512, 4096, 1024, 3584, 4096, 4096, 3072, 4096])
+    U.check_snr(z2, z_ref)
+
+
 # ------------------------------------------------------------------ peaks mode 1
 def test_peaks_mode1_paper_rule(sp, U):
     rng = np.random.default_rng(8)

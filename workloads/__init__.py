@@ -11,5 +11,5 @@ from .gen import (  # noqa: F401
     halfband_taps, detector_geometry, random_bank, chirp_waveform,
     chirp_matched_template, gaussian_strain, inject_chirp, snr_snippets,
     antenna_response, arrival_time, bank_for_config, strain_for_config,
-    C_LIGHT, frontend_taps, frontend_psd, frontend_strain,
+    C_LIGHT, frontend_taps, frontend_psd, frontend_strain, early_warning_bank,
 )

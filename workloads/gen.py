@@ -188,6 +188,53 @@ def random_bank(rng, n_templates, filters_per_template, band_rates, out_band=0,
     )
 
 
+def early_warning_bank(bank, rng, f_cut_range=(30.0, 60.0), max_rate_hz=256, exact_norm=True):
+    """Early-warning variant of a multirate ``random_bank`` ("the early-warning configuration of the
+    pipeline"): templates truncated before merger, so that a candidate exists while
+    the signal is still in band.  Every template gets a seeded cut-off f_c ~ U[f_cut_range] Hz and keeps only the
+    filters that (i) sit in a band of rate <= ``max_rate_hz`` and (ii) have a centre frequency arg(a) rate / (2 pi)
+    <= f_c; b is rescaled so that the truncated template has unit noise variance again (A8: E|z|^2 = 2 in the
+    steady state, i.e. once the longest delay line, 2047 samples of the 32 Hz band = 64 s, has filled).  The
+    result is ragged (CSR) and leaves the bands above ``max_rate_hz`` without any filter.  Returns the new bank dict
+    (plus ``f_cut`` [T]); the input is not modified."""
+    T = int(bank["n_templates"])
+    off = np.asarray(bank["tmpl_offset"])
+    L = int(off[1] - off[0]) if T else 0
+    assert np.array_equal(off, np.arange(T + 1, dtype=np.int64) * L), "needs the dense layout random_bank returns"
+    rates = np.asarray(bank["band_rates"], dtype=np.float64)
+    a = bank["a"].reshape(T, L).astype(np.complex128)
+    b = bank["b"].reshape(T, L).astype(np.complex128)
+    d = bank["delay"].reshape(T, L)
+    band = bank["band"].reshape(T, L)
+    f_cut = rng.uniform(*f_cut_range, size=T)
+    f_centre = np.abs(np.angle(a)) * rates[band] / (2.0 * np.pi)
+    keep = (rates[band] <= max_rate_hz) & (f_centre <= f_cut[:, None])
+    bz = np.where(keep, b, 0.0)
+    V = np.zeros(T)
+    for bi in range(len(rates)):                               # filters of a template are stored sorted by band
+        cols = np.nonzero(band[0] == bi)[0]
+        if cols.size == 0 or not keep[:, cols].any():
+            continue
+        sl = slice(cols[0], cols[-1] + 1)
+        # every band sees unit-variance noise (the decimation taps have unit noise gain, M2), as in random_bank
+        if exact_norm:
+            V += _noise_variance(a[:, sl], bz[:, sl], d[:, sl])
+        else:
+            V += np.sum(np.abs(bz[:, sl]) ** 2 / (1.0 - np.abs(a[:, sl]) ** 2), axis=1)
+    scale = np.where(V > 0, np.sqrt(2.0 / np.where(V > 0, V, 1.0)), 1.0)
+    b = b * scale[:, None]
+    counts = keep.sum(axis=1)
+    out = dict(bank)
+    out.update(
+        tmpl_offset=np.concatenate([[0], np.cumsum(counts)]).astype(np.int64),
+        a=bank["a"].reshape(T, L)[keep], b=b.astype(np.complex64)[keep],
+        delay=d[keep].astype(np.int32), band=band[keep].astype(np.uint8),
+        max_delay=list(bank["max_delay"]), f_cut=f_cut,
+    )
+    out.pop("chirp_overlap", None)
+    return out
+
+
 # --------------------------------------------------------------------------
 # Chirp (BASELINE.json config 1) and a naive SPIIR fit to it (generator only)
 # --------------------------------------------------------------------------
