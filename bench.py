@@ -70,11 +70,12 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (2 or 4 stream a bank)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (1, 2 or 4 stream a bank; 3 = sky search alone)")
     ap.add_argument("--templates", type=int, default=None, help="override the template count (debugging)")
     ap.add_argument("--slides", type=int, default=None, help="override the number of time slides")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cfg3", action="store_true", help="skip the config-3 sky-search row (about 15 s of set-up)")
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check after the timed region")
     ap.add_argument("--fast-norm", action="store_true",
                     help="diagonal approximation of the bank's noise normalisation (quicker set-up)")
@@ -402,6 +403,23 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     sp.lib()                                             # fails loudly if libspiir_b200.so is missing
 
+    if args.config == 3:
+        # the sky-search stress config has no filter bank: one line with the sky search alone (single GPU; the default
+        # line carries the same row as `sky_stress_cfg3`)
+        if rank == 0:
+            row = sky_stress_cfg3_row(sp, workloads, torch, reps=max(1, args.steps))
+            ms = row["ms_foreground"] + row["ms_slides"]
+            print(json.dumps({"metric": "spiir_sky_evals_per_s", "value": row["evals_per_s"], "unit": "evals/s", "n_gpus": 1,
+                              "steps": max(1, args.steps), "warmup": 1, "ms_per_step": ms, "higher_is_better": True,
+                              "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                              "config": {"workload": row["workload"], "l2": "no flush: 2 GB of snippets per pass"},
+                              "roofline": {"kernel": "k_sky", "bound": "alu", "achieved": FLOP_PER_EVAL * row["evals_per_s"] / 1e12,
+                                           "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": row["frac_of_fp32_peak"],
+                                           "traffic": None, "flop_per_unit": "9 executed per evaluation"},
+                              "sky_stress_cfg3": row}), flush=True)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     w = workload_params(args)
     cfg, T, S, D, chunk = w["cfg"], w["T"], w["S"], w["D"], w["chunk"]
     multirate = len(cfg["band_rates"]) > 1
@@ -666,6 +684,12 @@ def run_ours(args):
     if rank == 0 and multirate and len(cfg["band_rates"]) == 8:
         ew_info = early_warning_row(sp, workloads, torch, cfg, T, D, chunk, dec, itp, x_dev, dev)
 
+    # ---- BASELINE.json configs[3], the sky-search stress shape (4096 candidates on packed +-50 ms snippets, nside 64,
+    #      100 slides), sky search only, outside the timed step: the driver-run figure behind README's config-3 numbers
+    cfg3_info = None
+    if rank == 0 and has_sky and not args.no_cfg3:
+        cfg3_info = sky_stress_cfg3_row(sp, workloads, torch)
+
     # ---- end to end: pinned host strain in, host candidates and results out, every step
     e2e = None
     if not args.no_e2e:
@@ -774,7 +798,7 @@ def run_ours(args):
         "roofline": dict(dominant, other_kernel=other), "roofline_other": other, "pipe_probes": probes,
         "next_rows": {"xi2": xi2_info, "rank": rank_info, "sub_sample_foreground": sub_info, "frontend": fe_info,
                       "early_warning": ew_info},
-        "background_on_paper_grid_nside8": bg8_info,
+        "background_on_paper_grid_nside8": bg8_info, "sky_stress_cfg3": cfg3_info,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "setup_s": t_setup,
     }
     if world == 1 and not args.no_cpu_baseline:
@@ -850,6 +874,55 @@ def early_warning_row(sp, workloads, torch, cfg, T, D, chunk, dec, itp, x_dev, d
                             "neither (hbm_frac and fp32_lane_frac_stage both < 0.5): fixed per-chunk cost of k_prep + k_combine"),
             "note": "not part of the timed step; diagonal noise normalisation (set-up time)"}
     del bk
+    return info
+
+
+def sky_stress_cfg3_row(sp, workloads, torch, reps=3):
+    """coherent_sky_search + timeslide_background on BASELINE.json configs[3] exactly as tests/test_gpu_parity.py::
+    test_cfg3_full sets it up (there every one of the 4096 x 101 results is held against the oracle): seeded packed
+    snippets, library-built nside-64 table, 100 slides of one window each.  CUDA events around `reps` passes after one
+    warm-up pass; the 2 GB of snippets exceed the 126 MB L2."""
+    cfg = workloads.config(3)
+    n, S, half = cfg["n_triggers"], cfg["n_slides"], cfg["snippet_half"]
+    W = 2 * half + 1
+    pos, resp = workloads.detector_geometry(cfg["dets"])
+    u2, delay = sp.sky_table_build(cfg["nside"], pos, resp, cfg["sigma"], 0.7, 2048.0)
+    z, tdet, k, _ = workloads.snr_snippets(workloads.streams(cfg["seed"])["snippets"], u2, delay, n, S + 1, half,
+                                           cfg["coherent_fraction"])
+    trig = np.zeros(n, sp.TRIGGER_DTYPE)
+    trig["valid"] = 1; trig["tmpl"] = np.arange(n); trig["det"] = tdet; trig["k"] = k
+    zd = torch.from_numpy(z).cuda()
+    del z
+    plan = sp.SkyPlan(u2, delay, max_slots=n)
+    view = sp.SnrView(zd)
+    td = sp.triggers_from_numpy(trig)
+    fg = torch.empty(n, 16, dtype=torch.uint8, device="cuda")
+    bg = torch.empty(n * S, 16, dtype=torch.uint8, device="cuda")
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ms_f = ms_b = 0.0
+    for r in range(reps + 1):
+        ev[0].record()
+        plan.search(view, td, n, out=fg)
+        ev[1].record()
+        plan.background(view, td, n, S, W, [1] * len(cfg["dets"]), out=bg)
+        ev[2].record()
+        torch.cuda.synchronize()
+        if r:
+            ms_f += ev[0].elapsed_time(ev[1]) / reps
+            ms_b += ev[1].elapsed_time(ev[2]) / reps
+    res = sp.results_to_numpy(bg)
+    evals = float(n) * (1 + S) * len(u2)
+    rate = evals / ((ms_f + ms_b) * 1e-3)
+    info = {"workload": "BASELINE.json configs[3]: %d candidates, %d detectors, nside %d (%d directions), %d slides, packed "
+                        "snippets of %d samples" % (n, len(cfg["dets"]), cfg["nside"], len(u2), S, W),
+            "ms_foreground": ms_f, "ms_slides": ms_b, "evals": evals, "evals_per_s": rate,
+            "flop_per_eval_executed": FLOP_PER_EVAL, "frac_of_fp32_peak": FLOP_PER_EVAL * rate / 1e12 / FP32_PEAK_TFLOPS,
+            "fp32_lane_frac_executed": 5.5 * rate / FP32_LANE_OPS_PER_S,
+            "results_with_a_pixel": int((res["pix"] >= 0).sum()), "n_tuples": plan.n_tuples,
+            "parity": "the same inputs and calls as tests/test_gpu_parity.py::test_cfg3_full (all results vs the oracle)",
+            "note": "not part of the timed step"}
+    plan.close()
+    del zd, view, fg, bg
     return info
 
 
